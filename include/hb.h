@@ -1,0 +1,160 @@
+/*
+ * hb.h -- C ABI of libhb.so: B200-native (sm_100a) hybrid conventional/surrogate beamline push.
+ *
+ * Method: Sandberg et al., "Synthesizing Particle-in-Cell Simulations Through Learning and GPU
+ * Computing for Hybrid Particle Accelerator Beamlines", PASC'24 (arXiv 2402.17248).
+ * Citations "P:NN" are lines of PAPER.md; "R1..R10" / "G1..G17" are the readings in DESIGN.md.
+ *
+ * What one hb_push computes (every element, conventional or surrogate, is a per-particle
+ * map R^6 -> R^6, so the whole push is data-parallel over particles): an N-particle bunch, resident
+ * in device memory as six fp32 arrays (x, px, y, py, t, pt; s-based coordinates relative to a
+ * reference particle, R1), is pushed IN PLACE through the lattice:
+ *   - runs of conventional elements (drift R2, thick quadrupole R3, sector bend R4)
+ *     are fused into one pass over HBM per run;
+ *   - a surrogate stage is  [s->t conversion, R6]  ->  per-coordinate normalisation
+ *     (R8)  ->  MLP  F = L_l o sigma o ... o sigma o L_0  (Eq. 1-3, R9)  ->
+ *     de-normalisation  ->  [reference update R7, t->s conversion R6];
+ *   - a monitor records the bunch moments (R10) of the current state.
+ *
+ * Everything is extern "C"; no C++ or torch types cross the boundary.  Particle arrays and the
+ * moments buffer are DEVICE pointers borrowed for the duration of the enqueued work; every other
+ * pointer is a HOST pointer that is deep-copied before the call returns.  All device work is
+ * enqueued on the caller's stream; no entry point synchronises the device except
+ * hb_lattice_finalize (uploads) and hb_lattice_destroy.  There is no CPU fallback: without a
+ * usable sm_100 device the calls fail with HB_ERR_CUDA / HB_ERR_UNSUPPORTED.
+ */
+#ifndef HB_H
+#define HB_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hb_lattice hb_lattice; /* opaque; owned by the library */
+
+typedef enum {
+    HB_OK = 0,
+    HB_ERR_INVALID_ARG = 1, /* NULL / misaligned / aliasing pointers, non-finite or out-of-range values */
+    HB_ERR_STATE = 2,       /* adding to a finalized lattice, pushing a non-finalized one */
+    HB_ERR_ALLOC = 3,       /* host or device allocation failed */
+    HB_ERR_CUDA = 4,        /* a CUDA runtime call or a kernel launch failed (see hb_last_error) */
+    HB_ERR_UNSUPPORTED = 5  /* valid request the library has no kernel for (never a CPU fallback) */
+} hb_status;
+
+/* Conventional elements (formulas R2-R4).  MONITOR is the identity map that emits one
+ * 27-double moment record (R10) and splits runs (R5, G17). */
+typedef enum { HB_ELEM_DRIFT = 0, HB_ELEM_QUAD = 1, HB_ELEM_SBEND = 2, HB_ELEM_MONITOR = 3 } hb_elem_kind;
+
+/* Activation sigma of Eq. 3: identity; ReLU Eq. 1; PReLU Eq. 2, one learned
+ * slope per activation layer (G9); tanh (the "sigmoidal function" of P:90; BASELINE configs 1,4,5). */
+typedef enum { HB_ACT_IDENTITY = 0, HB_ACT_RELU = 1, HB_ACT_PRELU = 2, HB_ACT_TANH = 3 } hb_act;
+
+/* Arithmetic of the MLP layers.  FP32: CUDA-core FFMA.  BF16/F16/TF32: tcgen05 tensor cores with
+ * operands rounded to that type and fp32 accumulation in TMEM. */
+typedef enum { HB_PREC_FP32 = 0, HB_PREC_BF16 = 1, HB_PREC_F16 = 2, HB_PREC_TF32 = 3 } hb_prec;
+
+/* Coordinates the surrogate was trained in.  HB_COORD_S: the net sees (x,px,y,py,t,pt) as is.
+ * HB_COORD_T: the net sees fixed-time coordinates (x,y,z,ux,uy,uz), momenta in units of mc
+ * (P:60-62); the library converts s->t before and t->s after (R6) and moves the
+ * reference particle to the stage's output energy (R7; "about 7 GeV energy gain per stage"). */
+typedef enum { HB_COORD_S = 0, HB_COORD_T = 1 } hb_coord;
+
+/* How a run of conventional elements is applied.
+ * COMPOSED: the run's elements are concatenated on the host in fp64 into one 6x6 map (standard
+ *   transfer-matrix concatenation), rounded once to fp32 and applied in one HBM pass.
+ * SEQUENTIAL: the element list is applied one by one in fp64 registers, one rounding at the store.
+ * SEQUENTIAL_FP32: as SEQUENTIAL but in fp32 registers (literal reading of "fp32, element parameters
+ *   in constant or shared memory"); accumulates ~3e-8 relative per element -- see DESIGN.md. */
+typedef enum { HB_RUN_COMPOSED = 0, HB_RUN_SEQUENTIAL = 1, HB_RUN_SEQUENTIAL_FP32 = 2 } hb_run_mode;
+
+/* One surrogate stage (all pointers HOST pointers, deep-copied by hb_lattice_add_surrogate). */
+typedef struct {
+    int n_linear;            /* l+1 linear maps L_0..L_l; >= 1                                   */
+    const int *widths;       /* n_linear+1 entries: 6, H_1, ..., H_l, 6  (n = m = 6); 1<=H<=1024 */
+    const float *const *W;   /* n_linear matrices A_i, row-major [out][in]                               */
+    const float *const *b;   /* n_linear bias vectors b_i, [out]                                          */
+    hb_act act;              /* the same sigma after L_0..L_{l-1}, none after L_l (G7)         */
+    const float *prelu_a;    /* HB_ACT_PRELU: n_linear-1 slopes (one per activation layer, G9); else NULL */
+    double in_mean[6], in_std[6];   /* input normalisation  v^ = (v - mean)/std  (R8), std > 0    */
+    double out_mean[6], out_std[6]; /* output de-normalisation w = w^ * std + mean        */
+    hb_coord coord;
+    double ref_bg_out;       /* COORD_T: (beta gamma) of the reference after the stage; NaN = evaluate the
+                                net on the reference input (0,0,0,0,0,(beta gamma)_in) in fp64 on the host
+                                at finalize and take component uz (R7)                                    */
+    double ref_z_out;        /* COORD_T: reference z after the stage, subtracted from every particle's z;
+                                NaN = component z of the same host evaluation                            */
+    hb_prec prec;
+} hb_surrogate_desc;
+
+/* Create an empty lattice for a reference particle of the given kinetic and rest energy [MeV] (R1:
+ * gamma0 = 1 + T/mc^2).  Errors: NULL out, non-finite / non-positive energies -> INVALID_ARG. */
+hb_status hb_lattice_create(double ref_kinetic_energy_MeV, double rest_energy_MeV, hb_lattice **out);
+
+/* Append a conventional element.  length_m: DRIFT any finite value (negative allowed: the
+ * drift(L) o drift(-L) identity test needs it); QUAD, SBEND >= 0; MONITOR ignored.
+ * param: QUAD k [1/m^2] (k > 0 focuses x, R3); SBEND bend angle [rad], signed (R4); else ignored.
+ * Errors: finalized lattice -> STATE; non-finite or negative QUAD/SBEND length -> INVALID_ARG. */
+hb_status hb_lattice_add_element(hb_lattice *lat, hb_elem_kind kind, double length_m, double param);
+
+/* Append a surrogate stage; deep-copies every host array of *desc.
+ * Errors: widths[0] != 6 or widths[last] != 6, H outside [1,1024], std <= 0, non-finite values,
+ * PRELU without slopes -> INVALID_ARG; finalized lattice -> STATE. */
+hb_status hb_lattice_add_surrogate(hb_lattice *lat, const hb_surrogate_desc *desc);
+
+/* Choose how conventional runs are applied (default HB_RUN_COMPOSED).  Before finalize only. */
+hb_status hb_lattice_set_run_mode(hb_lattice *lat, hb_run_mode mode);
+
+/* Split the element list into segments (maximal runs of conventional elements; single surrogate
+ * stages; monitors), track the reference particle (R7), compose runs in fp64, pack the weights into
+ * the tensor-core operand layout, upload constants and allocate all scratch on `cuda_device`.
+ * Synchronises that device's uploads.  Errors: no such device / not sm_100 -> CUDA / UNSUPPORTED;
+ * a surrogate shape the library has no kernel for -> UNSUPPORTED; second call -> STATE. */
+hb_status hb_lattice_finalize(hb_lattice *lat, int cuda_device);
+
+/* Number of MONITOR elements (= moment records one push produces). */
+hb_status hb_lattice_num_monitors(const hb_lattice *lat, int *out);
+
+/* Number of kernel launches one hb_push / hb_push_moments enqueues (for launch accounting). */
+hb_status hb_lattice_num_launches(const hb_lattice *lat, int with_moments, int *out);
+
+/* (beta gamma) of the reference particle after the last element (valid after finalize). */
+hb_status hb_lattice_ref_bg_out(const hb_lattice *lat, double *out);
+
+/* Push n particles through the lattice in place.  x..pt: six DEVICE arrays of n floats each, 16-byte
+ * aligned, pairwise non-overlapping; borrowed until the enqueued work completes.  n >= 0 (0 is a
+ * no-op).  cuda_stream: a cudaStream_t (NULL = legacy default stream).  Returns after enqueueing;
+ * MONITOR elements are skipped.  Errors: not finalized -> STATE; NULL / misaligned / overlapping
+ * arrays -> INVALID_ARG; launch failure -> CUDA. */
+hb_status hb_push(hb_lattice *lat, float *x, float *px, float *y, float *py, float *t, float *pt,
+                  size_t n, void *cuda_stream);
+
+/* As hb_push, and writes one record of 27 doubles per MONITOR to d_moments (DEVICE, 8-byte aligned,
+ * num_monitors x 27): [0..5] means of (x,px,y,py,t,pt); [6..26] upper triangle, row-major, of the
+ * centred second moments with uniform weights and 1/N (R10, G11; sigma_x, eps_x of P:138, P:146
+ * follow from these).  Moments are accumulated in fp64 inside the kernel that produces the state
+ * (or by a standalone pass when a monitor has no producing kernel) and finished by a fixed-order
+ * reduction: deterministic, no floating-point atomics.  n = 0 writes NaN records. */
+hb_status hb_push_moments(hb_lattice *lat, float *x, float *px, float *y, float *py, float *t, float *pt,
+                          size_t n, double *d_moments, void *cuda_stream);
+
+/* Standalone moments of a bunch (R10).  pivot: 6 HOST doubles subtracted before accumulation (any
+ * value near the bunch centre; NULL = zeros); the result does not depend on it beyond rounding.
+ * d_out27: DEVICE, 27 doubles.  d_scratch: DEVICE scratch of hb_moments_scratch_bytes() bytes. */
+hb_status hb_moments(const float *x, const float *px, const float *y, const float *py, const float *t,
+                     const float *pt, size_t n, const double *pivot, double *d_out27, void *d_scratch,
+                     void *cuda_stream);
+size_t hb_moments_scratch_bytes(void);
+
+/* Destroy the lattice and free everything it owns (synchronises its device).  NULL is a no-op. */
+hb_status hb_lattice_destroy(hb_lattice *lat);
+
+const char *hb_status_string(hb_status s);
+const char *hb_last_error(void); /* thread-local message of the last failing call on this thread */
+const char *hb_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HB_H */

@@ -1,0 +1,322 @@
+"""ctypes marshalling for include/hb.h.  Same names as the C ABI; plus `Lattice`, a small RAII wrapper."""
+from __future__ import annotations
+
+import ctypes
+import math
+import os
+from ctypes import POINTER, c_char_p, c_double, c_float, c_int, c_size_t, c_void_p
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libhb.so")
+
+ELEM_KINDS = {"drift": 0, "quad": 1, "sbend": 2, "monitor": 3}
+ACTS = {"identity": 0, "relu": 1, "prelu": 2, "tanh": 3}
+PRECS = {"fp32": 0, "bf16": 1, "f16": 2, "tf32": 3}
+COORDS = {"s": 0, "t": 1}
+RUN_MODES = {"composed": 0, "sequential": 1, "sequential_fp32": 2}
+
+EXPORTED_SYMBOLS = [
+    "hb_lattice_create", "hb_lattice_add_element", "hb_lattice_add_surrogate", "hb_lattice_set_run_mode",
+    "hb_lattice_finalize", "hb_lattice_num_monitors", "hb_lattice_num_launches", "hb_lattice_ref_bg_out",
+    "hb_push", "hb_push_moments", "hb_moments", "hb_moments_scratch_bytes", "hb_lattice_destroy",
+    "hb_status_string", "hb_last_error", "hb_version",
+]
+
+
+class HbError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = int(status)
+        msg = "%s: %s (%s)" % (where, hb_status_string(status), hb_last_error())
+        super().__init__(msg)
+
+
+class _SurrogateDesc(ctypes.Structure):
+    _fields_ = [
+        ("n_linear", c_int),
+        ("widths", POINTER(c_int)),
+        ("W", POINTER(POINTER(c_float))),
+        ("b", POINTER(POINTER(c_float))),
+        ("act", c_int),
+        ("prelu_a", POINTER(c_float)),
+        ("in_mean", c_double * 6), ("in_std", c_double * 6),
+        ("out_mean", c_double * 6), ("out_std", c_double * 6),
+        ("coord", c_int),
+        ("ref_bg_out", c_double),
+        ("ref_z_out", c_double),
+        ("prec", c_int),
+    ]
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def lib():
+    """Load libhb.so (built in-tree by paper_2402_17248_b200/build.py).  Fails loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError("libhb.so is not built: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                          "(there is no CPU fallback)")
+    L = ctypes.CDLL(_LIB_PATH)
+    fp = POINTER(c_float)
+    L.hb_lattice_create.argtypes = [c_double, c_double, POINTER(c_void_p)]
+    L.hb_lattice_add_element.argtypes = [c_void_p, c_int, c_double, c_double]
+    L.hb_lattice_add_surrogate.argtypes = [c_void_p, POINTER(_SurrogateDesc)]
+    L.hb_lattice_set_run_mode.argtypes = [c_void_p, c_int]
+    L.hb_lattice_finalize.argtypes = [c_void_p, c_int]
+    L.hb_lattice_num_monitors.argtypes = [c_void_p, POINTER(c_int)]
+    L.hb_lattice_num_launches.argtypes = [c_void_p, c_int, POINTER(c_int)]
+    L.hb_lattice_ref_bg_out.argtypes = [c_void_p, POINTER(c_double)]
+    L.hb_push.argtypes = [c_void_p] + [c_void_p] * 6 + [c_size_t, c_void_p]
+    L.hb_push_moments.argtypes = [c_void_p] + [c_void_p] * 6 + [c_size_t, c_void_p, c_void_p]
+    L.hb_moments.argtypes = [c_void_p] * 6 + [c_size_t, POINTER(c_double), c_void_p, c_void_p, c_void_p]
+    L.hb_moments_scratch_bytes.restype = c_size_t
+    L.hb_moments_scratch_bytes.argtypes = []
+    L.hb_lattice_destroy.argtypes = [c_void_p]
+    L.hb_status_string.restype = c_char_p
+    L.hb_status_string.argtypes = [c_int]
+    L.hb_last_error.restype = c_char_p
+    L.hb_version.restype = c_char_p
+    for name in EXPORTED_SYMBOLS:
+        getattr(L, name)
+    _lib = L
+    return L
+
+
+# ------------------------------------------------------------------ C-ABI mirrors (argument marshalling only)
+def hb_status_string(status) -> str:
+    return lib().hb_status_string(int(status)).decode()
+
+
+def hb_last_error() -> str:
+    return lib().hb_last_error().decode()
+
+
+def hb_version() -> str:
+    return lib().hb_version().decode()
+
+
+def _check(status, where):
+    if status != 0:
+        raise HbError(status, where)
+
+
+def hb_lattice_create(ref_kinetic_energy_MeV: float, rest_energy_MeV: float):
+    h = c_void_p()
+    _check(lib().hb_lattice_create(ref_kinetic_energy_MeV, rest_energy_MeV, ctypes.byref(h)), "hb_lattice_create")
+    return h
+
+
+def hb_lattice_add_element(lat, kind, length_m: float = 0.0, param: float = 0.0):
+    k = ELEM_KINDS[kind] if isinstance(kind, str) else int(kind)
+    _check(lib().hb_lattice_add_element(lat, k, float(length_m), float(param)), "hb_lattice_add_element")
+
+
+def hb_lattice_add_surrogate(lat, widths, W, b, act, in_mean, in_std, out_mean, out_std, coord="s",
+                             prelu_a=None, ref_bg_out=float("nan"), ref_z_out=float("nan"), prec="fp32"):
+    nl = len(widths) - 1
+    Wc = [np.ascontiguousarray(w, dtype=np.float32) for w in W]
+    bc = [np.ascontiguousarray(x, dtype=np.float32) for x in b]
+    if len(Wc) != nl or len(bc) != nl:
+        raise ValueError("need %d weight matrices and biases" % nl)
+    for l in range(nl):
+        if Wc[l].shape != (widths[l + 1], widths[l]) or bc[l].shape != (widths[l + 1],):
+            raise ValueError("layer %d: W must be [out,in]=%s, b [out]" % (l, (widths[l + 1], widths[l])))
+    d = _SurrogateDesc()
+    d.n_linear = nl
+    wid = (c_int * (nl + 1))(*[int(w) for w in widths])
+    d.widths = ctypes.cast(wid, POINTER(c_int))
+    fp = POINTER(c_float)
+    Wp = (fp * nl)(*[w.ctypes.data_as(fp) for w in Wc])
+    bp = (fp * nl)(*[x.ctypes.data_as(fp) for x in bc])
+    d.W = ctypes.cast(Wp, POINTER(fp))
+    d.b = ctypes.cast(bp, POINTER(fp))
+    d.act = ACTS[act] if isinstance(act, str) else int(act)
+    a = None
+    if prelu_a is not None:
+        a = np.ascontiguousarray(prelu_a, dtype=np.float32)
+        d.prelu_a = a.ctypes.data_as(fp)
+    for name, src in (("in_mean", in_mean), ("in_std", in_std), ("out_mean", out_mean), ("out_std", out_std)):
+        arr = getattr(d, name)
+        for j in range(6):
+            arr[j] = float(src[j])
+    d.coord = COORDS[coord] if isinstance(coord, str) else int(coord)
+    d.ref_bg_out = float(ref_bg_out)
+    d.ref_z_out = float(ref_z_out)
+    d.prec = PRECS[prec] if isinstance(prec, str) else int(prec)
+    _check(lib().hb_lattice_add_surrogate(lat, ctypes.byref(d)), "hb_lattice_add_surrogate")
+
+
+def hb_lattice_set_run_mode(lat, mode):
+    m = RUN_MODES[mode] if isinstance(mode, str) else int(mode)
+    _check(lib().hb_lattice_set_run_mode(lat, m), "hb_lattice_set_run_mode")
+
+
+def hb_lattice_finalize(lat, cuda_device: int = 0):
+    _check(lib().hb_lattice_finalize(lat, int(cuda_device)), "hb_lattice_finalize")
+
+
+def hb_lattice_num_monitors(lat) -> int:
+    n = c_int()
+    _check(lib().hb_lattice_num_monitors(lat, ctypes.byref(n)), "hb_lattice_num_monitors")
+    return n.value
+
+
+def hb_lattice_num_launches(lat, with_moments: bool) -> int:
+    n = c_int()
+    _check(lib().hb_lattice_num_launches(lat, int(bool(with_moments)), ctypes.byref(n)), "hb_lattice_num_launches")
+    return n.value
+
+
+def hb_lattice_ref_bg_out(lat) -> float:
+    v = c_double()
+    _check(lib().hb_lattice_ref_bg_out(lat, ctypes.byref(v)), "hb_lattice_ref_bg_out")
+    return v.value
+
+
+def hb_push(lat, x, px, y, py, t, pt, n: int, cuda_stream: int = 0):
+    """x..pt: device addresses (ints).  Enqueues on cuda_stream and returns."""
+    _check(lib().hb_push(lat, x, px, y, py, t, pt, n, cuda_stream), "hb_push")
+
+
+def hb_push_moments(lat, x, px, y, py, t, pt, n: int, d_moments: int, cuda_stream: int = 0):
+    _check(lib().hb_push_moments(lat, x, px, y, py, t, pt, n, d_moments, cuda_stream), "hb_push_moments")
+
+
+def hb_moments_scratch_bytes() -> int:
+    return int(lib().hb_moments_scratch_bytes())
+
+
+def hb_moments(x, px, y, py, t, pt, n: int, pivot, d_out27: int, d_scratch: int, cuda_stream: int = 0):
+    pv = None
+    if pivot is not None:
+        pv = (c_double * 6)(*[float(v) for v in pivot])
+    _check(lib().hb_moments(x, px, y, py, t, pt, n, pv, d_out27, d_scratch, cuda_stream), "hb_moments")
+
+
+def hb_lattice_destroy(lat):
+    _check(lib().hb_lattice_destroy(lat), "hb_lattice_destroy")
+
+
+# ------------------------------------------------------------------ torch plumbing (pointers + streams only)
+def _rows(coords):
+    """coords: torch float32 CUDA tensor [6, n] (rows contiguous) or a sequence of six 1-D tensors."""
+    import torch
+    rows = [coords[j] for j in range(6)]
+    n = rows[0].numel()
+    for r in rows:
+        if not (isinstance(r, torch.Tensor) and r.is_cuda and r.dtype == torch.float32 and r.dim() == 1
+                and r.is_contiguous() and r.numel() == n):
+            raise ValueError("need six contiguous float32 CUDA vectors of equal length")
+    return rows, n
+
+
+def _stream(dev):
+    import torch
+    return torch.cuda.current_stream(dev).cuda_stream
+
+
+class Lattice:
+    """Owning wrapper of an hb_lattice.  `Lattice.from_description(desc)` consumes the plain-data lattice
+    description of workloads/ (also consumed, independently, by the oracle)."""
+
+    def __init__(self, kinetic_MeV: float, rest_MeV: float):
+        self._h = hb_lattice_create(kinetic_MeV, rest_MeV)
+        self.device = None
+
+    @classmethod
+    def from_description(cls, desc, run_mode="composed", device=0, prec=None, finalize=True):
+        lat = cls(desc["kinetic_MeV"], desc["rest_MeV"])
+        for el in desc["elements"]:
+            k = el["kind"]
+            if k == "drift":
+                lat.add_element("drift", el["L"])
+            elif k == "quad":
+                lat.add_element("quad", el["L"], el["k"])
+            elif k == "sbend":
+                lat.add_element("sbend", el["L"], el["theta"])
+            elif k == "monitor":
+                lat.add_element("monitor")
+            elif k == "surrogate":
+                lat.add_surrogate(el["widths"], el["W"], el["b"], el["act"], el["in_mean"], el["in_std"],
+                                  el["out_mean"], el["out_std"], coord=el["coord"], prelu_a=el.get("prelu_a"),
+                                  ref_bg_out=el["ref_bg_out"], ref_z_out=el["ref_z_out"],
+                                  prec=prec if prec is not None else el["prec"])
+            else:
+                raise ValueError(k)
+        lat.set_run_mode(run_mode)
+        if finalize:
+            lat.finalize(device)
+        return lat
+
+    def add_element(self, kind, length_m=0.0, param=0.0):
+        hb_lattice_add_element(self._h, kind, length_m, param)
+
+    def add_surrogate(self, *a, **k):
+        hb_lattice_add_surrogate(self._h, *a, **k)
+
+    def set_run_mode(self, mode):
+        hb_lattice_set_run_mode(self._h, mode)
+
+    def finalize(self, device=0):
+        hb_lattice_finalize(self._h, device)
+        self.device = device
+
+    @property
+    def num_monitors(self):
+        return hb_lattice_num_monitors(self._h)
+
+    def num_launches(self, with_moments):
+        return hb_lattice_num_launches(self._h, with_moments)
+
+    @property
+    def ref_bg_out(self):
+        return hb_lattice_ref_bg_out(self._h)
+
+    def push(self, coords):
+        rows, n = _rows(coords)
+        hb_push(self._h, *[r.data_ptr() for r in rows], n, _stream(rows[0].device))
+
+    def push_moments(self, coords, out=None):
+        import torch
+        rows, n = _rows(coords)
+        m = self.num_monitors
+        if out is None:
+            out = torch.empty((m, 27), dtype=torch.float64, device=rows[0].device)
+        hb_push_moments(self._h, *[r.data_ptr() for r in rows], n, out.data_ptr(), _stream(rows[0].device))
+        return out
+
+    def close(self):
+        if self._h is not None:
+            hb_lattice_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+_scratch = {}
+
+
+def moments(coords, pivot=None, out=None):
+    """Standalone bunch moments (27 doubles, R10) of a [6,n] float32 CUDA tensor."""
+    import torch
+    rows, n = _rows(coords)
+    dev = rows[0].device
+    if out is None:
+        out = torch.empty(27, dtype=torch.float64, device=dev)
+    key = (dev.index, _stream(dev))
+    if key not in _scratch:
+        _scratch[key] = torch.empty(hb_moments_scratch_bytes(), dtype=torch.uint8, device=dev)
+    hb_moments(*[r.data_ptr() for r in rows], n, pivot, out.data_ptr(), _scratch[key].data_ptr(), _stream(dev))
+    return out

@@ -1,0 +1,626 @@
+// hb_api.cu -- the C ABI of include/hb.h: lattice construction, reference tracking (R1, R7), fp64
+// composition of conventional runs (R2-R5), weight packing, segment sequencing (row a7).
+// Host code only; kernels live in hb_run.cu / hb_sur_fp32.cu / hb_sur_tc.cu.
+#include "../../include/hb.h"
+#include "hb_internal.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+namespace {
+
+thread_local std::string g_err;
+
+hb_status fail(hb_status s, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return s;
+}
+
+#define HB_CUDA(call)                                                                              \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) return fail(HB_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_));  \
+    } while (0)
+
+struct Elem {
+    int kind;        // hb_elem_kind, or 4 = surrogate
+    double L, param;
+    int sur;         // index into surrogates
+};
+
+struct SurHost {
+    int n_linear;
+    std::vector<int> widths;
+    std::vector<std::vector<float>> W, b;
+    int act;
+    std::vector<float> prelu;
+    double in_mean[6], in_std[6], out_mean[6], out_std[6];
+    int coord;
+    double ref_bg_out, ref_z_out;
+    int prec;
+};
+
+enum SegType { SEG_RUN = 0, SEG_SUR = 1, SEG_MON = 2 };
+
+struct Segment {
+    int type;
+    HbRunMap map;          // SEG_RUN composed
+    int seq_off, seq_cnt;  // SEG_RUN sequential: range in d_seq
+    HbSurDev sd;           // SEG_SUR
+    bool tc;               // SEG_SUR: tensor-core kernel
+    int monitor;           // record index written after this segment, -1 = none
+};
+
+// ---- fp64 6x6 helpers (transfer-matrix concatenation, R5) ---------------------------------
+struct Mat6 { double m[6][6]; };
+
+Mat6 mat_identity() {
+    Mat6 r;
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) r.m[i][j] = i == j ? 1.0 : 0.0;
+    return r;
+}
+
+Mat6 mat_mul(const Mat6& a, const Mat6& b) {   // a * b
+    Mat6 r;
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) {
+            double s = 0.0;
+            for (int k = 0; k < 6; ++k) s += a.m[i][k] * b.m[k][j];
+            r.m[i][j] = s;
+        }
+    return r;
+}
+
+// sin(x)/x and (1-cos x)/x without a branch on x == 0 in the result (series for tiny |x|)
+double sinc_(double x) { return std::fabs(x) < 1e-6 ? 1.0 - x * x / 6.0 : std::sin(x) / x; }
+double cosc_(double x) {   // (1 - cos x)/x = sin^2(x/2)/(x/2)
+    const double h = 0.5 * x;
+    return std::sin(h) * sinc_(h);
+}
+
+// element matrix in the lattice's s-coordinates (x,px,y,py,t,pt); bg = (beta gamma) of the reference
+Mat6 elem_matrix(const Elem& e, double bg) {
+    Mat6 M = mat_identity();
+    const double L = e.L;
+    const double r56 = L / (bg * bg);
+    if (e.kind == HB_ELEM_DRIFT) {
+        M.m[0][1] = L; M.m[2][3] = L; M.m[4][5] = r56;
+    } else if (e.kind == HB_ELEM_QUAD) {
+        const double k = e.param, w = std::sqrt(std::fabs(k)), ph = w * L;
+        // focusing plane: [cos, sin/w; -w sin, cos]; defocusing: [cosh, sinh/w; w sinh, cosh]
+        double f[4], d[4];
+        f[0] = std::cos(ph); f[1] = L * sinc_(ph); f[2] = -w * std::sin(ph); f[3] = f[0];
+        d[0] = std::cosh(ph);
+        d[1] = ph < 1e-6 ? L * (1.0 + ph * ph / 6.0) : std::sinh(ph) / w;
+        d[2] = w * std::sinh(ph); d[3] = d[0];
+        const double* X = k >= 0 ? f : d;
+        const double* Y = k >= 0 ? d : f;
+        M.m[0][0] = X[0]; M.m[0][1] = X[1]; M.m[1][0] = X[2]; M.m[1][1] = X[3];
+        M.m[2][2] = Y[0]; M.m[2][3] = Y[1]; M.m[3][2] = Y[2]; M.m[3][3] = Y[3];
+        M.m[4][5] = r56;
+    } else if (e.kind == HB_ELEM_SBEND) {
+        const double th = e.param;
+        const double g = std::sqrt(1.0 + bg * bg), b0 = bg / g;
+        const double s = std::sin(th), c = std::cos(th);
+        const double rs = L * sinc_(th);        // rho sin(theta)
+        const double rc = L * cosc_(th);        // rho (1 - cos theta)
+        const double h_s = th == 0.0 ? 0.0 : s * th / L;   // sin(theta)/rho
+        M.m[0][0] = c;    M.m[0][1] = rs;  M.m[0][5] = -rc / b0;
+        M.m[1][0] = -h_s; M.m[1][1] = c;   M.m[1][5] = -s / b0;
+        M.m[2][3] = L;
+        M.m[4][0] = s / b0; M.m[4][1] = rc / b0;
+        // rho(-theta + sin(theta)/b0^2) = -L + rs/b0^2 = L(1-b0^2)/b0^2 - (L - rs)/b0^2 ; 1-b0^2 = 1/g^2
+        M.m[4][5] = L / (bg * bg) - (L - rs) / (b0 * b0);
+    }
+    return M;
+}
+
+HbSeqElem seq_elem(const Elem& e, double bg) {
+    const Mat6 M = elem_matrix(e, bg);
+    HbSeqElem s;
+    std::memset(&s, 0, sizeof s);
+    s.kind = e.kind;
+    if (e.kind == HB_ELEM_DRIFT) {
+        s.a[0] = e.L; s.a[1] = M.m[4][5];
+    } else if (e.kind == HB_ELEM_QUAD) {
+        s.a[0] = M.m[0][0]; s.a[1] = M.m[0][1]; s.a[2] = M.m[1][0]; s.a[3] = M.m[1][1];
+        s.a[4] = M.m[2][2]; s.a[5] = M.m[2][3]; s.a[6] = M.m[3][2]; s.a[7] = M.m[3][3];
+        s.a[8] = M.m[4][5];
+    } else {
+        s.a[0] = M.m[0][0]; s.a[1] = M.m[0][1]; s.a[2] = M.m[1][0]; s.a[3] = M.m[1][1];
+        s.a[4] = M.m[0][5]; s.a[5] = M.m[1][5]; s.a[6] = M.m[2][3];
+        s.a[7] = M.m[4][0]; s.a[8] = M.m[4][1]; s.a[9] = M.m[4][5];
+    }
+    return s;
+}
+
+double act_host(double z, int act, double a) {
+    switch (act) {
+    case HB_ACT_RELU: return z >= 0 ? z : 0.0;
+    case HB_ACT_PRELU: return z >= 0 ? z : a * z;
+    case HB_ACT_TANH: return std::tanh(z);
+    default: return z;
+    }
+}
+
+// fp64 host evaluation of the net on one vector (R7: reference particle through a COORD_T stage)
+void mlp_host(const SurHost& s, const double in[6], double out[6]) {
+    std::vector<double> h(in, in + 6), g;
+    for (int j = 0; j < 6; ++j) h[j] = (in[j] - s.in_mean[j]) / s.in_std[j];
+    for (int l = 0; l < s.n_linear; ++l) {
+        const int fin = s.widths[l], fout = s.widths[l + 1];
+        g.assign(fout, 0.0);
+        for (int o = 0; o < fout; ++o) {
+            double acc = 0.0;
+            for (int k = 0; k < fin; ++k) acc += (double)s.W[l][(size_t)o * fin + k] * h[k];
+            acc += (double)s.b[l][o];
+            if (l < s.n_linear - 1) acc = act_host(acc, s.act, s.act == HB_ACT_PRELU ? (double)s.prelu[l] : 0.0);
+            g[o] = acc;
+        }
+        h.swap(g);
+    }
+    for (int j = 0; j < 6; ++j) out[j] = h[j] * s.out_std[j] + s.out_mean[j];
+}
+
+void split_hi_lo(double v, float& hi, float& lo) {
+    hi = (float)v;
+    lo = (float)(v - (double)hi);
+}
+
+}  // namespace
+
+struct hb_lattice {
+    double kinetic, rest;
+    double gamma0, bg0;
+    std::vector<Elem> elems;
+    std::vector<SurHost> surs;
+    int run_mode = HB_RUN_COMPOSED;
+    bool finalized = false;
+    int device = -1;
+    int sm_count = 0;
+    int n_monitors = 0;
+    double bg_out = 0.0;
+    std::vector<Segment> segs;
+    // device allocations
+    HbSeqElem* d_seq = nullptr;
+    double* d_partials = nullptr;
+    std::vector<void*> d_bufs;
+};
+
+extern "C" {
+
+const char* hb_status_string(hb_status s) {
+    switch (s) {
+    case HB_OK: return "HB_OK";
+    case HB_ERR_INVALID_ARG: return "HB_ERR_INVALID_ARG";
+    case HB_ERR_STATE: return "HB_ERR_STATE";
+    case HB_ERR_ALLOC: return "HB_ERR_ALLOC";
+    case HB_ERR_CUDA: return "HB_ERR_CUDA";
+    case HB_ERR_UNSUPPORTED: return "HB_ERR_UNSUPPORTED";
+    }
+    return "HB_ERR_UNKNOWN";
+}
+
+const char* hb_last_error(void) { return g_err.c_str(); }
+const char* hb_version(void) { return "hb 0.1 (sm_100a)"; }
+
+hb_status hb_lattice_create(double kin, double rest, hb_lattice** out) {
+    if (!out) return fail(HB_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (!std::isfinite(kin) || !std::isfinite(rest) || kin <= 0.0 || rest <= 0.0)
+        return fail(HB_ERR_INVALID_ARG, "energies must be finite and positive");
+    hb_lattice* l = new (std::nothrow) hb_lattice();
+    if (!l) return fail(HB_ERR_ALLOC, "out of host memory");
+    l->kinetic = kin;
+    l->rest = rest;
+    l->gamma0 = 1.0 + kin / rest;                         // R1
+    l->bg0 = std::sqrt(l->gamma0 * l->gamma0 - 1.0);
+    *out = l;
+    return HB_OK;
+}
+
+hb_status hb_lattice_add_element(hb_lattice* lat, hb_elem_kind kind, double L, double param) {
+    if (!lat) return fail(HB_ERR_INVALID_ARG, "lattice is NULL");
+    if (lat->finalized) return fail(HB_ERR_STATE, "lattice already finalized");
+    if ((int)kind < 0 || (int)kind > HB_ELEM_MONITOR) return fail(HB_ERR_INVALID_ARG, "unknown element kind %d", (int)kind);
+    Elem e{(int)kind, 0.0, 0.0, -1};
+    if (kind != HB_ELEM_MONITOR) {
+        if (!std::isfinite(L)) return fail(HB_ERR_INVALID_ARG, "length must be finite");
+        if (kind != HB_ELEM_DRIFT && (!std::isfinite(param) || L < 0.0))
+            return fail(HB_ERR_INVALID_ARG, "quad/sbend need a finite parameter and length >= 0");
+        e.L = L;
+        e.param = kind == HB_ELEM_DRIFT ? 0.0 : param;
+    }
+    lat->elems.push_back(e);
+    return HB_OK;
+}
+
+hb_status hb_lattice_add_surrogate(hb_lattice* lat, const hb_surrogate_desc* d) {
+    if (!lat || !d) return fail(HB_ERR_INVALID_ARG, "NULL argument");
+    if (lat->finalized) return fail(HB_ERR_STATE, "lattice already finalized");
+    if (d->n_linear < 1 || d->n_linear > HB_MAX_LINEAR) return fail(HB_ERR_INVALID_ARG, "n_linear must be in [1,%d]", HB_MAX_LINEAR);
+    if (!d->widths || !d->W || !d->b) return fail(HB_ERR_INVALID_ARG, "widths/W/b is NULL");
+    if (d->widths[0] != 6 || d->widths[d->n_linear] != 6) return fail(HB_ERR_INVALID_ARG, "first and last width must be 6 (n = m = 6, P:105)");
+    if ((int)d->act < 0 || (int)d->act > HB_ACT_TANH) return fail(HB_ERR_INVALID_ARG, "unknown activation");
+    if ((int)d->prec < 0 || (int)d->prec > HB_PREC_TF32) return fail(HB_ERR_INVALID_ARG, "unknown precision");
+    if ((int)d->coord < 0 || (int)d->coord > HB_COORD_T) return fail(HB_ERR_INVALID_ARG, "unknown coord");
+    if (d->act == HB_ACT_PRELU && d->n_linear > 1 && !d->prelu_a) return fail(HB_ERR_INVALID_ARG, "PReLU needs slopes");
+    SurHost s;
+    s.n_linear = d->n_linear;
+    s.widths.assign(d->widths, d->widths + d->n_linear + 1);
+    for (int l = 1; l < d->n_linear; ++l)
+        if (s.widths[l] < 1 || s.widths[l] > HB_MAX_WIDTH) return fail(HB_ERR_INVALID_ARG, "hidden width %d outside [1,%d]", s.widths[l], HB_MAX_WIDTH);
+    for (int l = 0; l < d->n_linear; ++l) {
+        if (!d->W[l] || !d->b[l]) return fail(HB_ERR_INVALID_ARG, "W[%d] or b[%d] is NULL", l, l);
+        const size_t nw = (size_t)s.widths[l] * s.widths[l + 1];
+        s.W.emplace_back(d->W[l], d->W[l] + nw);
+        s.b.emplace_back(d->b[l], d->b[l] + s.widths[l + 1]);
+        for (float v : s.W.back()) if (!std::isfinite(v)) return fail(HB_ERR_INVALID_ARG, "non-finite weight in layer %d", l);
+        for (float v : s.b.back()) if (!std::isfinite(v)) return fail(HB_ERR_INVALID_ARG, "non-finite bias in layer %d", l);
+    }
+    s.act = d->act;
+    s.prelu.assign(HB_MAX_LINEAR, 0.0f);
+    if (d->act == HB_ACT_PRELU)
+        for (int l = 0; l < d->n_linear - 1; ++l) {
+            if (!std::isfinite(d->prelu_a[l])) return fail(HB_ERR_INVALID_ARG, "non-finite PReLU slope");
+            s.prelu[l] = d->prelu_a[l];
+        }
+    for (int j = 0; j < 6; ++j) {
+        if (!std::isfinite(d->in_mean[j]) || !std::isfinite(d->out_mean[j]) || !(d->in_std[j] > 0.0) ||
+            !(d->out_std[j] > 0.0) || !std::isfinite(d->in_std[j]) || !std::isfinite(d->out_std[j]))
+            return fail(HB_ERR_INVALID_ARG, "normalisation constants must be finite with std > 0");
+        s.in_mean[j] = d->in_mean[j]; s.in_std[j] = d->in_std[j];
+        s.out_mean[j] = d->out_mean[j]; s.out_std[j] = d->out_std[j];
+    }
+    s.coord = d->coord;
+    s.ref_bg_out = d->ref_bg_out;
+    s.ref_z_out = d->ref_z_out;
+    if (d->coord == HB_COORD_T && !std::isnan(d->ref_bg_out) && !(d->ref_bg_out > 0.0))
+        return fail(HB_ERR_INVALID_ARG, "ref_bg_out must be positive or NaN");
+    s.prec = d->prec;
+    lat->surs.push_back(std::move(s));
+    lat->elems.push_back(Elem{4, 0.0, 0.0, (int)lat->surs.size() - 1});
+    return HB_OK;
+}
+
+hb_status hb_lattice_set_run_mode(hb_lattice* lat, hb_run_mode mode) {
+    if (!lat) return fail(HB_ERR_INVALID_ARG, "lattice is NULL");
+    if (lat->finalized) return fail(HB_ERR_STATE, "lattice already finalized");
+    if ((int)mode < 0 || (int)mode > HB_RUN_SEQUENTIAL_FP32) return fail(HB_ERR_INVALID_ARG, "unknown run mode");
+    lat->run_mode = mode;
+    return HB_OK;
+}
+
+static hb_status upload(hb_lattice* lat, const void* src, size_t bytes, void** dst) {
+    *dst = nullptr;
+    if (bytes == 0) bytes = 16;
+    void* d = nullptr;
+    cudaError_t e = cudaMalloc(&d, bytes);
+    if (e != cudaSuccess) return fail(HB_ERR_ALLOC, "cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e));
+    lat->d_bufs.push_back(d);
+    if (src) HB_CUDA(cudaMemcpy(d, src, bytes, cudaMemcpyHostToDevice));
+    *dst = d;
+    return HB_OK;
+}
+
+static hb_status build_surrogate(hb_lattice* lat, const SurHost& s, double bg_in, double* bg_out, Segment& seg) {
+    HbSurDev& sd = seg.sd;
+    std::memset(&sd, 0, sizeof sd);
+    sd.n_linear = s.n_linear;
+    sd.act = s.act;
+    sd.coord = s.coord;
+    sd.prec = s.prec;
+    for (int l = 0; l <= s.n_linear; ++l) sd.widths[l] = s.widths[l];
+    for (int l = 0; l < HB_MAX_LINEAR; ++l) sd.prelu[l] = s.prelu[l];
+    for (int j = 0; j < 6; ++j) {
+        split_hi_lo(s.in_mean[j], sd.mu_hi[j], sd.mu_lo[j]);
+        sd.inv_sd[j] = (float)(1.0 / s.in_std[j]);
+        sd.out_sd[j] = (float)s.out_std[j];
+        sd.out_mu[j] = (float)s.out_mean[j];
+    }
+    *bg_out = bg_in;
+    if (s.coord == HB_COORD_T) {      // R6, R7
+        double bg1 = s.ref_bg_out, z1 = s.ref_z_out;
+        if (std::isnan(bg1) || std::isnan(z1)) {
+            const double rin[6] = {0, 0, 0, 0, 0, bg_in};
+            double rout[6];
+            mlp_host(s, rin, rout);
+            if (std::isnan(bg1)) bg1 = rout[5];
+            if (std::isnan(z1)) z1 = rout[2];
+        }
+        if (!(bg1 > 0.0) || !std::isfinite(bg1) || !std::isfinite(z1))
+            return fail(HB_ERR_INVALID_ARG, "surrogate reference output is unphysical (bg=%g, z=%g)", bg1, z1);
+        const double g0 = std::sqrt(1.0 + bg_in * bg_in), g1 = std::sqrt(1.0 + bg1 * bg1);
+        sd.bg0 = (float)bg_in; sd.g0 = (float)g0;
+        sd.bg1 = (float)bg1; sd.g1 = (float)g1; sd.inv_bg1 = (float)(1.0 / bg1);
+        sd.uz_in_shift = (float)(bg_in - s.in_mean[5]);
+        sd.uz_out_shift = (float)(s.out_mean[5] - bg1);
+        sd.z_out_mu = (float)(s.out_mean[2] - z1);
+        *bg_out = bg1;
+    }
+    // ---- fp32 image: W^T [k][npad], zero padded to 64 outputs
+    if (s.prec == HB_PREC_FP32) {
+        std::vector<float> w, b;
+        for (int l = 0; l < s.n_linear; ++l) {
+            const int fin = s.widths[l], fout = s.widths[l + 1];
+            const int npad = (fout + 63) / 64 * 64;
+            sd.npad32[l] = npad;
+            sd.w32_off[l] = (long long)w.size();
+            sd.b32_off[l] = (int)b.size();
+            w.resize(w.size() + (size_t)fin * npad, 0.0f);
+            b.resize(b.size() + npad, 0.0f);
+            float* wp = w.data() + sd.w32_off[l];
+            for (int o = 0; o < fout; ++o)
+                for (int k = 0; k < fin; ++k) wp[(size_t)k * npad + o] = s.W[l][(size_t)o * fin + k];
+            for (int o = 0; o < fout; ++o) b[sd.b32_off[l] + o] = s.b[l][o];
+        }
+        void *dw, *db;
+        hb_status st = upload(lat, w.data(), w.size() * sizeof(float), &dw);
+        if (st != HB_OK) return st;
+        st = upload(lat, b.data(), b.size() * sizeof(float), &db);
+        if (st != HB_OK) return st;
+        sd.w32 = (const float*)dw;
+        sd.b32 = (const float*)db;
+        seg.tc = false;
+    } else {
+        char why[256];
+        if (!hb_tc_supported(s.prec, s.n_linear, s.widths.data(), why, sizeof why))
+            return fail(HB_ERR_UNSUPPORTED, "tensor-core surrogate: %s", why);
+        std::vector<const float*> Wp;
+        for (int l = 0; l < s.n_linear; ++l) Wp.push_back(s.W[l].data());
+        const size_t bytes = hb_tc_pack_weights(s.prec, s.n_linear, s.widths.data(), Wp.data(), nullptr,
+                                                sd.wtc_off, sd.kpad, sd.npadtc);
+        std::vector<unsigned char> img(bytes);
+        hb_tc_pack_weights(s.prec, s.n_linear, s.widths.data(), Wp.data(), img.data(), sd.wtc_off, sd.kpad, sd.npadtc);
+        std::vector<float> b;
+        for (int l = 0; l < s.n_linear; ++l) {
+            sd.btc_off[l] = (int)b.size();
+            b.resize(b.size() + sd.npadtc[l], 0.0f);
+            for (int o = 0; o < s.widths[l + 1]; ++o) b[sd.btc_off[l] + o] = s.b[l][o];
+        }
+        void *dw, *db;
+        hb_status st = upload(lat, img.data(), img.size(), &dw);
+        if (st != HB_OK) return st;
+        st = upload(lat, b.data(), b.size() * sizeof(float), &db);
+        if (st != HB_OK) return st;
+        sd.wtc = dw;
+        sd.btc = (const float*)db;
+        seg.tc = true;
+    }
+    return HB_OK;
+}
+
+hb_status hb_lattice_finalize(hb_lattice* lat, int device) {
+    if (!lat) return fail(HB_ERR_INVALID_ARG, "lattice is NULL");
+    if (lat->finalized) return fail(HB_ERR_STATE, "lattice already finalized");
+    int ndev = 0;
+    HB_CUDA(cudaGetDeviceCount(&ndev));
+    if (device < 0 || device >= ndev) return fail(HB_ERR_CUDA, "no CUDA device %d (have %d)", device, ndev);
+    cudaDeviceProp prop;
+    HB_CUDA(cudaGetDeviceProperties(&prop, device));
+    if (prop.major != 10) return fail(HB_ERR_UNSUPPORTED, "device %d is sm_%d%d; libhb is built for sm_100a only", device, prop.major, prop.minor);
+    int prev = 0;
+    HB_CUDA(cudaGetDevice(&prev));
+    HB_CUDA(cudaSetDevice(device));
+    lat->device = device;
+    lat->sm_count = prop.multiProcessorCount;
+
+    // ---- split into segments, tracking the reference (R5, R7, G17)
+    std::vector<HbSeqElem> seq;
+    double bg = lat->bg0;
+    lat->segs.clear();
+    lat->n_monitors = 0;
+    size_t i = 0;
+    hb_status st = HB_OK;
+    while (i < lat->elems.size() && st == HB_OK) {
+        const Elem& e = lat->elems[i];
+        if (e.kind == HB_ELEM_MONITOR) {
+            if (!lat->segs.empty() && lat->segs.back().monitor < 0 && lat->segs.back().type != SEG_MON) {
+                lat->segs.back().monitor = lat->n_monitors++;
+            } else {
+                Segment s{};
+                s.type = SEG_MON;
+                s.monitor = lat->n_monitors++;
+                lat->segs.push_back(s);
+            }
+            ++i;
+        } else if (e.kind == 4) {
+            Segment s{};
+            s.type = SEG_SUR;
+            s.monitor = -1;
+            double bg1 = bg;
+            st = build_surrogate(lat, lat->surs[e.sur], bg, &bg1, s);
+            bg = bg1;
+            lat->segs.push_back(s);
+            ++i;
+        } else {
+            Segment s{};
+            s.type = SEG_RUN;
+            s.monitor = -1;
+            s.seq_off = (int)seq.size();
+            Mat6 M = mat_identity();
+            while (i < lat->elems.size() && lat->elems[i].kind <= HB_ELEM_SBEND) {
+                M = mat_mul(elem_matrix(lat->elems[i], bg), M);
+                seq.push_back(seq_elem(lat->elems[i], bg));
+                ++i;
+            }
+            s.seq_cnt = (int)seq.size() - s.seq_off;
+            for (int r = 0; r < 6; ++r)
+                for (int c = 0; c < 6; ++c) s.map.m[r * 6 + c] = (float)M.m[r][c];
+            lat->segs.push_back(s);
+        }
+    }
+    if (st == HB_OK) {
+        void* d = nullptr;
+        st = upload(lat, seq.data(), seq.size() * sizeof(HbSeqElem), &d);
+        lat->d_seq = (HbSeqElem*)d;
+    }
+    if (st == HB_OK) {
+        void* d = nullptr;
+        st = upload(lat, nullptr, (size_t)HB_MOM_MAX_BLOCKS * HB_NMOM * sizeof(double), &d);
+        lat->d_partials = (double*)d;
+    }
+    if (st == HB_OK) {
+        cudaError_t e = cudaDeviceSynchronize();
+        if (e != cudaSuccess) st = fail(HB_ERR_CUDA, "cudaDeviceSynchronize: %s", cudaGetErrorString(e));
+    }
+    lat->bg_out = bg;
+    cudaSetDevice(prev);
+    if (st != HB_OK) {
+        for (void* p : lat->d_bufs) cudaFree(p);
+        lat->d_bufs.clear();
+        lat->segs.clear();
+        return st;
+    }
+    lat->finalized = true;
+    return HB_OK;
+}
+
+hb_status hb_lattice_num_monitors(const hb_lattice* lat, int* out) {
+    if (!lat || !out) return fail(HB_ERR_INVALID_ARG, "NULL argument");
+    int n = 0;
+    for (const Elem& e : lat->elems) n += e.kind == HB_ELEM_MONITOR;
+    *out = n;
+    return HB_OK;
+}
+
+hb_status hb_lattice_num_launches(const hb_lattice* lat, int with_moments, int* out) {
+    if (!lat || !out) return fail(HB_ERR_INVALID_ARG, "NULL argument");
+    if (!lat->finalized) return fail(HB_ERR_STATE, "lattice not finalized");
+    int n = 0;
+    for (const Segment& s : lat->segs) {
+        if (s.type == SEG_MON) n += with_moments ? 2 : 0;
+        else n += 1 + ((with_moments && s.monitor >= 0) ? 1 : 0);
+    }
+    *out = n;
+    return HB_OK;
+}
+
+hb_status hb_lattice_ref_bg_out(const hb_lattice* lat, double* out) {
+    if (!lat || !out) return fail(HB_ERR_INVALID_ARG, "NULL argument");
+    if (!lat->finalized) return fail(HB_ERR_STATE, "lattice not finalized");
+    *out = lat->bg_out;
+    return HB_OK;
+}
+
+static hb_status check_arrays(const float* const a[6], size_t n) {
+    for (int j = 0; j < 6; ++j) {
+        if (!a[j]) return fail(HB_ERR_INVALID_ARG, "particle array %d is NULL", j);
+        if ((uintptr_t)a[j] & 15u) return fail(HB_ERR_INVALID_ARG, "particle array %d is not 16-byte aligned", j);
+    }
+    const size_t bytes = n * sizeof(float);
+    for (int j = 0; j < 6; ++j)
+        for (int k = j + 1; k < 6; ++k) {
+            const uintptr_t a0 = (uintptr_t)a[j], b0 = (uintptr_t)a[k];
+            if (a0 < b0 + bytes && b0 < a0 + bytes)
+                return fail(HB_ERR_INVALID_ARG, "particle arrays %d and %d overlap", j, k);
+        }
+    return HB_OK;
+}
+
+static hb_status push_impl(hb_lattice* lat, float* x, float* px, float* y, float* py, float* t, float* pt, size_t n,
+                           double* d_moments, bool want_moments, void* stream) {
+    if (!lat) return fail(HB_ERR_INVALID_ARG, "lattice is NULL");
+    if (!lat->finalized) return fail(HB_ERR_STATE, "lattice not finalized");
+    cudaStream_t s = (cudaStream_t)stream;
+    if (want_moments && lat->n_monitors > 0) {
+        if (!d_moments) return fail(HB_ERR_INVALID_ARG, "d_moments is NULL");
+        if ((uintptr_t)d_moments & 7u) return fail(HB_ERR_INVALID_ARG, "d_moments is not 8-byte aligned");
+    }
+    int prev = 0;
+    HB_CUDA(cudaGetDevice(&prev));
+    if (prev != lat->device) HB_CUDA(cudaSetDevice(lat->device));
+    hb_status st = HB_OK;
+    if (n == 0) {
+        if (want_moments && lat->n_monitors > 0) {    // NaN records: all-ones bytes are a quiet NaN
+            cudaError_t e = cudaMemsetAsync(d_moments, 0xff, (size_t)lat->n_monitors * HB_NMOM * sizeof(double), s);
+            if (e != cudaSuccess) st = fail(HB_ERR_CUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e));
+        }
+    } else {
+        const float* arr[6] = {x, px, y, py, t, pt};
+        st = check_arrays(arr, n);
+        HbParticles p;
+        p.v[0] = x; p.v[1] = px; p.v[2] = y; p.v[3] = py; p.v[4] = t; p.v[5] = pt;
+        for (size_t k = 0; k < lat->segs.size() && st == HB_OK; ++k) {
+            const Segment& g = lat->segs[k];
+            const bool mom = want_moments && g.monitor >= 0;
+            double* partials = mom ? lat->d_partials : nullptr;
+            int nblocks = 0;
+            cudaError_t e = cudaSuccess;
+            if (g.type == SEG_RUN) {
+                if (lat->run_mode == HB_RUN_COMPOSED) e = hb_launch_run_composed(p, n, g.map, partials, &nblocks, s);
+                else e = hb_launch_run_sequential(p, n, lat->d_seq + g.seq_off, g.seq_cnt,
+                                                  lat->run_mode == HB_RUN_SEQUENTIAL_FP32, partials, &nblocks, s);
+            } else if (g.type == SEG_SUR) {
+                e = g.tc ? hb_launch_sur_tc(p, n, g.sd, partials, &nblocks, lat->sm_count, s)
+                         : hb_launch_sur_fp32(p, n, g.sd, partials, &nblocks, lat->sm_count, s);
+            } else if (mom) {
+                e = hb_launch_moments_partials(p, n, nullptr, partials, &nblocks, s);
+            }
+            if (e != cudaSuccess) { st = fail(HB_ERR_CUDA, "kernel launch (segment %zu): %s", k, cudaGetErrorString(e)); break; }
+            if (mom) {
+                e = hb_launch_moments_finalize(partials, nblocks, n, nullptr, d_moments + (size_t)g.monitor * HB_NMOM, s);
+                if (e != cudaSuccess) st = fail(HB_ERR_CUDA, "moments finalize: %s", cudaGetErrorString(e));
+            }
+        }
+    }
+    if (prev != lat->device) cudaSetDevice(prev);
+    return st;
+}
+
+hb_status hb_push(hb_lattice* lat, float* x, float* px, float* y, float* py, float* t, float* pt, size_t n, void* stream) {
+    return push_impl(lat, x, px, y, py, t, pt, n, nullptr, false, stream);
+}
+
+hb_status hb_push_moments(hb_lattice* lat, float* x, float* px, float* y, float* py, float* t, float* pt, size_t n,
+                          double* d_moments, void* stream) {
+    return push_impl(lat, x, px, y, py, t, pt, n, d_moments, true, stream);
+}
+
+size_t hb_moments_scratch_bytes(void) { return (size_t)HB_MOM_MAX_BLOCKS * HB_NMOM * sizeof(double); }
+
+hb_status hb_moments(const float* x, const float* px, const float* y, const float* py, const float* t, const float* pt,
+                     size_t n, const double* pivot, double* d_out27, void* d_scratch, void* stream) {
+    if (!d_out27 || !d_scratch) return fail(HB_ERR_INVALID_ARG, "d_out27 / d_scratch is NULL");
+    cudaStream_t s = (cudaStream_t)stream;
+    if (n == 0) {
+        HB_CUDA(cudaMemsetAsync(d_out27, 0xff, HB_NMOM * sizeof(double), s));
+        return HB_OK;
+    }
+    const float* arr[6] = {x, px, y, py, t, pt};
+    hb_status st = check_arrays(arr, n);
+    if (st != HB_OK) return st;
+    HbParticles p;
+    for (int j = 0; j < 6; ++j) p.v[j] = const_cast<float*>(arr[j]);
+    int nblocks = 0;
+    HB_CUDA(hb_launch_moments_partials(p, n, pivot, (double*)d_scratch, &nblocks, s));
+    HB_CUDA(hb_launch_moments_finalize((const double*)d_scratch, nblocks, n, pivot, d_out27, s));
+    return HB_OK;
+}
+
+hb_status hb_lattice_destroy(hb_lattice* lat) {
+    if (!lat) return HB_OK;
+    if (lat->finalized) {
+        int prev = 0;
+        cudaGetDevice(&prev);
+        cudaSetDevice(lat->device);
+        cudaDeviceSynchronize();
+        for (void* p : lat->d_bufs) cudaFree(p);
+        cudaSetDevice(prev);
+    }
+    delete lat;
+    return HB_OK;
+}
+
+}  // extern "C"

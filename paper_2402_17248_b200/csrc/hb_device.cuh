@@ -1,0 +1,121 @@
+// hb_device.cuh -- device helpers shared by libhb's kernels: moment accumulation (R10),
+// s<->t conversion in deviation form (R6, R7), activations (Eq. 1, 2; tanh).
+#pragma once
+#include "hb_internal.h"
+
+// ------------------------------------------------------------------------- moments (R10)
+// Per-thread fp64 accumulators of the (pivot-shifted) raw sums:  S1_j = sum v_j,  S2_jk = sum v_j v_k (j<=k).
+struct HbMomAcc {
+    double s[HB_NMOM];
+    __device__ __forceinline__ void clear() {
+#pragma unroll
+        for (int i = 0; i < HB_NMOM; ++i) s[i] = 0.0;
+    }
+    __device__ __forceinline__ void add(const double (&v)[6]) {
+#pragma unroll
+        for (int j = 0; j < 6; ++j) s[j] += v[j];
+        int idx = 6;
+#pragma unroll
+        for (int j = 0; j < 6; ++j)
+#pragma unroll
+            for (int k = j; k < 6; ++k) { s[idx] = fma(v[j], v[k], s[idx]); ++idx; }
+    }
+    __device__ __forceinline__ void add(float x, float px, float y, float py, float t, float pt) {
+        const double v[6] = {(double)x, (double)px, (double)y, (double)py, (double)t, (double)pt};
+        add(v);
+    }
+};
+
+// Block-level fixed-order reduction of the 27 accumulators: warp xor-shuffle tree, then warp 0..
+// sums the per-warp values in warp order.  `scratch` : shared, >= (blockDim/32)*27 doubles.
+// All threads of the participating group [tid0, tid0+nthreads) must call; `bar_id` named barrier.
+__device__ __forceinline__ void hb_block_reduce_moments(HbMomAcc& acc, double* scratch, double* out_partial,
+                                                        int tid, int nthreads, int bar_id) {
+    const int lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
+#pragma unroll
+    for (int i = 0; i < HB_NMOM; ++i) {
+        double v = acc.s[i];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) scratch[warp * HB_NMOM + i] = v;
+    }
+    asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "r"(nthreads) : "memory");
+    if (tid < HB_NMOM) {
+        double v = 0.0;
+        for (int w = 0; w < nwarps; ++w) v += scratch[w * HB_NMOM + tid];
+        out_partial[tid] = v;
+    }
+}
+
+// ------------------------------------------------------------------------- activations
+__device__ __forceinline__ float hb_tanh_approx(float x) {
+    float y;
+    asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+template <int ACT, bool FAST>
+__device__ __forceinline__ float hb_activate(float z, float a) {
+    if (ACT == 1) return fmaxf(z, 0.0f);                  // Eq. 1
+    if (ACT == 2) return z >= 0.0f ? z : a * z;           // Eq. 2
+    if (ACT == 3) return FAST ? hb_tanh_approx(z) : tanhf(z);
+    return z;
+}
+
+// ------------------------------------------------------------------------- R6 / R8: prologue and epilogue
+// s-coordinates of one particle -> the six NORMALISED network inputs.
+__device__ __forceinline__ void hb_sur_prologue(const HbSurDev& sd, float x, float px, float y, float py,
+                                                float t, float pt, float (&nin)[6]) {
+    if (sd.coord == 0) {
+        const float v[6] = {x, px, y, py, t, pt};
+#pragma unroll
+        for (int j = 0; j < 6; ++j) nin[j] = ((v[j] - sd.mu_hi[j]) - sd.mu_lo[j]) * sd.inv_sd[j];
+    } else {
+        // to_t in deviation form: never forms uz (~1958) and subtracts its mean in fp32
+        const float ux = px * sd.bg0, uy = py * sd.bg0;
+        const float dg = -pt * sd.bg0;                                   // gamma - gamma0
+        const float g = sd.g0 + dg;
+        const float num = fmaf(dg, 2.0f * sd.g0 + dg, -fmaf(ux, ux, uy * uy));  // uz^2 - uz0^2
+        const float uz = sqrtf(fmaxf(fmaf(sd.bg0, sd.bg0, num), 0.0f));
+        const float duz = num / (uz + sd.bg0);                           // uz - uz0
+        const float ig = 1.0f / g;
+        const float xt = fmaf(-ux * ig, t, x);
+        const float yt = fmaf(-uy * ig, t, y);
+        const float zt = -(uz * ig) * t;
+        const float v[5] = {xt, yt, zt, ux, uy};
+#pragma unroll
+        for (int j = 0; j < 5; ++j) nin[j] = ((v[j] - sd.mu_hi[j]) - sd.mu_lo[j]) * sd.inv_sd[j];
+        nin[5] = (duz + sd.uz_in_shift) * sd.inv_sd[5];
+    }
+}
+
+// six raw network outputs -> s-coordinates (about the new reference for COORD_T)
+__device__ __forceinline__ void hb_sur_epilogue(const HbSurDev& sd, const float (&w)[6], float& x, float& px,
+                                                float& y, float& py, float& t, float& pt) {
+    if (sd.coord == 0) {
+        x = fmaf(w[0], sd.out_sd[0], sd.out_mu[0]);
+        px = fmaf(w[1], sd.out_sd[1], sd.out_mu[1]);
+        y = fmaf(w[2], sd.out_sd[2], sd.out_mu[2]);
+        py = fmaf(w[3], sd.out_sd[3], sd.out_mu[3]);
+        t = fmaf(w[4], sd.out_sd[4], sd.out_mu[4]);
+        pt = fmaf(w[5], sd.out_sd[5], sd.out_mu[5]);
+    } else {
+        const float xt = fmaf(w[0], sd.out_sd[0], sd.out_mu[0]);
+        const float yt = fmaf(w[1], sd.out_sd[1], sd.out_mu[1]);
+        const float zt = fmaf(w[2], sd.out_sd[2], sd.z_out_mu);          // z - z_ref  (R7)
+        const float ux = fmaf(w[3], sd.out_sd[3], sd.out_mu[3]);
+        const float uy = fmaf(w[4], sd.out_sd[4], sd.out_mu[4]);
+        const float d = fmaf(w[5], sd.out_sd[5], sd.uz_out_shift);       // uz - uz1
+        const float uz = sd.bg1 + d;
+        const float s2 = fmaf(ux, ux, uy * uy);
+        const float g = sqrtf(1.0f + s2 + uz * uz);
+        const float dgam = fmaf(d, 2.0f * sd.bg1 + d, s2) / (g + sd.g1); // gamma - gamma1
+        const float iuz = 1.0f / uz;
+        x = fmaf(-ux * iuz, zt, xt);
+        y = fmaf(-uy * iuz, zt, yt);
+        t = -zt * g * iuz;
+        px = ux * sd.inv_bg1;
+        py = uy * sd.inv_bg1;
+        pt = -dgam * sd.inv_bg1;
+    }
+}

@@ -1,0 +1,84 @@
+// hb_internal.h -- shared declarations of libhb.so's translation units (host + device).
+// Not part of the public ABI (include/hb.h) and not shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#define HB_MAX_LINEAR 12      // L_0 .. L_l, l <= 11 hidden layers
+#define HB_MAX_WIDTH 1024
+#define HB_NMOM 27            // 6 first + 21 second moments
+#define HB_MOM_MAX_BLOCKS 2368  // 148 SMs x 16: upper bound on blocks that write moment partials
+
+// ---- conventional runs -------------------------------------------------------------------
+struct HbRunMap {             // composed run: v' = M v (row-major 6x6, fp32, built in fp64 on the host)
+    float m[36];
+};
+
+// one conventional element in sequential mode (coefficients in fp64)
+//  kind 0 drift : a0 = L, a1 = L/(bg)^2
+//  kind 1 quad  : a0..a3 = x-plane 2x2 (row-major), a4..a7 = y-plane 2x2, a8 = L/(bg)^2
+//  kind 2 sbend : a0..a3 = x-plane 2x2, a4 = R16, a5 = R26, a6 = L (y drift), a7 = R51, a8 = R52, a9 = R56
+struct HbSeqElem {
+    double a[10];
+    int kind;
+    int pad;
+};
+
+// ---- surrogate stage ---------------------------------------------------------------------
+struct HbSurDev {             // passed by value to the surrogate kernels
+    int n_linear;
+    int act;                  // hb_act
+    int coord;                // hb_coord
+    int prec;                 // hb_prec
+    int widths[HB_MAX_LINEAR + 1];
+    float prelu[HB_MAX_LINEAR];
+    // input normalisation  v^ = ((v - mu_hi) - mu_lo) * inv_sd   (mu split so that fp32 loses nothing)
+    float mu_hi[6], mu_lo[6], inv_sd[6];
+    // output  w = w^ * out_sd + out_mu
+    float out_sd[6], out_mu[6];
+    // COORD_T constants (R6, R7), all formed in fp64 on the host
+    float bg0, g0;            // incoming reference
+    float bg1, g1, inv_bg1;   // outgoing reference
+    float uz_in_shift;        // (bg0 - in_mean[5])            : n5 = (duz + uz_in_shift) * inv_sd[5]
+    float uz_out_shift;       // (out_mean[5] - bg1)           : d  = w^5 * out_sd[5] + uz_out_shift
+    float z_out_mu;           // (out_mean[2] - z_ref)
+    // fp32 path: packed W^T  [layer][k][npad]  and biases [layer][npad]
+    const float* w32;
+    const float* b32;
+    long long w32_off[HB_MAX_LINEAR];
+    int b32_off[HB_MAX_LINEAR];
+    int npad32[HB_MAX_LINEAR];
+    // tensor-core path: packed 16-bit (or tf32) operand image, see hb_sur_tc.cu
+    const void* wtc;
+    const float* btc;         // biases fp32, padded, per layer
+    long long wtc_off[HB_MAX_LINEAR];   // byte offsets
+    int btc_off[HB_MAX_LINEAR];
+    int kpad[HB_MAX_LINEAR];  // padded fan-in  (multiple of 64 elements; layer 0: 64)
+    int npadtc[HB_MAX_LINEAR];// padded fan-out (multiple of 16; hidden: multiple of 64)
+};
+
+struct HbParticles {
+    float* v[6];              // x, px, y, py, t, pt
+};
+
+// ---- launchers (each returns the cudaError_t of the launch) ---------------------------------
+// partials: device [>= gridDim][27] doubles or nullptr (no moments)
+cudaError_t hb_launch_run_composed(const HbParticles& p, size_t n, const HbRunMap& map,
+                                   double* partials, int* nblocks_out, cudaStream_t s);
+cudaError_t hb_launch_run_sequential(const HbParticles& p, size_t n, const HbSeqElem* d_elems, int count,
+                                     bool fp32_regs, double* partials, int* nblocks_out, cudaStream_t s);
+cudaError_t hb_launch_moments_partials(const HbParticles& p, size_t n, const double* pivot6_host,
+                                       double* partials, int* nblocks_out, cudaStream_t s);
+// fixed-order sum of `nblocks` partials -> 27-double record (pivot added back to the means)
+cudaError_t hb_launch_moments_finalize(const double* partials, int nblocks, size_t n,
+                                       const double* pivot6_host, double* d_out27, cudaStream_t s);
+cudaError_t hb_launch_sur_fp32(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials,
+                               int* nblocks_out, int sm_count, cudaStream_t s);
+cudaError_t hb_launch_sur_tc(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials,
+                             int* nblocks_out, int sm_count, cudaStream_t s);
+// host-side packing for the tensor-core path (hb_sur_tc.cu owns the layout)
+//  returns bytes needed; if dst != nullptr writes the image.  W row-major [out][in] fp32.
+size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float* const* W,
+                          void* dst, long long* off_bytes, int* kpad, int* npad);
+bool hb_tc_supported(int prec, int n_linear, const int* widths, char* why, size_t why_len);

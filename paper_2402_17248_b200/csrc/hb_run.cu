@@ -1,0 +1,284 @@
+// hb_run.cu -- fused conventional-run kernels (a2), moment partials / finalize (a3).
+//
+// Row a2 of the hot path: a whole run of consecutive conventional elements (drift R2,
+// thick quad R3, sector bend R4) is applied with ONE read and ONE write of the six
+// SoA arrays: 48 B per particle per run, HBM-bound.  Loads/stores are 128-bit (4 particles per
+// thread per coordinate), streaming (evict-first) cache hints, in place.
+//   composed  : v' = M_run v, M_run concatenated in fp64 on the host, 36 FFMA per particle.
+//   sequential: element list staged in shared memory, applied one by one in registers
+//               (fp64, or fp32 for HB_RUN_SEQUENTIAL_FP32), one rounding at the store.
+// Row a3: when a monitor follows the run, the 27 raw moment sums (R10) are accumulated in fp64 from
+// the values already in registers, reduced by warp shuffles, and one partial per block is written.
+#include "hb_device.cuh"
+
+#define RUN_THREADS 256
+
+__device__ __forceinline__ float4 ld_stream(const float* p) { return __ldcs(reinterpret_cast<const float4*>(p)); }
+__device__ __forceinline__ void st_stream(float* p, const float4& v) { __stcs(reinterpret_cast<float4*>(p), v); }
+
+__device__ __forceinline__ void apply_map(const HbRunMap& M, const float (&in)[6], float (&out)[6]) {
+#pragma unroll
+    for (int r = 0; r < 6; ++r) {
+        float acc = M.m[r * 6] * in[0];
+#pragma unroll
+        for (int c = 1; c < 6; ++c) acc = fmaf(M.m[r * 6 + c], in[c], acc);
+        out[r] = acc;
+    }
+}
+
+template <bool MOM>
+__global__ void __launch_bounds__(RUN_THREADS, MOM ? 2 : 4)
+hb_run_composed_kernel(HbParticles p, size_t n, const __grid_constant__ HbRunMap M, double* __restrict__ partials) {
+    __shared__ double red[(RUN_THREADS / 32) * HB_NMOM];
+    HbMomAcc acc;
+    if (MOM) acc.clear();
+    const size_t nq = n >> 2;
+    const size_t stride = (size_t)gridDim.x * RUN_THREADS;
+    for (size_t q = (size_t)blockIdx.x * RUN_THREADS + threadIdx.x; q < nq; q += stride) {
+        float4 c[6];
+#pragma unroll
+        for (int j = 0; j < 6; ++j) c[j] = ld_stream(p.v[j] + 4 * q);
+        float4 o[6];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            float in[6], out[6];
+#pragma unroll
+            for (int j = 0; j < 6; ++j) in[j] = reinterpret_cast<const float*>(&c[j])[e];
+            apply_map(M, in, out);
+#pragma unroll
+            for (int j = 0; j < 6; ++j) reinterpret_cast<float*>(&o[j])[e] = out[j];
+            if (MOM) acc.add(out[0], out[1], out[2], out[3], out[4], out[5]);
+        }
+#pragma unroll
+        for (int j = 0; j < 6; ++j) st_stream(p.v[j] + 4 * q, o[j]);
+    }
+    // ragged tail (n mod 4 particles): scalar, by the first threads of block 0
+    if (blockIdx.x == 0 && threadIdx.x < (n & 3)) {
+        const size_t i = (nq << 2) + threadIdx.x;
+        float in[6], out[6];
+#pragma unroll
+        for (int j = 0; j < 6; ++j) in[j] = p.v[j][i];
+        apply_map(M, in, out);
+#pragma unroll
+        for (int j = 0; j < 6; ++j) p.v[j][i] = out[j];
+        if (MOM) acc.add(out[0], out[1], out[2], out[3], out[4], out[5]);
+    }
+    if (MOM) hb_block_reduce_moments(acc, red, partials + (size_t)blockIdx.x * HB_NMOM, threadIdx.x, RUN_THREADS, 1);
+}
+
+// ---------------------------------------------------------------------------------- sequential
+#define SEQ_CHUNK 128
+template <typename T>
+struct SeqElemT { T a[10]; int kind; };
+
+template <typename T>
+__device__ __forceinline__ void seq_apply(const SeqElemT<T>& e, T (&v)[6]) {
+    // v = (x, px, y, py, t, pt); pt never changes (R2-R4)
+    if (e.kind == 0) {                 // drift R2
+        v[0] = fma(e.a[0], v[1], v[0]);
+        v[2] = fma(e.a[0], v[3], v[2]);
+        v[4] = fma(e.a[1], v[5], v[4]);
+    } else if (e.kind == 1) {          // thick quad R3
+        const T x = v[0], px = v[1], y = v[2], py = v[3];
+        v[0] = fma(e.a[0], x, e.a[1] * px);
+        v[1] = fma(e.a[2], x, e.a[3] * px);
+        v[2] = fma(e.a[4], y, e.a[5] * py);
+        v[3] = fma(e.a[6], y, e.a[7] * py);
+        v[4] = fma(e.a[8], v[5], v[4]);
+    } else {                           // sector bend R4
+        const T x = v[0], px = v[1], d = v[5];
+        v[0] = fma(e.a[0], x, fma(e.a[1], px, e.a[4] * d));
+        v[1] = fma(e.a[2], x, fma(e.a[3], px, e.a[5] * d));
+        v[2] = fma(e.a[6], v[3], v[2]);
+        v[4] = fma(e.a[7], x, fma(e.a[8], px, fma(e.a[9], d, v[4])));
+    }
+}
+
+template <typename T, bool MOM>
+__global__ void __launch_bounds__(RUN_THREADS, 2)
+hb_run_sequential_kernel(HbParticles p, size_t n, const HbSeqElem* __restrict__ elems, int count,
+                         double* __restrict__ partials) {
+    __shared__ SeqElemT<T> se[SEQ_CHUNK];
+    __shared__ double red[(RUN_THREADS / 32) * HB_NMOM];
+    HbMomAcc acc;
+    if (MOM) acc.clear();
+    const size_t nq = n >> 2;
+    const size_t nwork = nq + ((n & 3) ? 1 : 0);           // last work item = ragged tail
+    const size_t stride = (size_t)gridDim.x * RUN_THREADS;
+    const size_t first = (size_t)blockIdx.x * RUN_THREADS + threadIdx.x;
+    // every thread of the block runs the same number of outer iterations (the element staging syncs)
+    const size_t base0 = (size_t)blockIdx.x * RUN_THREADS;
+    for (size_t base = base0; base < nwork; base += stride) {
+        const size_t q = base + threadIdx.x;
+        const bool active = q < nwork;
+        const bool tail = active && q == nq;
+        const int cnt = !active ? 0 : (tail ? (int)(n & 3) : 4);
+        T v[4][6];
+        if (active && !tail) {
+            float4 c[6];
+#pragma unroll
+            for (int j = 0; j < 6; ++j) c[j] = ld_stream(p.v[j] + 4 * q);
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+#pragma unroll
+                for (int j = 0; j < 6; ++j) v[e][j] = (T) reinterpret_cast<const float*>(&c[j])[e];
+        } else {
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+#pragma unroll
+                for (int j = 0; j < 6; ++j) v[e][j] = (e < cnt) ? (T)p.v[j][4 * nq + e] : (T)0;
+        }
+        for (int c0 = 0; c0 < count; c0 += SEQ_CHUNK) {
+            const int m = min(SEQ_CHUNK, count - c0);
+            __syncthreads();
+            for (int i = threadIdx.x; i < m; i += RUN_THREADS) {
+                const HbSeqElem& g = elems[c0 + i];
+#pragma unroll
+                for (int k = 0; k < 10; ++k) se[i].a[k] = (T)g.a[k];
+                se[i].kind = g.kind;
+            }
+            __syncthreads();
+            for (int i = 0; i < m; ++i) {
+                const SeqElemT<T> e = se[i];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) seq_apply(e, v[k]);
+            }
+        }
+        if (active && !tail) {
+            float4 o[6];
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+#pragma unroll
+                for (int j = 0; j < 6; ++j) reinterpret_cast<float*>(&o[j])[e] = (float)v[e][j];
+#pragma unroll
+            for (int j = 0; j < 6; ++j) st_stream(p.v[j] + 4 * q, o[j]);
+        } else {
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+                if (e < cnt)
+#pragma unroll
+                    for (int j = 0; j < 6; ++j) p.v[j][4 * nq + e] = (float)v[e][j];
+        }
+        if (MOM) {
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+                if (e < cnt)
+                    acc.add((float)v[e][0], (float)v[e][1], (float)v[e][2], (float)v[e][3], (float)v[e][4],
+                            (float)v[e][5]);
+        }
+    }
+    (void)first;
+    if (MOM) hb_block_reduce_moments(acc, red, partials + (size_t)blockIdx.x * HB_NMOM, threadIdx.x, RUN_THREADS, 1);
+}
+
+// ---------------------------------------------------------------------------------- standalone moments
+struct HbPivot { double p[6]; };
+
+__global__ void __launch_bounds__(RUN_THREADS, 2)
+hb_moments_partials_kernel(HbParticles p, size_t n, const __grid_constant__ HbPivot pv, double* __restrict__ partials) {
+    __shared__ double red[(RUN_THREADS / 32) * HB_NMOM];
+    HbMomAcc acc;
+    acc.clear();
+    const size_t nq = n >> 2;
+    const size_t stride = (size_t)gridDim.x * RUN_THREADS;
+    for (size_t q = (size_t)blockIdx.x * RUN_THREADS + threadIdx.x; q < nq; q += stride) {
+        float4 c[6];
+#pragma unroll
+        for (int j = 0; j < 6; ++j) c[j] = ld_stream(p.v[j] + 4 * q);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            double v[6];
+#pragma unroll
+            for (int j = 0; j < 6; ++j) v[j] = (double)reinterpret_cast<const float*>(&c[j])[e] - pv.p[j];
+            acc.add(v);
+        }
+    }
+    if (blockIdx.x == 0 && threadIdx.x < (n & 3)) {
+        const size_t i = (nq << 2) + threadIdx.x;
+        double v[6];
+#pragma unroll
+        for (int j = 0; j < 6; ++j) v[j] = (double)p.v[j][i] - pv.p[j];
+        acc.add(v);
+    }
+    hb_block_reduce_moments(acc, red, partials + (size_t)blockIdx.x * HB_NMOM, threadIdx.x, RUN_THREADS, 1);
+}
+
+// One block of 27 warps: warp j sums partial[k][j], k = lane, lane+32, ... in a fixed order, then a
+// shuffle tree.  Then threads 0..26 turn the raw sums into the record (means + centred covariance, 1/N).
+__global__ void __launch_bounds__(HB_NMOM * 32, 1)
+hb_moments_finalize_kernel(const double* __restrict__ partials, int nblocks, size_t n,
+                           const __grid_constant__ HbPivot pv, double* __restrict__ out) {
+    __shared__ double S[HB_NMOM];
+    const int j = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double v = 0.0;
+    for (int k = lane; k < nblocks; k += 32) v += partials[(size_t)k * HB_NMOM + j];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (lane == 0) S[j] = v;
+    __syncthreads();
+    if (threadIdx.x < HB_NMOM) {
+        const int i = threadIdx.x;
+        const double inv = n > 0 ? 1.0 / (double)n : __longlong_as_double(0x7ff8000000000000LL);
+        if (i < 6) {
+            out[i] = S[i] * inv + pv.p[i];
+        } else {
+            int a = 0, rem = i - 6;
+            while (rem >= 6 - a) { rem -= 6 - a; ++a; }
+            const int b = a + rem;
+            out[i] = S[i] * inv - (S[a] * inv) * (S[b] * inv);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------- launchers
+static int run_grid(size_t n, bool moments) {
+    const size_t nq = (n >> 2) + ((n & 3) ? 1 : 0);
+    size_t blocks = (nq + RUN_THREADS - 1) / RUN_THREADS;
+    if (blocks < 1) blocks = 1;
+    const size_t cap = moments ? HB_MOM_MAX_BLOCKS / 4 : 148 * 32;   // moments: 592 = 148 x 4 (2 resident x 2 waves)
+    if (blocks > cap) blocks = cap;
+    return (int)blocks;
+}
+
+cudaError_t hb_launch_run_composed(const HbParticles& p, size_t n, const HbRunMap& map, double* partials,
+                                   int* nblocks_out, cudaStream_t s) {
+    const int grid = run_grid(n, partials != nullptr);
+    if (nblocks_out) *nblocks_out = grid;
+    if (partials)
+        hb_run_composed_kernel<true><<<grid, RUN_THREADS, 0, s>>>(p, n, map, partials);
+    else
+        hb_run_composed_kernel<false><<<grid, RUN_THREADS, 0, s>>>(p, n, map, partials);
+    return cudaGetLastError();
+}
+
+cudaError_t hb_launch_run_sequential(const HbParticles& p, size_t n, const HbSeqElem* d_elems, int count,
+                                     bool fp32_regs, double* partials, int* nblocks_out, cudaStream_t s) {
+    const int grid = run_grid(n, partials != nullptr);
+    if (nblocks_out) *nblocks_out = grid;
+    if (fp32_regs) {
+        if (partials) hb_run_sequential_kernel<float, true><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
+        else hb_run_sequential_kernel<float, false><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
+    } else {
+        if (partials) hb_run_sequential_kernel<double, true><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
+        else hb_run_sequential_kernel<double, false><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t hb_launch_moments_partials(const HbParticles& p, size_t n, const double* pivot6_host, double* partials,
+                                       int* nblocks_out, cudaStream_t s) {
+    HbPivot pv;
+    for (int j = 0; j < 6; ++j) pv.p[j] = pivot6_host ? pivot6_host[j] : 0.0;
+    const int grid = run_grid(n, true);
+    if (nblocks_out) *nblocks_out = grid;
+    hb_moments_partials_kernel<<<grid, RUN_THREADS, 0, s>>>(p, n, pv, partials);
+    return cudaGetLastError();
+}
+
+cudaError_t hb_launch_moments_finalize(const double* partials, int nblocks, size_t n, const double* pivot6_host,
+                                       double* d_out27, cudaStream_t s) {
+    HbPivot pv;
+    for (int j = 0; j < 6; ++j) pv.p[j] = pivot6_host ? pivot6_host[j] : 0.0;
+    hb_moments_finalize_kernel<<<1, HB_NMOM * 32, 0, s>>>(partials, nblocks, n, pv, d_out27);
+    return cudaGetLastError();
+}

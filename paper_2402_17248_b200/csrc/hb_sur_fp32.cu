@@ -1,0 +1,159 @@
+// hb_sur_fp32.cu -- surrogate stage on the CUDA cores (HB_PREC_FP32): rows a4-a6 with an FFMA GEMM chain.
+//
+// One block owns a tile of TP particles.  Activations live in shared memory as [feature][particle]
+// (two ping-pong buffers); the transposed weights W^T [k][n] (packed, zero-padded to 64 outputs, by
+// hb_api.cu) are streamed through a [32][64] shared slab.  Each thread owns a 4-particle x 4-output
+// register tile.  Partial sums of each 32-wide K chunk are formed separately and then added (shorter
+// rounding chains), bias is added last in fp32, tanh is tanhf.
+// Prologue (s->t R6, normalise R8) and epilogue (de-normalise R8, reference R7, t->s R6, moments R10)
+// are fused: hidden activations never touch HBM (data preparation is 1-2 % of the push).
+#include "hb_device.cuh"
+
+#define KC 32
+#define OC 64
+
+template <int TP, int ACT, bool MOM>
+__global__ void __launch_bounds__((TP / 4) * 16, 1)
+hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, int hmax, double* __restrict__ partials) {
+    constexpr int NT = (TP / 4) * 16;
+    extern __shared__ __align__(16) float smem[];
+    float* actA = smem;                          // [hmax][TP]
+    float* actB = actA + (size_t)hmax * TP;      // [hmax][TP]
+    float* Ws = actB + (size_t)hmax * TP;        // [KC][OC]
+    double* red = reinterpret_cast<double*>(Ws + KC * OC);
+
+    const int tid = threadIdx.x;
+    const int og = tid & 15, pg = tid >> 4;
+    HbMomAcc acc;
+    if (MOM) acc.clear();
+    const size_t ntiles = (n + TP - 1) / TP;
+
+    for (size_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const size_t i0 = tile * TP;
+        __syncthreads();
+        if (tid < TP) {
+            const size_t i = i0 + tid;
+            float nin[6] = {0, 0, 0, 0, 0, 0};
+            if (i < n) hb_sur_prologue(sd, p.v[0][i], p.v[1][i], p.v[2][i], p.v[3][i], p.v[4][i], p.v[5][i], nin);
+#pragma unroll
+            for (int j = 0; j < 6; ++j) actA[j * TP + tid] = nin[j];
+        }
+        float* in = actA;
+        float* out = actB;
+        for (int l = 0; l < sd.n_linear; ++l) {
+            const int K = sd.widths[l], npad = sd.npad32[l];
+            const float* __restrict__ Wt = sd.w32 + sd.w32_off[l];
+            const float* __restrict__ bias = sd.b32 + sd.b32_off[l];
+            const bool last = (l == sd.n_linear - 1);
+            const float slope = sd.prelu[l];
+            for (int o0 = 0; o0 < npad; o0 += OC) {
+                float tot[4][4];
+#pragma unroll
+                for (int a = 0; a < 4; ++a)
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) tot[a][b] = 0.0f;
+                for (int k0 = 0; k0 < K; k0 += KC) {
+                    const int kk = min(KC, K - k0);
+                    __syncthreads();          // previous slab consumed; layer input complete
+                    for (int idx = tid; idx < kk * (OC / 4); idx += NT) {
+                        const int k = idx / (OC / 4), c4 = idx % (OC / 4);
+                        reinterpret_cast<float4*>(Ws)[k * (OC / 4) + c4] =
+                            __ldg(reinterpret_cast<const float4*>(Wt + (size_t)(k0 + k) * npad + o0) + c4);
+                    }
+                    __syncthreads();
+                    float part[4][4];
+#pragma unroll
+                    for (int a = 0; a < 4; ++a)
+#pragma unroll
+                        for (int b = 0; b < 4; ++b) part[a][b] = 0.0f;
+#pragma unroll 8
+                    for (int k = 0; k < kk; ++k) {
+                        const float4 av = *reinterpret_cast<const float4*>(in + (size_t)(k0 + k) * TP + 4 * pg);
+                        const float4 wv = *reinterpret_cast<const float4*>(Ws + k * OC + 4 * og);
+                        const float a4[4] = {av.x, av.y, av.z, av.w};
+                        const float w4[4] = {wv.x, wv.y, wv.z, wv.w};
+#pragma unroll
+                        for (int a = 0; a < 4; ++a)
+#pragma unroll
+                            for (int b = 0; b < 4; ++b) part[a][b] = fmaf(a4[a], w4[b], part[a][b]);
+                    }
+#pragma unroll
+                    for (int a = 0; a < 4; ++a)
+#pragma unroll
+                        for (int b = 0; b < 4; ++b) tot[a][b] += part[a][b];
+                }
+                const float4 bv = __ldg(reinterpret_cast<const float4*>(bias + o0) + og);
+                const float b4[4] = {bv.x, bv.y, bv.z, bv.w};
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    float r[4];
+#pragma unroll
+                    for (int a = 0; a < 4; ++a) {
+                        const float z = tot[a][b] + b4[b];
+                        r[a] = last ? z : hb_activate<ACT, false>(z, slope);
+                    }
+                    *reinterpret_cast<float4*>(out + (size_t)(o0 + 4 * og + b) * TP + 4 * pg) =
+                        make_float4(r[0], r[1], r[2], r[3]);
+                }
+            }
+            float* tmp = in; in = out; out = tmp;
+        }
+        __syncthreads();
+        if (tid < TP) {
+            const size_t i = i0 + tid;
+            if (i < n) {
+                float w[6];
+#pragma unroll
+                for (int j = 0; j < 6; ++j) w[j] = in[j * TP + tid];
+                float x, px, y, py, t, pt;
+                hb_sur_epilogue(sd, w, x, px, y, py, t, pt);
+                p.v[0][i] = x; p.v[1][i] = px; p.v[2][i] = y; p.v[3][i] = py; p.v[4][i] = t; p.v[5][i] = pt;
+                if (MOM) acc.add(x, px, y, py, t, pt);
+            }
+        }
+    }
+    if (MOM) {
+        __syncthreads();
+        hb_block_reduce_moments(acc, red, partials + (size_t)blockIdx.x * HB_NMOM, tid, NT, 1);
+    }
+}
+
+template <int TP, bool MOM>
+static cudaError_t launch_tp(const HbParticles& p, size_t n, const HbSurDev& sd, int hmax, double* partials,
+                             int grid, cudaStream_t s) {
+    constexpr int NT = (TP / 4) * 16;
+    const size_t smem = ((size_t)2 * hmax * TP + KC * OC) * sizeof(float) + (NT / 32) * HB_NMOM * sizeof(double);
+#define HB_LAUNCH_ACT(A)                                                                                         \
+    {                                                                                                            \
+        cudaError_t e = cudaFuncSetAttribute(hb_sur_fp32_kernel<TP, A, MOM>,                                     \
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);            \
+        if (e != cudaSuccess) return e;                                                                          \
+        hb_sur_fp32_kernel<TP, A, MOM><<<grid, NT, smem, s>>>(p, n, sd, hmax, partials);                         \
+    }
+    switch (sd.act) {
+    case 0: HB_LAUNCH_ACT(0) break;
+    case 1: HB_LAUNCH_ACT(1) break;
+    case 2: HB_LAUNCH_ACT(2) break;
+    default: HB_LAUNCH_ACT(3) break;
+    }
+#undef HB_LAUNCH_ACT
+    return cudaGetLastError();
+}
+
+cudaError_t hb_launch_sur_fp32(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials,
+                               int* nblocks_out, int sm_count, cudaStream_t s) {
+    int hmax = 64;
+    for (int l = 0; l < sd.n_linear; ++l) hmax = hmax > sd.npad32[l] ? hmax : sd.npad32[l];
+    // tile size: two activation buffers of hmax x TP floats must fit beside the weight slab
+    int tp = hmax <= 384 ? 64 : (hmax <= 768 ? 32 : 16);
+    const size_t ntiles = (n + tp - 1) / tp;
+    size_t g = (size_t)sm_count * (tp == 64 ? 1 : 1);
+    if (g > ntiles) g = ntiles;
+    if (g < 1) g = 1;
+    const int grid = (int)g;
+    if (nblocks_out) *nblocks_out = grid;
+    const bool mom = partials != nullptr;
+    if (tp == 64) return mom ? launch_tp<64, true>(p, n, sd, hmax, partials, grid, s) : launch_tp<64, false>(p, n, sd, hmax, partials, grid, s);
+    if (tp == 32) return mom ? launch_tp<32, true>(p, n, sd, hmax, partials, grid, s) : launch_tp<32, false>(p, n, sd, hmax, partials, grid, s);
+    return mom ? launch_tp<16, true>(p, n, sd, hmax, partials, grid, s) : launch_tp<16, false>(p, n, sd, hmax, partials, grid, s);
+}

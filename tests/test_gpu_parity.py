@@ -1,0 +1,287 @@
+"""GPU-vs-oracle parity through the C ABI (run with -m gpu on a B200).
+
+Tolerances (BASELINE.json north_star): max |gpu - oracle| <= 1e-6 x std(oracle coordinate) for fp32
+element maps, <= 1e-5 for the fp32 surrogate path, <= 2e-2 for the 16-bit tensor-core path; moments
+within 1e-4 relative.  "std" = centred std of the oracle's output coordinate (G14).
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def hb():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2402_17248_b200 as hb
+    hb.lib()
+    return hb
+
+
+def gpu_push(hb, desc, x, run_mode="composed", moments=True, prec=None):
+    import torch
+    lat = hb.Lattice.from_description(desc, run_mode=run_mode, device=0, prec=prec)
+    c = torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    rec = None
+    if moments:
+        rec = lat.push_moments(c)
+    else:
+        lat.push(c)
+    torch.cuda.synchronize()
+    out = c.cpu().numpy().astype(np.float64)
+    rec = None if rec is None else rec.cpu().numpy()
+    lat.close()
+    return out, rec
+
+
+def rel_err(got, ref):
+    return np.max(np.abs(got - ref), axis=1) / ref.std(axis=1)
+
+
+def sym(rec):
+    C = np.zeros((6, 6))
+    C[np.triu_indices(6)] = rec[6:]
+    return C + C.T - np.diag(np.diag(C))
+
+
+def moments_close(rec, ref, tol):
+    """means relative to sigma, second moments relative to sqrt(C_jj C_kk)"""
+    C, R = sym(rec), sym(ref)
+    sd = np.sqrt(np.diag(R))
+    assert np.max(np.abs(rec[:6] - ref[:6]) / sd) <= tol
+    assert np.max(np.abs(C - R) / np.outer(sd, sd)) <= tol
+
+
+# --------------------------------------------------------------------------------- a2: conventional runs
+@pytest.mark.parametrize("mode,tol", [("composed", 1e-6), ("sequential", 1e-6)])
+@pytest.mark.parametrize("n", [1, 3, 4, 5, 1023, 4096, 100003])
+def test_run_parity_small(hb, mode, tol, n):
+    desc = wl.lattice(wl.fodo_cell(1.0) + wl.c4_transport() + [wl.monitor()])
+    x = wl.gaussian_bunch(max(n, 8), 11)[:, :n].copy()
+    ref, ref_rec = oracle.push(desc, x)
+    got, rec = gpu_push(hb, desc, x, run_mode=mode)
+    if n >= 1000:
+        assert rel_err(got, ref).max() <= tol
+        moments_close(rec[0], ref_rec[0], 1e-4)
+    else:
+        scale = wl.NOMINAL_SIGMA[:, None] * 5
+        assert np.max(np.abs(got - ref) / scale) <= tol
+
+
+@pytest.mark.parametrize("mode", ["composed", "sequential"])
+def test_config2_parity_and_emittance(hb, mode):
+    desc, x = wl.config2()
+    ref, ref_rec = oracle.push(desc, x)
+    got, rec = gpu_push(hb, desc, x, run_mode=mode)
+    e = rel_err(got, ref)
+    print("C2", mode, "max err/std per coordinate:", e)
+    assert e.max() <= 1e-6
+    moments_close(rec[0], ref_rec[0], 1e-4)
+    # the GPU's fused fp64 moments equal the fp64 moments of the GPU's own fp32 output (pure reduction check)
+    own = oracle.moments(np.ascontiguousarray(got))
+    moments_close(rec[0], own, 1e-10)
+    # rms emittance from the GPU record vs oracle
+    for j in (0, 2):
+        C, R = sym(rec[0]), sym(ref_rec[0])
+        eg = math.sqrt(C[j, j] * C[j + 1, j + 1] - C[j, j + 1] ** 2)
+        eo = math.sqrt(R[j, j] * R[j + 1, j + 1] - R[j, j + 1] ** 2)
+        assert abs(eg / eo - 1) <= 1e-4
+
+
+def test_sequential_fp32_reported_not_bounded(hb):
+    """HB_RUN_SEQUENTIAL_FP32 is the literal 'fp32 registers' reading; its error grows with run length
+    (DESIGN.md): report it, require only that it stays within 2e-4 over 500 elements."""
+    desc, x = wl.config2(n=200_000)
+    ref, _ = oracle.push(desc, x)
+    got, _ = gpu_push(hb, desc, x, run_mode="sequential_fp32", moments=False)
+    e = rel_err(got, ref)
+    print("C2 sequential_fp32 max err/std:", e)
+    assert e.max() <= 2e-4
+
+
+def test_drift_roundtrip_identity_on_gpu(hb):
+    desc = wl.lattice([wl.drift(0.7), wl.drift(-0.7)])
+    x = wl.gaussian_bunch(4096, 5)
+    got, _ = gpu_push(hb, desc, x, moments=False)
+    assert np.array_equal(got.astype(np.float32), x)          # composed run = identity matrix exactly
+    got, _ = gpu_push(hb, desc, x, run_mode="sequential", moments=False)
+    assert np.max(np.abs(got - x) / wl.NOMINAL_SIGMA[:, None]) < 1e-6
+
+
+def test_long_run_500_elements_and_single_element(hb):
+    desc = wl.lattice([wl.quad(0.1, 1.2)])
+    x = wl.gaussian_bunch(5000, 6)
+    ref, _ = oracle.push(desc, x)
+    for mode in ("composed", "sequential"):
+        got, _ = gpu_push(hb, desc, x, run_mode=mode, moments=False)
+        assert rel_err(got, ref).max() <= 1e-6
+
+
+# --------------------------------------------------------------------------------- a3: moments
+@pytest.mark.parametrize("n", [1, 2, 7, 4096, 1_000_003])
+def test_standalone_moments(hb, n):
+    import torch
+    x = wl.gaussian_bunch(max(n, 8), 21)[:, :n].copy() + (np.arange(6, dtype=np.float32)[:, None] * 1e-3)
+    ref = oracle.moments(np.ascontiguousarray(x.astype(np.float64)))
+    c = torch.from_numpy(x).cuda()
+    for pivot in (None, list(np.arange(6) * 1e-3)):
+        rec = hb.moments(c, pivot=pivot).cpu().numpy()
+        assert np.allclose(rec[:6], ref[:6], rtol=1e-12, atol=1e-18)
+        if n > 1:
+            C, R = sym(rec), sym(ref)
+            sd = np.sqrt(np.diag(R))
+            assert np.max(np.abs(C - R) / np.outer(sd, sd)) < 1e-9
+    assert np.array_equal(c.cpu().numpy(), x)                 # read-only
+
+
+def test_monitor_without_producer_and_double_monitor(hb):
+    desc = wl.lattice([wl.monitor(), wl.drift(1.0), wl.monitor(), wl.monitor()])
+    x = wl.gaussian_bunch(10_001, 8)
+    ref, ref_rec = oracle.push(desc, x)
+    got, rec = gpu_push(hb, desc, x)
+    assert rec.shape == (3, 27)
+    for k in range(3):
+        moments_close(rec[k], ref_rec[k], 1e-6)
+    assert np.allclose(rec[1], rec[2], rtol=1e-12, atol=1e-30)
+
+
+# --------------------------------------------------------------------------------- a4-a6: fp32 surrogate
+def test_config1_fp32_per_segment(hb):
+    desc, x = wl.config1(prec="fp32")
+    states = []
+    ref, ref_rec = oracle.push(desc, x, on_element=lambda i, el, c: states.append(c.copy()) if el["kind"] == "monitor" else None)
+    got, rec = gpu_push(hb, desc, x)
+    e = rel_err(got, ref)
+    print("C1 fp32 end-to-end err/std:", e)
+    assert e.max() <= 1e-5
+    for k in range(3):
+        moments_close(rec[k], ref_rec[k], 1e-4)
+    # segment 1 alone (conventional): 1e-6
+    cell = wl.lattice(desc["elements"][:5])
+    g1, _ = gpu_push(hb, cell, x, moments=False)
+    assert rel_err(g1, states[0]).max() <= 1e-6
+
+
+@pytest.mark.parametrize("act", ["identity", "relu", "prelu", "tanh"])
+@pytest.mark.parametrize("widths", [[6, 6], [6, 7, 6], [6, 64, 64, 6], [6, 100, 37, 6], [6, 256, 256, 256, 6]])
+def test_fp32_surrogate_shapes(hb, act, widths):
+    n = 3001
+    W, b = wl.make_mlp(widths, "he" if act in ("relu", "prelu") else "xavier", 77, len(widths))
+    rng = np.random.default_rng(5)
+    a = rng.uniform(0.05, 0.3, len(widths) - 2).astype(np.float32) if act == "prelu" else None
+    sur = wl.surrogate(widths, W, b, act, rng.normal(size=6) * 1e-4, wl.NOMINAL_SIGMA, rng.normal(size=6),
+                       rng.uniform(0.5, 2.0, 6), prelu_a=a)
+    desc = wl.lattice([sur, wl.monitor()])
+    x = wl.gaussian_bunch(n, 31)
+    ref, ref_rec = oracle.push(desc, x)
+    got, rec = gpu_push(hb, desc, x)
+    e = rel_err(got, ref)
+    assert e.max() <= 1e-5, e
+    moments_close(rec[0], ref_rec[0], 1e-4)
+
+
+def test_fp32_identity_initialised_net(hb):
+    H = 64
+    A0 = np.zeros((H, 6), np.float32); A0[:6] = np.eye(6)
+    A1 = np.zeros((H, H), np.float32); A1[:6, :6] = np.eye(6)
+    A2 = np.zeros((6, H), np.float32); A2[:, :6] = np.eye(6)
+    zb = [np.zeros(H, np.float32), np.zeros(H, np.float32), np.zeros(6, np.float32)]
+    z, o = np.zeros(6), np.ones(6)
+    sur = wl.surrogate([6, H, H, 6], [A0, A1, A2], zb, "prelu", z, o, z, o, prelu_a=[1.0, 1.0])
+    x = wl.gaussian_bunch(1000, 3, sigma=np.ones(6))
+    got, _ = gpu_push(hb, wl.lattice([sur]), x, moments=False)
+    assert np.array_equal(got.astype(np.float32), x)
+
+
+def test_fp32_coord_t_stage(hb):
+    desc, x = wl.config4(prec="fp32", n=20_000, stages=2)
+    ref, ref_rec = oracle.push(desc, x)
+    got, rec = gpu_push(hb, desc, x)
+    assert np.all(np.isfinite(got))
+    e = rel_err(got, ref)
+    print("C4 fp32 (2 stages, free running) err/std:", e)
+    assert e.max() <= 1e-4       # two stages compound; the per-stage bound is checked below
+    # per-stage: stage 1 only
+    d1 = wl.lattice(desc["elements"][:1])
+    r1, _ = oracle.push(d1, x)
+    g1, _ = gpu_push(hb, d1, x, moments=False)
+    e1 = rel_err(g1, r1)
+    print("C4 fp32 stage 1 err/std:", e1)
+    assert e1.max() <= 1e-5
+    for k in range(4):
+        moments_close(rec[k], ref_rec[k], 1e-4)
+
+
+def test_cross_pin_linear_surrogate_equals_run_kernel(hb):
+    """ties a5 to a2: identity-activation 1-layer surrogate with A = D^-1 M D reproduces the run kernel."""
+    els = wl.fodo_cell(1.2)
+    c = np.zeros((6, 6)); c[:] = np.eye(6)
+    M, _ = oracle.push(wl.lattice(els), c)
+    sd = wl.NOMINAL_SIGMA
+    A = (np.diag(1 / sd) @ M @ np.diag(sd)).astype(np.float32)
+    sur = wl.surrogate([6, 6], [A], [np.zeros(6, np.float32)], "identity", np.zeros(6), sd, np.zeros(6), sd)
+    x = wl.gaussian_bunch(4096, 9)
+    g_run, _ = gpu_push(hb, wl.lattice(els), x, moments=False)
+    g_sur, _ = gpu_push(hb, wl.lattice([sur]), x, moments=False)
+    assert np.max(np.abs(g_run - g_sur) / sd[:, None]) < 2e-6
+
+
+# --------------------------------------------------------------------------------- boundary behaviour
+def test_abi_errors(hb):
+    import torch
+    lat = hb.Lattice(1000.0, wl.ELECTRON_MEV)
+    lat.add_element("drift", 1.0)
+    c = torch.zeros((6, 16), dtype=torch.float32, device="cuda")
+    with pytest.raises(hb.HbError) as ei:
+        lat.push(c)                                            # not finalized
+    assert ei.value.status == 2
+    lat.finalize(0)
+    with pytest.raises(hb.HbError) as ei:
+        lat.add_element("drift", 1.0)                          # finalized
+    assert ei.value.status == 2
+    lat.push(c)
+    big = torch.zeros(6 * 16 + 1, dtype=torch.float32, device="cuda")
+    mis = [big[1 + 16 * j: 1 + 16 * (j + 1)] for j in range(6)]   # 4-byte offset: misaligned
+    with pytest.raises(hb.HbError) as ei:
+        lat.push(mis)
+    assert ei.value.status == 1
+    alias = [c[0], c[0], c[2], c[3], c[4], c[5]]
+    with pytest.raises(hb.HbError) as ei:
+        lat.push(alias)
+    assert ei.value.status == 1
+    e = torch.zeros((6, 0), dtype=torch.float32, device="cuda")
+    lat.push(e)                                                # n = 0 is a no-op
+    lat.close()
+    with pytest.raises(hb.HbError):
+        hb.hb_lattice_create(-1.0, 0.511)
+    h = hb.hb_lattice_create(1000.0, 0.511)
+    with pytest.raises(hb.HbError):
+        hb.hb_lattice_add_element(h, "quad", -0.1, 1.0)
+    with pytest.raises(hb.HbError):
+        hb.hb_lattice_add_surrogate(h, [6, 8, 5], [np.zeros((8, 6), np.float32), np.zeros((5, 8), np.float32)],
+                                    [np.zeros(8, np.float32), np.zeros(5, np.float32)], "relu",
+                                    np.zeros(6), np.ones(6), np.zeros(6), np.ones(6))
+    hb.hb_lattice_destroy(h)
+
+
+def test_stream_ordering_and_inplace(hb):
+    import torch
+    desc = wl.lattice(wl.fodo_cell(1.2))
+    x = wl.gaussian_bunch(50_000, 13)
+    ref, _ = oracle.push(wl.lattice(wl.fodo_cell(1.2) * 2), x)
+    lat = hb.Lattice.from_description(desc, device=0)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        c = torch.from_numpy(x).cuda()
+        lat.push(c)
+        lat.push(c)                                            # back-to-back on a non-default stream
+    s.synchronize()
+    got = c.cpu().numpy().astype(np.float64)
+    assert rel_err(got, ref).max() <= 2e-6
+    lat.close()

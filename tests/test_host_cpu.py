@@ -1,0 +1,90 @@
+"""CPU-only checks of the boundary: the library loads, exports every symbol of include/hb.h,
+validates arguments on the host, and fails loudly (never falls back) without a device."""
+import os
+import re
+
+import numpy as np
+import pytest
+
+import workloads as wl
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def hb():
+    from paper_2402_17248_b200.build import build_lib
+    build_lib()
+    import paper_2402_17248_b200 as hb
+    hb.lib()
+    return hb
+
+
+def test_every_declared_symbol_is_exported(hb):
+    hdr = open(os.path.join(ROOT, "include", "hb.h")).read()
+    declared = set(re.findall(r"\b(hb_[a-z0-9_]+)\s*\(", hdr))
+    assert declared, "no declarations parsed"
+    assert declared == set(hb.EXPORTED_SYMBOLS)
+    L = hb.lib()
+    for name in declared:
+        assert getattr(L, name) is not None
+
+
+def test_host_validation_without_device(hb):
+    assert hb.hb_status_string(0) == "HB_OK" and hb.hb_status_string(5) == "HB_ERR_UNSUPPORTED"
+    with pytest.raises(hb.HbError) as e:
+        hb.hb_lattice_create(float("nan"), 0.511)
+    assert e.value.status == 1
+    h = hb.hb_lattice_create(1000.0, wl.ELECTRON_MEV)
+    hb.hb_lattice_add_element(h, "drift", -0.5)                 # negative drift length is legal
+    hb.hb_lattice_add_element(h, "monitor")
+    with pytest.raises(hb.HbError):
+        hb.hb_lattice_add_element(h, "sbend", -0.5, 0.01)
+    with pytest.raises(hb.HbError):
+        hb.hb_lattice_add_element(h, "quad", 0.1, float("inf"))
+    W, b = wl.make_mlp([6, 8, 6], "xavier", 1, 0)
+    z, o = np.zeros(6), np.ones(6)
+    hb.hb_lattice_add_surrogate(h, [6, 8, 6], W, b, "tanh", z, o, z, o)
+    with pytest.raises(hb.HbError):
+        hb.hb_lattice_add_surrogate(h, [6, 8, 6], W, b, "tanh", z, np.array([1, 1, 0, 1, 1, 1.0]), z, o)
+    with pytest.raises(hb.HbError):
+        hb.hb_lattice_add_surrogate(h, [6, 8, 6], W, b, "prelu", z, o, z, o)      # slopes missing
+    assert hb.hb_lattice_num_monitors(h) == 1
+    hb.hb_lattice_destroy(h)
+
+
+def test_no_cpu_fallback(hb):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("device present")
+    h = hb.hb_lattice_create(1000.0, wl.ELECTRON_MEV)
+    hb.hb_lattice_add_element(h, "drift", 1.0)
+    with pytest.raises(hb.HbError) as e:
+        hb.hb_lattice_finalize(h, 0)
+    assert e.value.status in (4, 5)
+    with pytest.raises(hb.HbError) as e:
+        hb.hb_push(h, 0, 0, 0, 0, 0, 0, 0, 0)
+    assert e.value.status == 2
+    hb.hb_lattice_destroy(h)
+
+
+def test_product_never_imports_oracle():
+    pkg = os.path.join(ROOT, "paper_2402_17248_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in src.replace("the oracle", "").replace("oracle/", "").replace("by the oracle", ""), f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            src = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2402_17248_b200" not in src and "libhb" not in src
+
+
+def test_shard_ranges_cover_everything():
+    for n in (0, 1, 7, 10_000_001):
+        for w in (1, 2, 3, 8):
+            r = [wl.shard_range(n, k, w) for k in range(w)]
+            assert r[0][0] == 0 and r[-1][1] == n
+            assert all(a[1] == b[0] for a, b in zip(r[:-1], r[1:]))
+            assert max(b - a for a, b in r) - min(b - a for a, b in r) <= 1
