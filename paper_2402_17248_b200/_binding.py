@@ -223,6 +223,22 @@ def _stream(dev):
     return torch.cuda.current_stream(dev).cuda_stream
 
 
+def to_device(x, device="cuda"):
+    """numpy/torch [6, n] float32 -> list of six 16-byte-aligned CUDA row views (row pitch padded to 4 floats)."""
+    import torch
+    t = torch.as_tensor(x, dtype=torch.float32)
+    n = t.shape[1]
+    pitch = (n + 3) // 4 * 4
+    buf = torch.zeros((6, max(pitch, 4)), dtype=torch.float32, device=device)
+    buf[:, :n] = t.to(device)
+    return [buf[j, :n] for j in range(6)]
+
+
+def to_host(rows):
+    import torch
+    return torch.stack([r for r in rows]).cpu().numpy()
+
+
 class Lattice:
     """Owning wrapper of an hb_lattice.  `Lattice.from_description(desc)` consumes the plain-data lattice
     description of workloads/ (also consumed, independently, by the oracle)."""

@@ -27,14 +27,14 @@ def hb():
 def gpu_push(hb, desc, x, run_mode="composed", moments=True, prec=None):
     import torch
     lat = hb.Lattice.from_description(desc, run_mode=run_mode, device=0, prec=prec)
-    c = torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    c = hb.to_device(x)
     rec = None
     if moments:
         rec = lat.push_moments(c)
     else:
         lat.push(c)
     torch.cuda.synchronize()
-    out = c.cpu().numpy().astype(np.float64)
+    out = hb.to_host(c).astype(np.float64)
     rec = None if rec is None else rec.cpu().numpy()
     lat.close()
     return out, rec
@@ -129,7 +129,7 @@ def test_standalone_moments(hb, n):
     import torch
     x = wl.gaussian_bunch(max(n, 8), 21)[:, :n].copy() + (np.arange(6, dtype=np.float32)[:, None] * 1e-3)
     ref = oracle.moments(np.ascontiguousarray(x.astype(np.float64)))
-    c = torch.from_numpy(x).cuda()
+    c = hb.to_device(x)
     for pivot in (None, list(np.arange(6) * 1e-3)):
         rec = hb.moments(c, pivot=pivot).cpu().numpy()
         assert np.allclose(rec[:6], ref[:6], rtol=1e-12, atol=1e-18)
@@ -137,7 +137,7 @@ def test_standalone_moments(hb, n):
             C, R = sym(rec), sym(ref)
             sd = np.sqrt(np.diag(R))
             assert np.max(np.abs(C - R) / np.outer(sd, sd)) < 1e-9
-    assert np.array_equal(c.cpu().numpy(), x)                 # read-only
+    assert np.array_equal(hb.to_host(c), x)                   # read-only
 
 
 def test_monitor_without_producer_and_double_monitor(hb):
