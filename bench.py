@@ -1,0 +1,422 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the hybrid-beamline hot path on B200 (one process per GPU).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3|C4|C2|C5] [--impl hb|reference]
+
+A step = one hb_push_moments of the whole lattice of the workload over one resident bunch.  Default
+workload = BASELINE.json config 3 ("surrogate particles/s at 1e7; % of tensor peak": N = 1e7,
+6-256^3-6 ReLU, bf16 tensor cores, moments after the stage).  The conventional-run kernel of the same
+metric ("particle-element pushes/s; % of HBM peak") is measured in the same run at N = 1e7 and reported
+under "kernels" with its own roofline, as are the f16 / fp32 variants and the C4 hybrid lattice.
+Inputs (240 MB) exceed L2 (126 MB) and L2 is flushed between timed steps; the bunch is restored from a
+pristine device copy before every step (outside the timed region) because the push is in place.
+Timing: CUDA events on the launching stream, per step, summed; max over ranks.  One JSON line on stdout.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as wl  # noqa: E402
+
+METRIC = "particle-element pushes/s & surrogate particles/s at 1e7; % of HBM/tensor peak"
+L2_FLUSH_BYTES = 256 << 20
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": d["hbm_gbs"], "bf16_tflops": d["bf16_tflops"],
+                "bf16_tflops_sustained": d.get("bf16_tflops_sustained", d["bf16_tflops"]), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks line of B200_PROFILING.md, sampled every 200 ms during the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "200"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def build_workload(name, prec, n):
+    if name == "C3":
+        desc, x = wl.config3(prec=prec, n=n or 10_000_000)
+        label = "C3 surrogate-only: N=%d correlated Gaussian, MLP 6-256-256-256-6 ReLU He, %s, monitor after stage"
+    elif name == "C4":
+        desc, x = wl.config4(prec=prec, n=n or 10_000_000)
+        label = "C4 hybrid: N=%d, 2 x [surrogate 6-128^3-6 tanh COORD_T %s + 9-element transport + 4-sbend chicane], 4 monitors"
+    elif name == "C2":
+        desc, x = wl.config2(n=n or 10_000_000)
+        label = "C2 conventional-only: N=%d, 100 FODO cells (one fused run of 500 elements)%s, 1 monitor"
+        prec = ""
+    elif name == "C5":
+        desc, x = wl.config5(prec=prec, n=n or 100_000_000)
+        label = "C5 large bunch: N=%d, 9 x surrogate 6-512^4-6 tanh %s + 8 x 10 FODO cells, 17 monitors"
+    else:
+        raise SystemExit("unknown workload " + name)
+    return desc, x, label % (x.shape[1], prec)
+
+
+def count_work(desc):
+    n_sur = sum(1 for e in desc["elements"] if e["kind"] == "surrogate")
+    n_el = sum(1 for e in desc["elements"] if e["kind"] in ("drift", "quad", "sbend"))
+    flops = sum(wl.flops_per_particle(e["widths"]) for e in desc["elements"] if e["kind"] == "surrogate")
+    return n_sur, n_el, flops
+
+
+def segment_kinds(desc):
+    """segment list as the library splits it: 'run' | 'sur' | 'mon' (standalone monitor)"""
+    kinds, prev = [], None
+    for e in desc["elements"]:
+        k = e["kind"]
+        if k == "monitor":
+            if prev in ("run", "sur"):
+                prev = "fusedmon"
+            else:
+                kinds.append("mon"); prev = "mon"
+        elif k == "surrogate":
+            kinds.append("sur"); prev = "sur"
+        else:
+            if prev != "run":
+                kinds.append("run")
+            prev = "run"
+    return kinds
+
+
+def timed_steps(torch, hb, lat, pristine, work, steps, warmup, flush, with_moments=True, segtimes=False):
+    """returns (total_ms over `steps`, per-segment mean ms or None)"""
+    rec = torch.empty((max(lat.num_monitors, 1), 27), dtype=torch.float64, device=work.device)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    seg_acc = None
+    if segtimes:
+        lat.enable_timing(True)
+    for it in range(warmup + steps):
+        work.copy_(pristine)
+        flush.fill_(it & 0xff)                   # L2 flush: write a buffer larger than L2
+        k = it - warmup
+        if k >= 0:
+            ev[k][0].record()
+        if with_moments:
+            lat.push_moments(work, out=rec)
+        else:
+            lat.push(work)
+        if k >= 0:
+            ev[k][1].record()
+            if segtimes:
+                t = np.array(lat.segment_times_ms())
+                seg_acc = t if seg_acc is None else seg_acc + t
+    torch.cuda.synchronize()
+    if segtimes:
+        lat.enable_timing(False)
+    total = sum(a.elapsed_time(b) for a, b in ev)
+    return total, (None if seg_acc is None else seg_acc / steps), rec
+
+
+def oracle_rate(desc, x, budget_s, unit_count):
+    """oracle (as it stands) on a bounded sample; returns (units/s, cores, sample description)"""
+    import oracle
+    n = x.shape[1]
+    probe = min(n, 4096)
+    t0 = time.perf_counter()
+    oracle.push(desc, x[:, :probe])
+    dt = max(time.perf_counter() - t0, 1e-4)
+    ns = int(min(n, max(probe, (probe / dt) * budget_s)))
+    ns = min(ns, 1 << 20)
+    t0 = time.perf_counter()
+    oracle.push(desc, x[:, :ns])
+    dt = time.perf_counter() - t0
+    return unit_count * ns / dt, oracle.num_threads(), "first %d particles of the workload, whole lattice, %.1f s" % (ns, dt)
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the fp64 oracle on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    import oracle
+    desc, x, label = build_workload(args.workload, args.prec, args.n)
+    n_sur, n_el, flops = count_work(desc)
+    units = n_sur if n_sur else n_el
+    probe = min(x.shape[1], 2048)
+    t0 = time.perf_counter()
+    oracle.push(desc, x[:, :probe])
+    rate = probe / max(time.perf_counter() - t0, 1e-4)
+    per_step_s = max(0.5, min(10.0, 100.0 / (args.steps + args.warmup)))
+    ns = int(max(256, min(x.shape[1], rate * per_step_s, 1 << 19)))
+    xs = np.ascontiguousarray(x[:, :ns])
+    for _ in range(args.warmup):
+        oracle.push(desc, xs)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.push(desc, xs)
+    dt = time.perf_counter() - t0
+    value = units * ns * args.steps / dt
+    unit = "surrogate particle-inferences/s" if n_sur else "particle-element pushes/s"
+    sample = "each step = first %d particles of the workload through the whole lattice" % ns
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": unit, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded; see DESIGN.md)",
+        "config": {"workload": label, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": unit, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def kernel_extras(torch, hb, args, pk, flush, dev):
+    """per-kernel measurements at N = 1e7 beside the headline step"""
+    out = []
+    n = args.n or 10_000_000
+    reps = 10
+
+    def measure(desc, xh, label, with_moments, steps=reps, run_mode="composed", prec=None):
+        lat = hb.Lattice.from_description(desc, run_mode=run_mode, device=dev.index, prec=prec)
+        pristine = torch.from_numpy(xh).to(dev)
+        work = torch.empty_like(pristine)
+        tot, seg, _ = timed_steps(torch, hb, lat, pristine, work, steps, 3, flush, with_moments=with_moments, segtimes=True)
+        lat.close()
+        del pristine, work
+        return tot / steps, seg
+
+    # (a) conventional run kernel, C2 lattice (500 elements) at N = 1e7: composed (HBM-bound)
+    desc2, x2 = wl.config2(n=n)
+    for mom in (False, True):
+        ms, seg = measure(desc2, x2, "run", mom)
+        k_ms = float(seg[0])
+        gbs = 48.0 * n / (k_ms * 1e-3) / 1e9
+        out.append({"kernel": "hb_run_composed_kernel" + ("<moments>" if mom else ""), "workload": "C2 lattice (500 elements, one run), N=%d" % n,
+                    "ms": k_ms, "particle_element_pushes_per_s": 500.0 * n / (k_ms * 1e-3),
+                    "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                                 "frac": gbs / pk["hbm_gbs"], "traffic": None, "peak_source": pk["source"]}})
+    # sequential (fp64 registers, ALU-bound): 2700 DFMA-class ops per particle
+    ms, seg = measure(desc2, x2, "run", False, steps=5, run_mode="sequential")
+    k_ms = float(seg[0])
+    dp_peak = 148 * 64 * 1.965e9 / 1e12   # 148 SMs x 64 DFMA lanes x max clock (TFMA/s), DESIGN.md
+    ach = 2700.0 * n / (k_ms * 1e-3) / 1e12
+    out.append({"kernel": "hb_run_sequential_kernel<double>", "workload": "C2 lattice, N=%d" % n, "ms": k_ms,
+                "particle_element_pushes_per_s": 500.0 * n / (k_ms * 1e-3),
+                "roofline": {"bound": "alu", "achieved": ach, "peak": dp_peak, "unit": "TFMA/s (fp64)", "frac": ach / dp_peak,
+                             "traffic": None}})
+    del x2
+    # (b) surrogate C3 in f16 (same instruction, same rate) and fp32 FFMA
+    if args.workload == "C3":
+        desc3, x3 = wl.config3(prec="f16", n=n)
+        fl = wl.flops_per_particle(desc3["elements"][0]["widths"])
+        ms, seg = measure(desc3, x3, "sur", True)
+        k_ms = float(seg[0])
+        tf = fl * n / (k_ms * 1e-3) / 1e12
+        out.append({"kernel": "hb_sur_tc_kernel<f16>", "workload": "C3, N=%d" % n, "ms": k_ms,
+                    "particle_inferences_per_s": n / (k_ms * 1e-3),
+                    "roofline": {"bound": "tensor", "achieved": tf, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
+                                 "frac": tf / pk["bf16_tflops"], "traffic": None, "peak_source": pk["source"]}})
+        ms, seg = measure(desc3, x3, "sur", True, steps=2, prec="fp32")
+        k_ms = float(seg[0])
+        fma_peak = 148 * 128 * 1.965e9 / 1e12
+        ach = 0.5 * fl * n / (k_ms * 1e-3) / 1e12
+        out.append({"kernel": "hb_sur_fp32_kernel", "workload": "C3, N=%d" % n, "ms": k_ms,
+                    "particle_inferences_per_s": n / (k_ms * 1e-3),
+                    "roofline": {"bound": "alu", "achieved": ach, "peak": fma_peak, "unit": "TFMA/s (fp32)",
+                                 "frac": ach / fma_peak, "traffic": None}})
+        del x3
+        # (c) C4 hybrid lattice (all rows a1-a7 in one push)
+        desc4, x4 = wl.config4(prec="bf16", n=n)
+        ms, seg = measure(desc4, x4, "c4", True)
+        fl4 = wl.flops_per_particle([6, 128, 128, 128, 6])
+        kinds = segment_kinds(desc4)
+        sur_ms = float(np.mean([t for t, k in zip(seg, kinds) if k == "sur"]))
+        run_ms = float(np.mean([t for t, k in zip(seg, kinds) if k == "run"]))
+        out.append({"kernel": "C4 whole push (2 surrogate + 2 run kernels + 4 moment finalizes)", "workload": "C4, N=%d" % n,
+                    "ms": ms, "particles_per_s": n / (ms * 1e-3), "surrogate_ms": sur_ms, "run_ms": run_ms,
+                    "surrogate_tflops": fl4 * n / (sur_ms * 1e-3) / 1e12, "run_gbs": 48.0 * n / (run_ms * 1e-3) / 1e9})
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="hb", choices=["hb", "reference"])
+    ap.add_argument("--workload", default="C3")
+    ap.add_argument("--prec", default="bf16")
+    ap.add_argument("--n", type=int, default=0, help="override particle count (testing)")
+    ap.add_argument("--no-extras", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "hb" else args.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import paper_2402_17248_b200 as hb
+    hb.lib()                                   # fail loudly if the CUDA library is missing
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    pk = peaks()
+
+    desc, x, label = build_workload(args.workload, args.prec, args.n)
+    if world > 1:   # weak scaling: every rank pushes its own bunch of the full size (particles shard)
+        x = np.roll(x, rank * 1009, axis=1)
+    n = x.shape[1]
+    n_sur, n_el, flops = count_work(desc)
+    lat = hb.Lattice.from_description(desc, device=local)
+    host = torch.from_numpy(x).pin_memory()
+    pristine = host.to(dev)
+    work = torch.empty_like(pristine)
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+
+    # ---- timed region: K steps, device time, barrier + synchronize on both sides
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local)
+    total_ms, seg_ms, rec = timed_steps(torch, hb, lat, pristine, work, args.steps, args.warmup, flush, True, True)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop()
+    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    ms_step = total_ms / args.steps
+    assert bool(torch.isfinite(rec).all()), "non-finite moments"
+
+    # ---- end to end through the public API with HOST buffers (H2D + push + D2H inside the timed region)
+    e2e_steps = max(2, min(args.steps, 5))
+    host_out = torch.empty_like(host).pin_memory()
+    rec_host = torch.empty((max(lat.num_monitors, 1), 27), dtype=torch.float64).pin_memory()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for it in range(1 + e2e_steps):
+        if it == 1:
+            torch.cuda.synchronize()
+            e0.record()
+        work.copy_(host, non_blocking=True)
+        r = lat.push_moments(work)
+        host_out.copy_(work, non_blocking=True)
+        rec_host.copy_(r, non_blocking=True)
+    e1.record()
+    torch.cuda.synchronize()
+    e2e_ms = torch.tensor([e0.elapsed_time(e1) / e2e_steps], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(e2e_ms, op=dist.ReduceOp.MAX)
+    e2e_ms = float(e2e_ms.item())
+
+    units = n_sur if n_sur else n_el
+    unit = "surrogate particle-inferences/s" if n_sur else "particle-element pushes/s"
+    value = units * n * world / (ms_step * 1e-3)
+    e2e_value = units * n * world / (e2e_ms * 1e-3)
+
+    # ---- roofline of the dominant kernel (live per-segment CUDA-event times of the timed steps)
+    kinds = segment_kinds(desc)
+    dom = int(np.argmax(seg_ms))
+    dom_ms = float(seg_ms[dom])
+    if kinds[dom] == "sur":
+        per = flops / max(n_sur, 1)
+        ach = per * n / (dom_ms * 1e-3) / 1e12
+        roof = {"bound": "tensor", "achieved": ach, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
+                "frac": ach / pk["bf16_tflops"], "traffic": None, "kernel": "hb_sur_tc_kernel",
+                "kernel_ms": dom_ms, "peak_source": pk["source"] + " (burst, cuBLAS bf16)",
+                "frac_of_sustained": ach / pk["bf16_tflops_sustained"],
+                "algorithmic_flop_per_particle": per}
+    else:
+        ach = 48.0 * n / (dom_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "achieved": ach, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": ach / pk["hbm_gbs"],
+                "traffic": None, "kernel": "hb_run_composed_kernel", "kernel_ms": dom_ms, "peak_source": pk["source"]}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": args.prec if n_sur else "f32", "data": "synthetic (seeded; shapes of the paper's workloads, DESIGN.md)",
+        "config": {"workload": label, "l2": "inputs (%d MB) exceed L2 and a 256 MB buffer is written between timed steps" % (24 * n // 1000000),
+                   "timing": "CUDA events per step on the launching stream, summed; max over ranks", "parallelism": "particles sharded, no collective"},
+        "element_pushes_per_s": n_el * n * world / (ms_step * 1e-3),
+        "particles_per_s": n * world / (ms_step * 1e-3),
+        "segment_ms": [float(v) for v in seg_ms],
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": unit, "h2d_bytes_per_step": int(host.numel() * 4),
+                "d2h_bytes_per_step": int(host.numel() * 4 + rec_host.numel() * 8), "ms_per_step": e2e_ms},
+        "gpu_launches": int(args.steps * lat.num_launches(True)),
+        "roofline": roof,
+    }
+    lat.close()
+    del host_out
+    if rank == 0 and world == 1:
+        if not args.no_extras:
+            del pristine, work
+            line["kernels"] = kernel_extras(torch, hb, args, pk, flush, dev)
+        if not args.no_cpu_baseline:
+            v, cores, sample = oracle_rate(desc, x, 12.0, units)
+            line["cpu_baseline"] = {"value": v, "unit": unit, "cores": cores, "kind": "oracle", "sample": sample}
+            line["paper_context"] = "paper: 632 ms/stage at N=1e7 on 1 x A100 (PAPER.md P:197), 1.58e7 particle-inferences/s; other nets, other hardware"
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line))
+
+
+if __name__ == "__main__":
+    main()

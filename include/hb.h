@@ -147,6 +147,14 @@ hb_status hb_moments(const float *x, const float *px, const float *y, const floa
                      void *cuda_stream);
 size_t hb_moments_scratch_bytes(void);
 
+/* Optional per-segment device timing (observability; P:199 gives the paper's manual breakdown).  When on,
+ * every push records a CUDA event before the first and after each segment's kernels on the caller's stream.
+ * hb_lattice_get_timing synchronises on the last event of the most recent push and writes, for each of the
+ * n segments (runs, surrogate stages, standalone monitors, in lattice order; a fused monitor's finalize is
+ * counted with its segment), the elapsed milliseconds to ms_out[0..min(n,capacity)) and n to *n_out. */
+hb_status hb_lattice_enable_timing(hb_lattice *lat, int on);
+hb_status hb_lattice_get_timing(hb_lattice *lat, float *ms_out, int capacity, int *n_out);
+
 /* Destroy the lattice and free everything it owns (synchronises its device).  NULL is a no-op. */
 hb_status hb_lattice_destroy(hb_lattice *lat);
 

@@ -21,6 +21,7 @@ EXPORTED_SYMBOLS = [
     "hb_lattice_create", "hb_lattice_add_element", "hb_lattice_add_surrogate", "hb_lattice_set_run_mode",
     "hb_lattice_finalize", "hb_lattice_num_monitors", "hb_lattice_num_launches", "hb_lattice_ref_bg_out",
     "hb_push", "hb_push_moments", "hb_moments", "hb_moments_scratch_bytes", "hb_lattice_destroy",
+    "hb_lattice_enable_timing", "hb_lattice_get_timing",
     "hb_status_string", "hb_last_error", "hb_version",
 ]
 
@@ -80,6 +81,8 @@ def lib():
     L.hb_moments_scratch_bytes.restype = c_size_t
     L.hb_moments_scratch_bytes.argtypes = []
     L.hb_lattice_destroy.argtypes = [c_void_p]
+    L.hb_lattice_enable_timing.argtypes = [c_void_p, c_int]
+    L.hb_lattice_get_timing.argtypes = [c_void_p, POINTER(c_float), c_int, POINTER(c_int)]
     L.hb_status_string.restype = c_char_p
     L.hb_status_string.argtypes = [c_int]
     L.hb_last_error.restype = c_char_p
@@ -201,6 +204,19 @@ def hb_moments(x, px, y, py, t, pt, n: int, pivot, d_out27: int, d_scratch: int,
     _check(lib().hb_moments(x, px, y, py, t, pt, n, pv, d_out27, d_scratch, cuda_stream), "hb_moments")
 
 
+def hb_lattice_enable_timing(lat, on: bool = True):
+    _check(lib().hb_lattice_enable_timing(lat, int(bool(on))), "hb_lattice_enable_timing")
+
+
+def hb_lattice_get_timing(lat):
+    """milliseconds per segment of the most recent push (synchronises on its last event)"""
+    cap = 4096
+    buf = (c_float * cap)()
+    n = c_int()
+    _check(lib().hb_lattice_get_timing(lat, buf, cap, ctypes.byref(n)), "hb_lattice_get_timing")
+    return [buf[i] for i in range(min(n.value, cap))]
+
+
 def hb_lattice_destroy(lat):
     _check(lib().hb_lattice_destroy(lat), "hb_lattice_destroy")
 
@@ -308,6 +324,12 @@ class Lattice:
             out = torch.empty((m, 27), dtype=torch.float64, device=rows[0].device)
         hb_push_moments(self._h, *[r.data_ptr() for r in rows], n, out.data_ptr(), _stream(rows[0].device))
         return out
+
+    def enable_timing(self, on=True):
+        hb_lattice_enable_timing(self._h, on)
+
+    def segment_times_ms(self):
+        return hb_lattice_get_timing(self._h)
 
     def close(self):
         if self._h is not None:

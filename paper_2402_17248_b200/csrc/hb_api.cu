@@ -196,6 +196,9 @@ struct hb_lattice {
     HbSeqElem* d_seq = nullptr;
     double* d_partials = nullptr;
     std::vector<void*> d_bufs;
+    bool timing = false;
+    bool timing_valid = false;
+    std::vector<cudaEvent_t> events;   // segs.size() + 1 when timing is on
 };
 
 extern "C" {
@@ -552,6 +555,9 @@ static hb_status push_impl(hb_lattice* lat, float* x, float* px, float* y, float
         st = check_arrays(arr, n);
         HbParticles p;
         p.v[0] = x; p.v[1] = px; p.v[2] = y; p.v[3] = py; p.v[4] = t; p.v[5] = pt;
+        const bool timing = lat->timing && lat->events.size() == lat->segs.size() + 1;
+        lat->timing_valid = false;
+        if (timing) cudaEventRecord(lat->events[0], s);
         for (size_t k = 0; k < lat->segs.size() && st == HB_OK; ++k) {
             const Segment& g = lat->segs[k];
             const bool mom = want_moments && g.monitor >= 0;
@@ -573,7 +579,9 @@ static hb_status push_impl(hb_lattice* lat, float* x, float* px, float* y, float
                 e = hb_launch_moments_finalize(partials, nblocks, n, nullptr, d_moments + (size_t)g.monitor * HB_NMOM, s);
                 if (e != cudaSuccess) st = fail(HB_ERR_CUDA, "moments finalize: %s", cudaGetErrorString(e));
             }
+            if (timing) cudaEventRecord(lat->events[k + 1], s);
         }
+        if (timing && st == HB_OK) lat->timing_valid = true;
     }
     if (prev != lat->device) cudaSetDevice(prev);
     return st;
@@ -609,6 +617,33 @@ hb_status hb_moments(const float* x, const float* px, const float* y, const floa
     return HB_OK;
 }
 
+hb_status hb_lattice_enable_timing(hb_lattice* lat, int on) {
+    if (!lat) return fail(HB_ERR_INVALID_ARG, "lattice is NULL");
+    if (!lat->finalized) return fail(HB_ERR_STATE, "lattice not finalized");
+    int prev = 0;
+    HB_CUDA(cudaGetDevice(&prev));
+    HB_CUDA(cudaSetDevice(lat->device));
+    if (on && lat->events.empty()) {
+        lat->events.resize(lat->segs.size() + 1);
+        for (auto& ev : lat->events) HB_CUDA(cudaEventCreate(&ev));
+    }
+    lat->timing = on != 0;
+    lat->timing_valid = false;
+    cudaSetDevice(prev);
+    return HB_OK;
+}
+
+hb_status hb_lattice_get_timing(hb_lattice* lat, float* ms_out, int capacity, int* n_out) {
+    if (!lat || !n_out) return fail(HB_ERR_INVALID_ARG, "NULL argument");
+    if (!lat->finalized || !lat->timing || !lat->timing_valid) return fail(HB_ERR_STATE, "no timed push to report");
+    HB_CUDA(cudaEventSynchronize(lat->events.back()));
+    const int n = (int)lat->segs.size();
+    *n_out = n;
+    for (int k = 0; k < n && k < capacity && ms_out; ++k)
+        HB_CUDA(cudaEventElapsedTime(&ms_out[k], lat->events[k], lat->events[k + 1]));
+    return HB_OK;
+}
+
 hb_status hb_lattice_destroy(hb_lattice* lat) {
     if (!lat) return HB_OK;
     if (lat->finalized) {
@@ -616,6 +651,7 @@ hb_status hb_lattice_destroy(hb_lattice* lat) {
         cudaGetDevice(&prev);
         cudaSetDevice(lat->device);
         cudaDeviceSynchronize();
+        for (auto& ev : lat->events) cudaEventDestroy(ev);
         for (void* p : lat->d_bufs) cudaFree(p);
         cudaSetDevice(prev);
     }

@@ -73,7 +73,7 @@ def test_tc_tiles_and_tails(hb, n, force_cg, monkeypatch):
     else:
         monkeypatch.delenv("HB_TC_FORCE_CG", raising=False)
     desc, _ = wl.config1(prec="f16", n=8)
-    desc = wl.lattice(desc["elements"][5:7])          # surrogate + monitor
+    desc = wl.lattice(desc["elements"][6:8])          # surrogate + monitor
     x = wl.gaussian_bunch(max(n, 8), 17)[:, :n].copy()
     ref, ref_rec = oracle.push(desc, x)
     got, rec = gpu_push(hb, desc, x, moments=True)
