@@ -1,19 +1,24 @@
 // hb_sur_tc.cu -- surrogate stage on the 5th-gen tensor cores (HB_PREC_BF16 / HB_PREC_F16): rows a4-a6.
 //
-// Per 128-particle tile (one TMEM lane per particle):
-//   a4  bulk-async copies (TMA engine, cp.async.bulk + mbarrier complete_tx) stage the six coordinate
-//       rows of the tile in shared memory; worker threads convert s->t (R6, deviation form), normalise
-//       (R8), split each input into hi + lo 16-bit parts (K padded 6 -> 16) and write the A operand.
-//   a5  one elected thread issues tcgen05.mma (kind::f16, fp32 accumulate in TMEM) for L_0 .. L_l (Eq. 3);
-//       between layers the worker warps read the accumulator with tcgen05.ld, add the bias in fp32,
-//       apply sigma (Eq. 1/2 or tanh), round to 16 bit and write the next A operand straight into the
-//       128-byte-swizzled K-major shared-memory layout the MMA reads.  Hidden activations never leave
-//       the SM.
-//   a6  the last accumulator (6 of 16 columns) is de-normalised (R8), moved to the new reference and
-//       converted t->s (R6, R7), stored coalesced, and folded into the fp64 moment sums (R10).
-// Weights are packed on the host into the exact shared-memory image (hb_tc_pack_weights) and stay
-// resident in shared memory for the whole kernel.  CG = 2 pairs two SMs (cta_group::2, M = 256): each
-// CTA holds half of every weight matrix (N split), which is what lets 6-256^3-6 stay resident.
+// One 128-particle tile per CTA (one TMEM lane per particle; a CTA pair works on 256 particles with
+// cta_group::2).  Warp roles:
+//   warp 0      copy producer : weights once, then the six coordinate rows of each tile through the TMA
+//                               engine (cp.async.bulk + mbarrier complete_tx) into a 2-stage ring.
+//   warp 1      MMA issuer    : one elected thread (leader CTA of a pair) issues every tcgen05.mma.
+//   warps 4-7   IO warps      : a4 prologue (s->t R6 in deviation form, normalise R8, hi/lo split, layer-0
+//                               operand) of tile i+1, then a6 epilogue of tile i (tcgen05.ld of the 6 outputs,
+//                               de-normalise R8, reference update R7, t->s R6, coalesced store, fp64 moments R10).
+//   warps 8..   hidden-layer epilogue warps: tcgen05.ld of the accumulator, + bias (fp32), sigma (Eq. 1/2,
+//                               tanh), round to 16 bit, write the next A operand in the 128-byte-swizzled
+//                               K-major layout the MMA reads.  Hidden activations never leave the SM.
+// Pipeline (v2).  The accumulator is double-buffered in TMEM (layer l writes D[l & 1]) and the next A operand
+// is handed to the MMA issuer per 64-column K slab: the MMAs of layer l+1 start as soon as the epilogue of
+// layer l has produced slab 0 and then run back to back while the epilogue finishes the other slabs, so the
+// tensor pipe idles only for the first slab of every layer.  The prologue and layer 0 of the next tile are
+// issued behind the last layer of the current one.
+// Weights are packed on the host into the exact shared-memory image (hb_tc_pack_weights) and stay resident in
+// shared memory for the whole kernel.  CG = 2 pairs two SMs (cta_group::2, M = 256): each CTA holds half of
+// every weight matrix (N split), which is what lets 6-256^3-6 stay resident.
 #include "hb_device.cuh"
 
 #include <cuda_bf16.h>
@@ -25,23 +30,26 @@
 namespace {
 
 constexpr int TILE_M = 128;
-constexpr int A_SLAB_BYTES = TILE_M * 128;       // 128 rows x 64 16-bit elements
-constexpr int WORKER_WARPS = 8;                  // two warps per TMEM lane quarter (column halves)
-constexpr int THREADS = 64 + 32 * WORKER_WARPS;  // warp 0: copy producer, warp 1: MMA issuer
+constexpr int A_SLAB_BYTES = TILE_M * 128;       // 128 rows x 64 16-bit elements, 128-byte swizzle
+constexpr int A0_BYTES = TILE_M * 32;            // layer-0 operand: 128 rows x 16 elements, no swizzle
+constexpr int IO_WARP0 = 4;                      // warps 4..7
+constexpr int EPI_WARP0 = 8;                     // warps 8..8+4G-1
 constexpr int IN_STAGES = 2;
 constexpr int STAGE_BYTES = 6 * TILE_M * 4;
+constexpr int MAX_SLABS = 4;                     // hidden width <= 256
 constexpr size_t SMEM_LIMIT = 227 * 1024;
 
 struct TcPlan {
     int n_linear;
     int ksteps[HB_MAX_LINEAR];        // K = 16 MMA steps of layer l
-    int nslab[HB_MAX_LINEAR];         // 64-wide K slabs of layer l's operands
+    int nslab[HB_MAX_LINEAR];         // 64-wide K slabs of layer l's operands (layer 0: 0, compact layout)
     int npad[HB_MAX_LINEAR];          // padded fan-out (whole layer, both CTAs of a pair)
-    int w_off[HB_MAX_LINEAR];         // smem byte offset of layer l's weight slabs (this CTA's rows)
-    int w_slab_bytes[HB_MAX_LINEAR];  // (npad / CG) * 128
+    int w_off[HB_MAX_LINEAR];         // smem byte offset of layer l's weights (this CTA's rows)
+    int w_slab_bytes[HB_MAX_LINEAR];  // l >= 1: (npad / CG) * 128;  l = 0: (npad / CG) * 32 (whole layer)
     int bias_off[HB_MAX_LINEAR];      // float offset inside the smem bias block
-    int a_off, stage_off, bias_base, bar_off, red_off, total;
-    int tmem_cols;
+    int a_off, a0_off, stage_off, bias_base, bar_off, red_off, total;
+    int d_cols;                       // columns of one accumulator buffer
+    int tmem_cols;                    // 2 * d_cols rounded to a power of two >= 32
     int w_bytes_total;                // bytes this CTA loads
 };
 
@@ -175,11 +183,99 @@ __device__ __forceinline__ float round16(float v) {   // value after rounding to
     return __bfloat162float(__float2bfloat16_rn(v));
 }
 
+
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr) : "memory");
+}
+template <int CW>
+__device__ __forceinline__ void tmem_ld(uint32_t taddr, uint32_t (&r)[CW]) {
+    static_assert(CW == 16 || CW == 32, "column chunk");
+    if constexpr (CW == 32) tmem_ld32(taddr, r);
+    else tmem_ld16(taddr, r);
+}
+
+// K-major, no swizzle (layer 0, K = 16): core matrices of 8 rows x 16 bytes; the two K chunks of an 8-row
+// group sit 128 B apart (LBO), 8-row groups 256 B apart (SBO).
+__device__ __forceinline__ uint64_t make_desc_l0(uint32_t saddr) {
+    uint64_t d = (uint64_t)((saddr & 0x3FFFFu) >> 4);
+    d |= (uint64_t)(128 >> 4) << 16;
+    d |= (uint64_t)(256 >> 4) << 32;
+    d |= (uint64_t)1 << 46;
+    return d;
+}
+
+// (a + bias) for two adjacent accumulator columns in one FADD2
+__device__ __forceinline__ void add2(float& a0, float& a1, float b0, float b1) {
+    uint64_t A, B;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(A) : "f"(a0), "f"(a1));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(B) : "f"(b0), "f"(b1));
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(A) : "l"(A), "l"(B));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(a0), "=f"(a1) : "l"(A));
+}
+template <bool F16>
+__device__ __forceinline__ uint32_t pack2_relu(float lo, float hi) {   // max(.,0) fused into the conversion
+    uint32_t d;
+    if (F16) asm("cvt.rn.relu.f16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+    else asm("cvt.rn.relu.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+    return d;
+}
+// sigma(z0 + b0), sigma(z1 + b1) -> two packed 16-bit operands (Eq. 1, Eq. 2, tanh)
+template <int ACT, bool F16>
+__device__ __forceinline__ uint32_t act_pack(float z0, float z1, float slope) {
+    if (ACT == 1) return pack2_relu<F16>(z0, z1);
+    if (ACT == 2) { z0 = z0 >= 0.0f ? z0 : slope * z0; z1 = z1 >= 0.0f ? z1 : slope * z1; }
+    if (ACT == 3) { z0 = hb_tanh_approx(z0); z1 = hb_tanh_approx(z1); }
+    return pack2<F16>(z0, z1);
+}
+
+// One hidden-layer epilogue step of one warp: CW accumulator columns [c0, c0+CW) of its 32 lanes -> bias,
+// sigma, 16-bit, stored as CW/8 16-byte chunks of the next A operand (row = lane's particle).
+template <int CW, int ACT, bool F16>
+__device__ __forceinline__ void epi_store(const uint32_t (&r)[CW], const float* __restrict__ bl, int c0, float slope,
+                                          uint32_t a_row, uint32_t sw) {
+    uint32_t q[CW / 2];
+#pragma unroll
+    for (int k = 0; k < CW / 4; ++k) {
+        const float4 b4 = *reinterpret_cast<const float4*>(bl + c0 + 4 * k);
+        float v0 = __uint_as_float(r[4 * k]), v1 = __uint_as_float(r[4 * k + 1]);
+        float v2 = __uint_as_float(r[4 * k + 2]), v3 = __uint_as_float(r[4 * k + 3]);
+        add2(v0, v1, b4.x, b4.y);
+        add2(v2, v3, b4.z, b4.w);
+        q[2 * k] = act_pack<ACT, F16>(v0, v1, slope);
+        q[2 * k + 1] = act_pack<ACT, F16>(v2, v3, slope);
+    }
+    const uint32_t slab = a_row + (uint32_t)(c0 >> 6) * A_SLAB_BYTES;
+    const uint32_t ch0 = (uint32_t)((c0 & 63) >> 3);
+#pragma unroll
+    for (int k = 0; k < CW / 8; ++k)
+        asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(slab + (((ch0 + k) ^ sw) << 4)),
+                     "r"(q[4 * k]), "r"(q[4 * k + 1]), "r"(q[4 * k + 2]), "r"(q[4 * k + 3]) : "memory");
+}
+
 // ------------------------------------------------------------------------------- kernel
-template <int CG, int ACT, bool F16>
-__global__ void __launch_bounds__(THREADS, 1)
+// barrier block (8 bytes each, at pl.bar_off):
+enum : int {
+    B_W = 0,              // weights resident (local)
+    B_IN_FULL = 1,        // [2] coordinate rows staged (local)
+    B_IN_EMPTY = 3,       // [2] stage consumed by the 4 IO warps (local)
+    B_A0_FULL = 5,        // [2] layer-0 operand written (leader; 4 IO warps x CG)
+    B_SLAB_FULL = 7,      // [MAX_SLABS] K slab of the next A operand written (leader; 4G warps x CG)
+    B_D_HID = 11,         // [2] accumulator D[b] of a hidden layer complete (both CTAs, MMA commit)
+    B_D_LAST = 13,        // accumulator of the last layer complete (both CTAs, MMA commit)
+    B_OUT_READ = 14,      // last layer's accumulator read by the IO warps (leader; 4 IO warps x CG)
+    B_COUNT = 15
+};
+
+template <int CG, int ACT, bool F16, int G>
+__global__ void __launch_bounds__(32 * (EPI_WARP0 + 4 * G), 1)
 hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, const __grid_constant__ TcPlan pl,
                  double* __restrict__ partials) {
+    constexpr int THREADS = 32 * (EPI_WARP0 + 4 * G);
+    constexpr int CW = 64 / G;                       // accumulator columns per epilogue step of one warp
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     // the 128-byte swizzle atoms (8 rows x 128 B) must sit on 1024-byte boundaries of the shared window
     unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
@@ -189,31 +285,36 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
     const size_t ntiles = (n + TILE_M - 1) / TILE_M;
     const size_t ngroups = (ntiles + CG - 1) / CG;
     const size_t cluster_id = blockIdx.x / CG, nclusters = gridDim.x / CG;
+    const int L = pl.n_linear;
+    const int last_buf = (L - 1) & 1;
 
-    // barriers: [0] w_full, [1..2] in_full, [3..4] in_empty, [5] a_ready, [6] d_full; then the TMEM pointer
     const uint32_t bar0 = sbase + pl.bar_off;
-    const uint32_t bar_w = bar0, bar_in_full = bar0 + 8, bar_in_empty = bar0 + 24, bar_a = bar0 + 40, bar_d = bar0 + 48;
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + pl.bar_off + 64);
+    auto bar = [&](int i) -> uint32_t { return bar0 + 8u * (uint32_t)i; };
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + pl.bar_off + 8 * B_COUNT);
     float* bias_s = reinterpret_cast<float*>(smem + pl.bias_base);
 
     if (tid == 0) {
-        mbar_init(bar_w, 1);
-        for (int s = 0; s < IN_STAGES; ++s) { mbar_init(bar_in_full + 8 * s, 1); mbar_init(bar_in_empty + 8 * s, 4); }
-        mbar_init(bar_a, WORKER_WARPS * CG);
-        mbar_init(bar_d, 1);
+        mbar_init(bar(B_W), 1);
+        for (int s = 0; s < IN_STAGES; ++s) {
+            mbar_init(bar(B_IN_FULL + s), 1);
+            mbar_init(bar(B_IN_EMPTY + s), 4);
+            mbar_init(bar(B_A0_FULL + s), 4 * CG);
+            mbar_init(bar(B_D_HID + s), 1);
+        }
+        for (int j = 0; j < MAX_SLABS; ++j) mbar_init(bar(B_SLAB_FULL + j), 4 * G * CG);
+        mbar_init(bar(B_D_LAST), 1);
+        mbar_init(bar(B_OUT_READ), 4 * CG);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 1) {
         tmem_alloc<CG>(smem_u32(tmem_slot), (uint32_t)pl.tmem_cols);
         tmem_relinquish<CG>();
     }
-    // biases -> shared (all layers)
-    {
-        int total = 0;
-        for (int l = 0; l < pl.n_linear; ++l) total = pl.bias_off[l] + pl.npad[l];
+    {   // biases -> shared (all layers)
+        const int total = pl.bias_off[L - 1] + pl.npad[L - 1];
         for (int i = tid; i < total; i += THREADS) {
             int l = 0;
-            while (l + 1 < pl.n_linear && i >= pl.bias_off[l + 1]) ++l;
+            while (l + 1 < L && i >= pl.bias_off[l + 1]) ++l;
             bias_s[i] = sd.btc[sd.btc_off[l] + (i - pl.bias_off[l])];
         }
     }
@@ -226,12 +327,15 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
     if (warp == 0) {
         // ===================================================== producer: weights once, then particle tiles
         if (lane == 0) {
-            mbar_expect_tx(bar_w, (uint32_t)pl.w_bytes_total);
+            mbar_expect_tx(bar(B_W), (uint32_t)pl.w_bytes_total);
             const unsigned char* wg = reinterpret_cast<const unsigned char*>(sd.wtc);
-            for (int l = 0; l < pl.n_linear; ++l)
+            // layer 0: one contiguous block of this CTA's rows
+            bulk_g2s(sbase + pl.w_off[0], wg + sd.wtc_off[0] + (size_t)rank * pl.w_slab_bytes[0],
+                     (uint32_t)pl.w_slab_bytes[0], bar(B_W));
+            for (int l = 1; l < L; ++l)
                 for (int s = 0; s < pl.nslab[l]; ++s) {
                     const unsigned char* src = wg + sd.wtc_off[l] + (size_t)s * pl.npad[l] * 128 + (size_t)rank * pl.w_slab_bytes[l];
-                    bulk_g2s(sbase + pl.w_off[l] + s * pl.w_slab_bytes[l], src, (uint32_t)pl.w_slab_bytes[l], bar_w);
+                    bulk_g2s(sbase + pl.w_off[l] + s * pl.w_slab_bytes[l], src, (uint32_t)pl.w_slab_bytes[l], bar(B_W));
                 }
             int stage = 0;
             uint32_t ph = 0;
@@ -239,11 +343,11 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                 const size_t tile = g * CG + rank;
                 const bool full = tile < ntiles && (tile + 1) * TILE_M <= n;
                 if (full) {
-                    mbar_wait<false>(bar_in_empty + 8 * stage, ph ^ 1);
-                    mbar_expect_tx(bar_in_full + 8 * stage, STAGE_BYTES);
+                    mbar_wait<false>(bar(B_IN_EMPTY + stage), ph ^ 1);
+                    mbar_expect_tx(bar(B_IN_FULL + stage), STAGE_BYTES);
                     for (int j = 0; j < 6; ++j)
                         bulk_g2s(sbase + pl.stage_off + stage * STAGE_BYTES + j * TILE_M * 4, p.v[j] + tile * TILE_M,
-                                 TILE_M * 4, bar_in_full + 8 * stage);
+                                 TILE_M * 4, bar(B_IN_FULL + stage));
                     stage ^= 1;
                     if (stage == 0) ph ^= 1;
                 }
@@ -255,131 +359,153 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
         if (rank == 0 && lane == 0) {
             const uint32_t fmt = F16 ? 0u : 1u;
             const uint32_t idesc_base = (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)((TILE_M * CG) >> 4) << 24);
-            uint32_t pa = 0;
-            for (size_t g = cluster_id; g < ngroups; g += nclusters) {
-                for (int l = 0; l < pl.n_linear; ++l) {
-                    mbar_wait<CG == 2>(bar_a, pa);
-                    pa ^= 1;
-                    tc_fence_after();
-                    const int npad = pl.npad[l];
-                    for (int n0 = 0; n0 < npad; n0 += 256) {
-                        const int nb = min(256, npad - n0);
-                        const uint32_t idesc = idesc_base | ((uint32_t)(nb >> 3) << 17);
-                        const uint32_t b_row0 = sbase + pl.w_off[l] + (n0 / CG) * 128;
-                        for (int ks = 0; ks < pl.ksteps[l]; ++ks) {
-                            const uint64_t ad = make_desc(sbase + pl.a_off + (ks >> 2) * A_SLAB_BYTES + (ks & 3) * 32);
-                            const uint64_t bd = make_desc(b_row0 + (ks >> 2) * pl.w_slab_bytes[l] + (ks & 3) * 32);
-                            umma<CG>(tmem_base + n0, ad, bd, idesc, ks > 0 ? 1u : 0u);
+            uint32_t ph_slab = 0;                    // bit j: parity of the next completion of SLAB_FULL[j]
+            uint32_t it = 0;
+            for (size_t g = cluster_id; g < ngroups; g += nclusters, ++it) {
+                for (int l = 0; l < L; ++l) {
+                    const uint32_t d_tmem = tmem_base + (uint32_t)((l & 1) * pl.d_cols);
+                    const uint32_t idesc = idesc_base | ((uint32_t)(pl.npad[l] >> 3) << 17);
+                    // D[last_buf] still holds the previous tile's outputs until the IO warps have read them
+                    if (it > 0 && l == last_buf) mbar_wait<CG == 2>(bar(B_OUT_READ), (it - 1) & 1);
+                    if (l == 0) {
+                        mbar_wait<CG == 2>(bar(B_A0_FULL + (it & 1)), (it >> 1) & 1);
+                        tc_fence_after();
+                        umma<CG>(d_tmem, make_desc_l0(sbase + pl.a0_off + (it & 1) * A0_BYTES), make_desc_l0(sbase + pl.w_off[0]),
+                                 idesc, 0u);
+                    } else {
+                        for (int j = 0; j < pl.nslab[l]; ++j) {
+                            mbar_wait<CG == 2>(bar(B_SLAB_FULL + j), (ph_slab >> j) & 1);
+                            ph_slab ^= 1u << j;
+                            tc_fence_after();
+                            const uint32_t a0 = sbase + pl.a_off + j * A_SLAB_BYTES;
+                            const uint32_t b0 = sbase + pl.w_off[l] + j * pl.w_slab_bytes[l];
+#pragma unroll
+                            for (int ks = 0; ks < 4; ++ks)
+                                umma<CG>(d_tmem, make_desc(a0 + ks * 32), make_desc(b0 + ks * 32), idesc, (j | ks) ? 1u : 0u);
                         }
                     }
-                    umma_commit<CG>(bar_d);
+                    umma_commit<CG>(l == L - 1 ? bar(B_D_LAST) : bar(B_D_HID + (l & 1)));
                 }
             }
         }
         __syncwarp();
-    } else {
-        // ===================================================== workers: prologue, layer epilogues, output
+    } else if (warp >= IO_WARP0 && warp < EPI_WARP0) {
+        // ===================================================== IO warps: prologue of tile i+1, output of tile i
         const int wq = warp & 3;                 // TMEM lane quarter this warp may access
-        const int half = (warp - 2) >> 2;        // column half
         const int row = 32 * wq + lane;          // tile row = TMEM lane = particle within the tile
-        const uint32_t a_row = sbase + pl.a_off + row * 128;
-        const uint32_t sw = (uint32_t)(row & 7);
-        const uint32_t tlane = tmem_base + ((uint32_t)(32 * wq) << 16);
+        const uint32_t a0_row = sbase + pl.a0_off + (uint32_t)(row >> 3) * 256 + (uint32_t)(row & 7) * 16;
+        const uint32_t tlane = tmem_base + ((uint32_t)(32 * wq) << 16) + (uint32_t)(last_buf * pl.d_cols);
+        const float* bl = bias_s + pl.bias_off[L - 1];
         HbMomAcc acc;
         acc.clear();
-        mbar_wait<false>(bar_w, 0);              // this CTA's weights are resident
         int stage = 0;
-        uint32_t pin = 0, pd = 0;
-        for (size_t g = cluster_id; g < ngroups; g += nclusters) {
+        uint32_t pin = 0;
+        // a4: load, convert, normalise, split, write the layer-0 operand of the tile of group g
+        auto prologue = [&](size_t g, uint32_t buf) {
             const size_t tile = g * CG + rank;
             const size_t i = tile * TILE_M + row;
             const bool valid = tile < ntiles && i < n;
             const bool full = tile < ntiles && (tile + 1) * TILE_M <= n;
-            if (half == 0) {
-                float c[6] = {0, 0, 0, 0, 0, 0};
-                if (full) {
-                    mbar_wait<false>(bar_in_full + 8 * stage, pin);
-                    const float* st = reinterpret_cast<const float*>(smem + pl.stage_off + stage * STAGE_BYTES);
+            float c[6] = {0, 0, 0, 0, 0, 0};
+            if (full) {
+                mbar_wait<false>(bar(B_IN_FULL + stage), pin);
+                const float* st = reinterpret_cast<const float*>(smem + pl.stage_off + stage * STAGE_BYTES);
 #pragma unroll
-                    for (int j = 0; j < 6; ++j) c[j] = st[j * TILE_M + row];
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive_local(bar_in_empty + 8 * stage);
-                    stage ^= 1;
-                    if (stage == 0) pin ^= 1;
-                } else if (valid) {
+                for (int j = 0; j < 6; ++j) c[j] = st[j * TILE_M + row];
+                __syncwarp();
+                if (lane == 0) mbar_arrive_local(bar(B_IN_EMPTY + stage));
+                stage ^= 1;
+                if (stage == 0) pin ^= 1;
+            } else if (valid) {
 #pragma unroll
-                    for (int j = 0; j < 6; ++j) c[j] = p.v[j][i];
-                }
-                float nin[6] = {0, 0, 0, 0, 0, 0};
-                if (valid) hb_sur_prologue(sd, c[0], c[1], c[2], c[3], c[4], c[5], nin);
-                float lo[6];
-#pragma unroll
-                for (int j = 0; j < 6; ++j) lo[j] = nin[j] - round16<F16>(nin[j]);
-                // K = 16 operand row: hi0..hi5, lo0..lo5, 0, 0, 0, 0  (two 16-byte chunks, swizzled)
-                const uint32_t q0[4] = {pack2<F16>(nin[0], nin[1]), pack2<F16>(nin[2], nin[3]), pack2<F16>(nin[4], nin[5]),
-                                        pack2<F16>(lo[0], lo[1])};
-                const uint32_t q1[4] = {pack2<F16>(lo[2], lo[3]), pack2<F16>(lo[4], lo[5]), 0u, 0u};
-                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a_row + ((0u ^ sw) << 4)), "r"(q0[0]), "r"(q0[1]), "r"(q0[2]), "r"(q0[3]) : "memory");
-                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a_row + ((1u ^ sw) << 4)), "r"(q1[0]), "r"(q1[1]), "r"(q1[2]), "r"(q1[3]) : "memory");
+                for (int j = 0; j < 6; ++j) c[j] = p.v[j][i];
             }
+            float nin[6] = {0, 0, 0, 0, 0, 0};
+            if (valid) hb_sur_prologue(sd, c[0], c[1], c[2], c[3], c[4], c[5], nin);
+            float lo[6];
+#pragma unroll
+            for (int j = 0; j < 6; ++j) lo[j] = nin[j] - round16<F16>(nin[j]);
+            // K = 16 operand row: hi0..hi5, lo0..lo5, 0, 0, 0, 0  (two 16-byte chunks, 128 B apart)
+            const uint32_t q0[4] = {pack2<F16>(nin[0], nin[1]), pack2<F16>(nin[2], nin[3]), pack2<F16>(nin[4], nin[5]),
+                                    pack2<F16>(lo[0], lo[1])};
+            const uint32_t q1[4] = {pack2<F16>(lo[2], lo[3]), pack2<F16>(lo[4], lo[5]), 0u, 0u};
+            const uint32_t dst = a0_row + buf * A0_BYTES;
+            asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(dst), "r"(q0[0]), "r"(q0[1]), "r"(q0[2]), "r"(q0[3]) : "memory");
+            asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(dst + 128), "r"(q1[0]), "r"(q1[1]), "r"(q1[2]), "r"(q1[3]) : "memory");
             fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(bar(B_A0_FULL + buf), 0);
+        };
+        mbar_wait<false>(bar(B_W), 0);           // this CTA's weights are resident before the first MMA may start
+        uint32_t it = 0;
+        if (cluster_id < ngroups) prologue(cluster_id, 0);
+        for (size_t g = cluster_id; g < ngroups; g += nclusters, ++it) {
+            if (g + nclusters < ngroups) prologue(g + nclusters, (it + 1) & 1);
+            const size_t tile = g * CG + rank;
+            const size_t i = tile * TILE_M + row;
+            const bool valid = tile < ntiles && i < n;
+            mbar_wait<false>(bar(B_D_LAST), it & 1);
+            tc_fence_after();
+            uint32_t r[8];
+            tmem_ld8(tlane, r);
+            tmem_ld_wait();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(bar_a, 0);
-
-            for (int l = 0; l < pl.n_linear; ++l) {
-                mbar_wait<false>(bar_d, pd);
-                pd ^= 1;
+            if (lane == 0) mbar_arrive_cluster(bar(B_OUT_READ), 0);
+            if (valid) {
+                float w[6];
+#pragma unroll
+                for (int j = 0; j < 6; ++j) w[j] = __uint_as_float(r[j]) + bl[j];
+                float x, px, y, py, t, pt;
+                hb_sur_epilogue(sd, w, x, px, y, py, t, pt);
+                p.v[0][i] = x; p.v[1][i] = px; p.v[2][i] = y; p.v[3][i] = py; p.v[4][i] = t; p.v[5][i] = pt;
+                if (partials) acc.add(x, px, y, py, t, pt);
+            }
+        }
+        if (partials) {
+            double* red = reinterpret_cast<double*>(smem + pl.red_off);
+            hb_block_reduce_moments(acc, red, partials + (size_t)blockIdx.x * HB_NMOM, tid - 32 * IO_WARP0, 128, 2);
+        }
+    } else if (warp >= EPI_WARP0) {
+        // ===================================================== hidden-layer epilogue warps
+        const int wq = warp & 3;
+        const int grp = (warp - EPI_WARP0) >> 2;  // column group inside every 64-column slab
+        const int row = 32 * wq + lane;
+        const uint32_t a_row = sbase + pl.a_off + row * 128;
+        const uint32_t sw = (uint32_t)(row & 7);
+        const uint32_t tlane = tmem_base + ((uint32_t)(32 * wq) << 16);
+        uint32_t ph_d = 0;                        // bit b: parity of the next completion of D_HID[b]
+        for (size_t g = cluster_id; g < ngroups; g += nclusters) {
+            for (int l = 0; l < L - 1; ++l) {
+                const int b = l & 1;
+                const int nsl = pl.npad[l] >> 6;
+                const float* bl = bias_s + pl.bias_off[l];
+                const float slope = sd.prelu[l];
+                const uint32_t t0 = tlane + (uint32_t)(b * pl.d_cols + grp * CW);
+                mbar_wait<false>(bar(B_D_HID + b), (ph_d >> b) & 1);
+                ph_d ^= 1u << b;
                 tc_fence_after();
-                if (l < pl.n_linear - 1) {
-                    const int npad = pl.npad[l];
-                    const float* bl = bias_s + pl.bias_off[l];
-                    const float slope = sd.prelu[l];
-                    const int c_begin = half * (npad >> 1), c_end = c_begin + (npad >> 1);
-                    for (int c0 = c_begin; c0 < c_end; c0 += 32) {
-                        uint32_t r[32];
-                        tmem_ld32(tlane + c0, r);
-                        tmem_ld_wait();
-                        uint32_t q[16];
-#pragma unroll
-                        for (int k = 0; k < 16; ++k) {
-                            const float2 b2 = *reinterpret_cast<const float2*>(bl + c0 + 2 * k);
-                            const float v0 = hb_activate<ACT, true>(__uint_as_float(r[2 * k]) + b2.x, slope);
-                            const float v1 = hb_activate<ACT, true>(__uint_as_float(r[2 * k + 1]) + b2.y, slope);
-                            q[k] = pack2<F16>(v0, v1);
-                        }
-                        const uint32_t slab = a_row + (c0 >> 6) * A_SLAB_BYTES;
-                        const uint32_t ch0 = (uint32_t)((c0 & 63) >> 3);
-#pragma unroll
-                        for (int k = 0; k < 4; ++k)
-                            asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(slab + (((ch0 + k) ^ sw) << 4)),
-                                         "r"(q[4 * k]), "r"(q[4 * k + 1]), "r"(q[4 * k + 2]), "r"(q[4 * k + 3]) : "memory");
-                    }
+                uint32_t ra[CW], rb[CW];
+                tmem_ld<CW>(t0, ra);
+                for (int j = 0; j < nsl; j += 2) {
+                    tmem_ld_wait();
+                    if (j + 1 < nsl) tmem_ld<CW>(t0 + 64 * (j + 1), rb);
+                    epi_store<CW, ACT, F16>(ra, bl, 64 * j + grp * CW, slope, a_row, sw);
                     fence_proxy_async();
                     tc_fence_before();
                     __syncwarp();
-                    if (lane == 0) mbar_arrive_cluster(bar_a, 0);
-                } else if (half == 0) {
-                    uint32_t r[8];
-                    tmem_ld8(tlane, r);
-                    tmem_ld_wait();
-                    tc_fence_before();
-                    if (valid) {
-                        const float* bl = bias_s + pl.bias_off[l];
-                        float w[6];
-#pragma unroll
-                        for (int j = 0; j < 6; ++j) w[j] = __uint_as_float(r[j]) + bl[j];
-                        float x, px, y, py, t, pt;
-                        hb_sur_epilogue(sd, w, x, px, y, py, t, pt);
-                        p.v[0][i] = x; p.v[1][i] = px; p.v[2][i] = y; p.v[3][i] = py; p.v[4][i] = t; p.v[5][i] = pt;
-                        if (partials) acc.add(x, px, y, py, t, pt);
+                    if (lane == 0) mbar_arrive_cluster(bar(B_SLAB_FULL + j), 0);
+                    if (j + 1 < nsl) {
+                        tmem_ld_wait();
+                        if (j + 2 < nsl) tmem_ld<CW>(t0 + 64 * (j + 2), ra);
+                        epi_store<CW, ACT, F16>(rb, bl, 64 * (j + 1) + grp * CW, slope, a_row, sw);
+                        fence_proxy_async();
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive_cluster(bar(B_SLAB_FULL + j + 1), 0);
                     }
                 }
             }
-        }
-        if (partials && half == 0) {
-            double* red = reinterpret_cast<double*>(smem + pl.red_off);
-            hb_block_reduce_moments(acc, red, partials + (size_t)blockIdx.x * HB_NMOM, tid - 64, 128, 2);
         }
     }
     // ---- teardown: everyone done with TMEM (both CTAs of a pair), then free it
@@ -399,7 +525,7 @@ void layer_geometry(int n_linear, const int* widths, int* kpad, int* npad, int* 
     for (int l = 0; l < n_linear; ++l) {
         const bool last = l == n_linear - 1;
         npad[l] = last ? 16 : round_up(widths[l + 1], 64);
-        if (l == 0) { kpad[l] = 64; ksteps[l] = 1; }                 // 6 hi + 6 lo + 4 zero
+        if (l == 0) { kpad[l] = 16; ksteps[l] = 1; }                 // 6 hi + 6 lo + 4 zero
         else { kpad[l] = npad[l - 1]; ksteps[l] = npad[l - 1] / 16; }
     }
 }
@@ -412,46 +538,49 @@ bool make_plan(int cg, int n_linear, const int* widths, TcPlan& pl) {
     int off = 0, boff = 0, maxslab = 1, maxn = 32;
     for (int l = 0; l < n_linear; ++l) {
         pl.ksteps[l] = ksteps[l];
-        pl.nslab[l] = kpad[l] / 64;
+        pl.nslab[l] = l == 0 ? 0 : kpad[l] / 64;
         if ((pl.npad[l] / cg) % 8) return false;
-        pl.w_slab_bytes[l] = pl.npad[l] / cg * 128;
+        pl.w_slab_bytes[l] = pl.npad[l] / cg * (l == 0 ? 32 : 128);
         pl.w_off[l] = off;
-        off += pl.nslab[l] * pl.w_slab_bytes[l];
+        off += (l == 0 ? 1 : pl.nslab[l]) * pl.w_slab_bytes[l];
+        off = round_up(off, 1024);
         pl.bias_off[l] = boff;
         boff += pl.npad[l];
         if (pl.nslab[l] > maxslab) maxslab = pl.nslab[l];
         if (pl.npad[l] > maxn) maxn = pl.npad[l];
     }
-    if (maxn > 512) return false;                                   // accumulator must fit the 512 TMEM columns
-    if (cg == 2 && maxn > 256) return false;                        // pair mode: one N block (rows split 0..N/2 | N/2..N)
-    pl.w_bytes_total = off;
-    off = round_up(off, 1024);
+    if (maxn > 256 || maxslab > MAX_SLABS) return false;            // two accumulators must fit the 512 TMEM columns
+    pl.w_bytes_total = 0;
+    for (int l = 0; l < n_linear; ++l) pl.w_bytes_total += (l == 0 ? 1 : pl.nslab[l]) * pl.w_slab_bytes[l];
     pl.a_off = off;
     off += maxslab * A_SLAB_BYTES;
+    pl.a0_off = off;
+    off += 2 * A0_BYTES;
     pl.stage_off = off;
     off += IN_STAGES * STAGE_BYTES;
     pl.bias_base = off;
     off += round_up(boff * 4, 16);
     pl.bar_off = off;
-    off += 128;
+    off += round_up(8 * B_COUNT + 8, 16);
     pl.red_off = off;
     off += 4 * HB_NMOM * 8;
     pl.total = off;
+    pl.d_cols = round_up(maxn, 64);
     int cols = 32;
-    while (cols < maxn) cols <<= 1;
+    while (cols < 2 * pl.d_cols) cols <<= 1;
     pl.tmem_cols = cols;
     return (size_t)pl.total + 1024 <= SMEM_LIMIT;
 }
 
-template <int CG, int ACT, bool F16>
+template <int CG, int ACT, bool F16, int G>
 cudaError_t launch_one(const HbParticles& p, size_t n, const HbSurDev& sd, const TcPlan& pl, double* partials, int grid,
                        cudaStream_t s) {
     const size_t smem = (size_t)pl.total + 1024;   // slack so the 1024-byte alignment of the swizzle atoms always holds
-    cudaError_t e = cudaFuncSetAttribute(hb_sur_tc_kernel<CG, ACT, F16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(hb_sur_tc_kernel<CG, ACT, F16, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(grid);
-    cfg.blockDim = dim3(THREADS);
+    cfg.blockDim = dim3(32 * (EPI_WARP0 + 4 * G));
     cfg.dynamicSmemBytes = smem;
     cfg.stream = s;
     cudaLaunchAttribute at[1];
@@ -461,18 +590,25 @@ cudaError_t launch_one(const HbParticles& p, size_t n, const HbSurDev& sd, const
     at[0].val.clusterDim.z = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, hb_sur_tc_kernel<CG, ACT, F16>, p, n, sd, pl, partials);
+    return cudaLaunchKernelEx(&cfg, hb_sur_tc_kernel<CG, ACT, F16, G>, p, n, sd, pl, partials);
 }
 
-template <int CG, bool F16>
+template <int CG, bool F16, int G>
 cudaError_t launch_act(const HbParticles& p, size_t n, const HbSurDev& sd, const TcPlan& pl, double* partials, int grid,
                        cudaStream_t s) {
     switch (sd.act) {
-    case 0: return launch_one<CG, 0, F16>(p, n, sd, pl, partials, grid, s);
-    case 1: return launch_one<CG, 1, F16>(p, n, sd, pl, partials, grid, s);
-    case 2: return launch_one<CG, 2, F16>(p, n, sd, pl, partials, grid, s);
-    default: return launch_one<CG, 3, F16>(p, n, sd, pl, partials, grid, s);
+    case 0: return launch_one<CG, 0, F16, G>(p, n, sd, pl, partials, grid, s);
+    case 1: return launch_one<CG, 1, F16, G>(p, n, sd, pl, partials, grid, s);
+    case 2: return launch_one<CG, 2, F16, G>(p, n, sd, pl, partials, grid, s);
+    default: return launch_one<CG, 3, F16, G>(p, n, sd, pl, partials, grid, s);
     }
+}
+
+template <int CG, bool F16>
+cudaError_t launch_g(int g, const HbParticles& p, size_t n, const HbSurDev& sd, const TcPlan& pl, double* partials, int grid,
+                     cudaStream_t s) {
+    if (g == 4) return launch_act<CG, F16, 4>(p, n, sd, pl, partials, grid, s);
+    return launch_act<CG, F16, 2>(p, n, sd, pl, partials, grid, s);
 }
 
 int choose_cg(int n_linear, const int* widths, TcPlan& pl) {
@@ -482,6 +618,12 @@ int choose_cg(int n_linear, const int* widths, TcPlan& pl) {
     if (make_plan(1, n_linear, widths, pl)) return 1;
     if (make_plan(2, n_linear, widths, pl)) return 2;
     return 0;
+}
+
+int choose_g() {
+    // HB_TC_EPI_GROUPS=2|4 : hidden-layer epilogue warps = 4 x groups (tuning hook; default 2)
+    const char* e = getenv("HB_TC_EPI_GROUPS");
+    return (e && e[0] == '4') ? 4 : 2;
 }
 
 }  // namespace
@@ -494,15 +636,16 @@ bool hb_tc_supported(int prec, int n_linear, const int* widths, char* why, size_
     TcPlan pl;
     if (!choose_cg(n_linear, widths, pl)) {
         snprintf(why, why_len, "weights do not fit resident in shared memory even split over a CTA pair "
-                               "(or a hidden width exceeds 512); weight streaming is not built yet");
+                               "(or a hidden width exceeds 256); weight streaming is not built yet");
         return false;
     }
     return true;
 }
 
-// Packed operand image: per layer, per 64-wide K slab, npad rows of 128 bytes (K-major, 128-byte swizzle:
-// the 16-byte chunk c of row r sits at chunk position c ^ (r mod 8)).  Layer 0 carries W_0 twice
-// (columns 0..5 multiply the hi parts of the inputs, 6..11 the lo parts).
+// Packed operand image.  Layer 0 (K = 16, no swizzle): per 8-row group 256 bytes = K chunk 0 of the 8 rows
+// (8 x 16 B) followed by K chunk 1; W_0 is carried twice (columns 0..5 multiply the hi parts of the inputs,
+// 6..11 the lo parts).  Layers >= 1: per 64-wide K slab, npad rows of 128 bytes (K-major, 128-byte swizzle:
+// the 16-byte chunk c of row r sits at chunk position c ^ (r mod 8)).
 size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float* const* W, void* dst,
                           long long* off_bytes, int* kpad, int* npad) {
     int ksteps[HB_MAX_LINEAR];
@@ -510,7 +653,8 @@ size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float
     size_t total = 0;
     for (int l = 0; l < n_linear; ++l) {
         off_bytes[l] = (long long)total;
-        total += (size_t)(kpad[l] / 64) * npad[l] * 128;
+        total += l == 0 ? (size_t)npad[l] * 32 : (size_t)(kpad[l] / 64) * npad[l] * 128;
+        total = (total + 15) / 16 * 16;
     }
     if (!dst) return total;
     std::memset(dst, 0, total);
@@ -521,9 +665,14 @@ size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float
         for (int o = 0; o < fout; ++o)
             for (int k = 0; k < kcols; ++k) {
                 const float w = l == 0 ? W[l][(size_t)o * fin + (k % 6)] : W[l][(size_t)o * fin + k];
-                const int slab = k / 64, kk = k % 64, c = kk / 8, e = kk % 8;
-                const size_t byte = (size_t)off_bytes[l] + (size_t)slab * npad[l] * 128 + (size_t)o * 128 +
-                                    (size_t)((c ^ (o & 7)) << 4) + (size_t)e * 2;
+                size_t byte;
+                if (l == 0) {
+                    byte = (size_t)off_bytes[l] + (size_t)(o / 8) * 256 + (size_t)(k / 8) * 128 + (size_t)(o % 8) * 16 + (size_t)(k % 8) * 2;
+                } else {
+                    const int slab = k / 64, kk = k % 64, c = kk / 8, e = kk % 8;
+                    byte = (size_t)off_bytes[l] + (size_t)slab * npad[l] * 128 + (size_t)o * 128 +
+                           (size_t)((c ^ (o & 7)) << 4) + (size_t)e * 2;
+                }
                 unsigned short bits;
                 if (prec == 2) { __half h = __float2half_rn(w); std::memcpy(&bits, &h, 2); }
                 else { __nv_bfloat16 h = __float2bfloat16_rn(w); std::memcpy(&bits, &h, 2); }
@@ -546,6 +695,7 @@ cudaError_t hb_launch_sur_tc(const HbParticles& p, size_t n, const HbSurDev& sd,
     const int grid = (int)clusters * cg;
     if (nblocks_out) *nblocks_out = grid;
     const bool f16 = sd.prec == 2;
-    if (cg == 1) return f16 ? launch_act<1, true>(p, n, sd, pl, partials, grid, s) : launch_act<1, false>(p, n, sd, pl, partials, grid, s);
-    return f16 ? launch_act<2, true>(p, n, sd, pl, partials, grid, s) : launch_act<2, false>(p, n, sd, pl, partials, grid, s);
+    const int g = choose_g();
+    if (cg == 1) return f16 ? launch_g<1, true>(g, p, n, sd, pl, partials, grid, s) : launch_g<1, false>(g, p, n, sd, pl, partials, grid, s);
+    return f16 ? launch_g<2, true>(g, p, n, sd, pl, partials, grid, s) : launch_g<2, false>(g, p, n, sd, pl, partials, grid, s);
 }
