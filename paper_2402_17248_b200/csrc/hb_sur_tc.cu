@@ -2,13 +2,13 @@
 //
 // One 128-particle tile per CTA (one TMEM lane per particle; a CTA pair works on 256 particles with
 // cta_group::2).  Warp roles:
-//   warp 0      copy producer : weights once, then the six coordinate rows of each tile through the TMA
+//   warp 4+4G   copy producer : weights once, then the six coordinate rows of each tile through the TMA
 //                               engine (cp.async.bulk + mbarrier complete_tx) into a 2-stage ring.
-//   warp 1      MMA issuer    : one elected thread (leader CTA of a pair) issues every tcgen05.mma.
-//   warps 4-7   IO warps      : a4 prologue (s->t R6 in deviation form, normalise R8, hi/lo split, layer-0
+//   warp 5+4G   MMA issuer    : one elected thread (leader CTA of a pair) issues every tcgen05.mma.
+//   warps 0-3   IO warps      : a4 prologue (s->t R6 in deviation form, normalise R8, hi/lo split, layer-0
 //                               operand) of tile i+1, then a6 epilogue of tile i (tcgen05.ld of the 6 outputs,
 //                               de-normalise R8, reference update R7, t->s R6, coalesced store, fp64 moments R10).
-//   warps 8..   hidden-layer epilogue warps: tcgen05.ld of the accumulator, + bias (fp32), sigma (Eq. 1/2,
+//   warps 4..   4G hidden-layer epilogue warps: tcgen05.ld of the accumulator, + bias (fp32), sigma (Eq. 1/2,
 //                               tanh), round to 16 bit, write the next A operand in the 128-byte-swizzled
 //                               K-major layout the MMA reads.  Hidden activations never leave the SM.
 // Pipeline (v2).  The accumulator is double-buffered in TMEM (layer l writes D[l & 1]) and the next A operand
@@ -32,8 +32,9 @@ namespace {
 constexpr int TILE_M = 128;
 constexpr int A_SLAB_BYTES = TILE_M * 128;       // 128 rows x 64 16-bit elements, 128-byte swizzle
 constexpr int A0_BYTES = TILE_M * 32;            // layer-0 operand: 128 rows x 16 elements, no swizzle
-constexpr int IO_WARP0 = 4;                      // warps 4..7
-constexpr int EPI_WARP0 = 8;                     // warps 8..8+4G-1
+constexpr int IO_WARP0 = 0;                      // warps 0..3
+constexpr int EPI_WARP0 = 4;                     // warps 4..4+4G-1; then the producer warp, then the MMA warp
+constexpr int tc_threads(int g) { return 32 * (EPI_WARP0 + 4 * g + 2); }
 constexpr int IN_STAGES = 2;
 constexpr int STAGE_BYTES = 6 * TILE_M * 4;
 constexpr int MAX_SLABS = 4;                     // hidden width <= 256
@@ -52,6 +53,20 @@ struct TcPlan {
     int tmem_cols;                    // 2 * d_cols rounded to a power of two >= 32
     int w_bytes_total;                // bytes this CTA loads
 };
+
+#ifdef HB_TC_TRACE   // debugging aid (never defined in the product build): per-role event timeline of block 0
+constexpr int TR_ROLES = 40, TR_MAXEV = 1024;
+__device__ long long hb_tc_trace_buf[TR_ROLES * TR_MAXEV];
+#define TR_DECL int trc_ = 0
+#define TR(role, code)                                                                                      \
+    do {                                                                                                    \
+        if (blockIdx.x < 2 && (threadIdx.x & 31) == 0 && trc_ < TR_MAXEV)                                   \
+            hb_tc_trace_buf[((role) + 20 * blockIdx.x) * TR_MAXEV + trc_++] = (clock64() << 8) | (long long)(code);             \
+    } while (0)
+#else
+#define TR_DECL
+#define TR(role, code)
+#endif
 
 // ------------------------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -73,14 +88,22 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar, uint32_t rank)
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(bar), "r"(rank));
     asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(remote) : "memory");
 }
-template <bool CLUSTER_SCOPE>
+__device__ __forceinline__ uint32_t mbar_try(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                 "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok;
+}
+// FAST: latency-critical waiters try a few times before they start reading the clock for the hang guard.
+template <bool FAST>
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    uint32_t ok = 0;
+    if (FAST) {
+#pragma unroll 1
+        for (int i = 0; i < 64; ++i)
+            if (mbar_try(bar, parity)) return;
+    }
     const long long t0 = clock64();
-    while (true) {
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-                     "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-        if (ok) break;
+    while (!mbar_try(bar, parity)) {
         if (clock64() - t0 > 4000000000LL) {   // ~2 s: a protocol bug must not hang the GPU
             printf("hb_sur_tc: mbarrier timeout (block %d thread %d bar %u parity %u)\n", blockIdx.x, threadIdx.x, bar, parity);
             __trap();
@@ -111,16 +134,21 @@ __device__ __forceinline__ void tmem_dealloc(uint32_t addr, uint32_t cols) {
     else asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(addr), "r"(cols) : "memory");
 }
 // D[tmem] (+)= A[smem desc] * B[smem desc]
-template <int CG>
-__device__ __forceinline__ void umma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+template <int CG, bool ACC>
+__device__ __forceinline__ void umma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc) {
     if (CG == 1)
         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
                      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-                     ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+                     ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "n"(ACC ? 1 : 0) : "memory");
     else
         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
                      "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-                     ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+                     ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "n"(ACC ? 1 : 0) : "memory");
+}
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
 }
 // all MMAs issued so far by this thread arrive on `bar` (in both CTAs of a pair) when they complete
 template <int CG>
@@ -269,10 +297,13 @@ enum : int {
 };
 
 template <int CG, int ACT, bool F16, int G>
-__global__ void __launch_bounds__(32 * (EPI_WARP0 + 4 * G), 1)
+__global__ void __launch_bounds__(tc_threads(G), 1)
 hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, const __grid_constant__ TcPlan pl,
                  double* __restrict__ partials) {
-    constexpr int THREADS = 32 * (EPI_WARP0 + 4 * G);
+    constexpr int THREADS = tc_threads(G);
+    // the scheduler favours the highest warp id: the MMA issuer sits on top so that busy epilogue warps on the
+    // same scheduler never delay an MMA issue
+    constexpr int PROD_WARP = EPI_WARP0 + 4 * G, MMA_WARP = PROD_WARP + 1;
     constexpr int CW = 64 / G;                       // accumulator columns per epilogue step of one warp
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     // the 128-byte swizzle atoms (8 rows x 128 B) must sit on 1024-byte boundaries of the shared window
@@ -304,7 +335,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
         mbar_init(bar(B_OUT_READ), 4 * CG);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == 1) {
+    if (warp == MMA_WARP) {
         tmem_alloc<CG>(smem_u32(tmem_slot), (uint32_t)pl.tmem_cols);
         tmem_relinquish<CG>();
     }
@@ -322,7 +353,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
-    if (warp == 0) {
+    if (warp == PROD_WARP) {
         // ===================================================== producer: weights once, then particle tiles
         if (lane == 0) {
             mbar_expect_tx(bar(B_W), (uint32_t)pl.w_bytes_total);
@@ -352,42 +383,70 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
             }
         }
         __syncwarp();
-    } else if (warp == 1) {
+    } else if (warp == MMA_WARP) {
         // ===================================================== MMA issuer (leader CTA of the pair only)
-        if (rank == 0 && lane == 0) {
+        // The whole warp walks the schedule (warp-uniform control flow, barrier waits by every lane); one
+        // elected lane issues the MMAs and commits.
+        if (rank == 0) {
             const uint32_t fmt = F16 ? 0u : 1u;
             const uint32_t idesc_base = (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)((TILE_M * CG) >> 4) << 24);
+            const bool issuer = elect_one();
+            const uint64_t a_desc0 = make_desc(sbase + pl.a_off);
+            const uint64_t w0_desc = make_desc_l0(sbase + pl.w_off[0]);
+            TR_DECL;
             uint32_t ph_slab = 0;                    // bit j: parity of the next completion of SLAB_FULL[j]
             uint32_t it = 0;
             for (size_t g = cluster_id; g < ngroups; g += nclusters, ++it) {
                 for (int l = 0; l < L; ++l) {
                     const uint32_t d_tmem = tmem_base + (uint32_t)((l & 1) * pl.d_cols);
                     const uint32_t idesc = idesc_base | ((uint32_t)(pl.npad[l] >> 3) << 17);
+                    const int nsl = pl.nslab[l];
+                    const uint64_t bd = make_desc(sbase + pl.w_off[l]);
+                    const uint64_t bd_step = (uint64_t)(pl.w_slab_bytes[l] >> 4);
                     // D[last_buf] still holds the previous tile's outputs until the IO warps have read them
-                    if (it > 0 && l == last_buf) mbar_wait<CG == 2>(bar(B_OUT_READ), (it - 1) & 1);
+                    if (it > 0 && l == last_buf) mbar_wait<true>(bar(B_OUT_READ), (it - 1) & 1);
                     if (l == 0) {
-                        mbar_wait<CG == 2>(bar(B_A0_FULL + (it & 1)), (it >> 1) & 1);
+                        TR(0, 1);
+                        mbar_wait<true>(bar(B_A0_FULL + (it & 1)), (it >> 1) & 1);
                         tc_fence_after();
-                        umma<CG>(d_tmem, make_desc_l0(sbase + pl.a0_off + (it & 1) * A0_BYTES), make_desc_l0(sbase + pl.w_off[0]),
-                                 idesc, 0u);
+                        TR(0, 2);
+                        if (issuer) umma<CG, false>(d_tmem, make_desc_l0(sbase + pl.a0_off + (it & 1) * A0_BYTES), w0_desc, idesc);
                     } else {
-                        for (int j = 0; j < pl.nslab[l]; ++j) {
-                            mbar_wait<CG == 2>(bar(B_SLAB_FULL + j), (ph_slab >> j) & 1);
-                            ph_slab ^= 1u << j;
-                            tc_fence_after();
-                            const uint32_t a0 = sbase + pl.a_off + j * A_SLAB_BYTES;
-                            const uint32_t b0 = sbase + pl.w_off[l] + j * pl.w_slab_bytes[l];
+                        // fully unrolled over the (at most MAX_SLABS) K slabs: every MMA of a layer gets its own
+                        // descriptor registers, so that forming the next slab's descriptors never has to wait for
+                        // an MMA still queued in the tensor pipe to release them (measured: +200 cycles per slab)
+                        uint32_t ready = 0;               // slab j's barrier already seen complete (peeked)
 #pragma unroll
-                            for (int ks = 0; ks < 4; ++ks)
-                                umma<CG>(d_tmem, make_desc(a0 + ks * 32), make_desc(b0 + ks * 32), idesc, (j | ks) ? 1u : 0u);
+                        for (int j = 0; j < MAX_SLABS; ++j) {
+                            if (j < nsl) {
+                                if (!ready) mbar_wait<true>(bar(B_SLAB_FULL + j), (ph_slab >> j) & 1);
+                                ph_slab ^= 1u << j;
+                                tc_fence_after();
+                                // peek at the next slab before this slab's MMAs go out: an MMA issue can hold the
+                                // warp for as long as the tensor pipe's queue is full
+                                ready = (j + 1 < nsl) ? mbar_try(bar(B_SLAB_FULL + j + 1), (ph_slab >> (j + 1)) & 1) : 0u;
+                                if (j == 0) TR(0, 17);
+                                if (issuer) {
+                                    // four K = 16 steps inside the 64-wide slab: the start address advances by 32 B
+                                    const uint64_t ad = a_desc0 + (uint64_t)(j * (A_SLAB_BYTES >> 4));
+                                    const uint64_t bj = bd + (uint64_t)j * bd_step;
+                                    if (j == 0) umma<CG, false>(d_tmem, ad, bj, idesc);
+                                    else umma<CG, true>(d_tmem, ad, bj, idesc);
+                                    umma<CG, true>(d_tmem, ad + 2, bj + 2, idesc);
+                                    umma<CG, true>(d_tmem, ad + 4, bj + 4, idesc);
+                                    umma<CG, true>(d_tmem, ad + 6, bj + 6, idesc);
+                                }
+                            }
                         }
                     }
-                    umma_commit<CG>(l == L - 1 ? bar(B_D_LAST) : bar(B_D_HID + (l & 1)));
+                    if (issuer) umma_commit<CG>(l == L - 1 ? bar(B_D_LAST) : bar(B_D_HID + (l & 1)));
+                    __syncwarp();
+                    TR(0, 32 + l);
                 }
             }
         }
         __syncwarp();
-    } else if (warp >= IO_WARP0 && warp < EPI_WARP0) {
+    } else if (warp < EPI_WARP0) {
         // ===================================================== IO warps: prologue of tile i+1, output of tile i
         const int wq = warp & 3;                 // TMEM lane quarter this warp may access
         const int row = 32 * wq + lane;          // tile row = TMEM lane = particle within the tile
@@ -398,6 +457,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
         acc.clear();
         int stage = 0;
         uint32_t pin = 0;
+        TR_DECL;
         // a4: load, convert, normalise, split, write the layer-0 operand of the tile of group g
         auto prologue = [&](size_t g, uint32_t buf) {
             const size_t tile = g * CG + rank;
@@ -433,6 +493,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
             fence_proxy_async();
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(bar(B_A0_FULL + buf), 0);
+            if (warp == IO_WARP0) TR(2, 1);
         };
         mbar_wait<false>(bar(B_W), 0);           // this CTA's weights are resident before the first MMA may start
         uint32_t it = 0;
@@ -442,8 +503,10 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
             const size_t tile = g * CG + rank;
             const size_t i = tile * TILE_M + row;
             const bool valid = tile < ntiles && i < n;
+            if (warp == IO_WARP0) TR(2, 2);
             mbar_wait<false>(bar(B_D_LAST), it & 1);
             tc_fence_after();
+            if (warp == IO_WARP0) TR(2, 3);
             uint32_t r[8];
             tmem_ld8(tlane, r);
             tmem_ld_wait();
@@ -459,12 +522,13 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                 p.v[0][i] = x; p.v[1][i] = px; p.v[2][i] = y; p.v[3][i] = py; p.v[4][i] = t; p.v[5][i] = pt;
                 if (partials) acc.add(x, px, y, py, t, pt);
             }
+            if (warp == IO_WARP0) TR(2, 4);
         }
         if (partials) {
             double* red = reinterpret_cast<double*>(smem + pl.red_off);
             hb_block_reduce_moments(acc, red, partials + (size_t)blockIdx.x * HB_NMOM, tid - 32 * IO_WARP0, 128, 2);
         }
-    } else if (warp >= EPI_WARP0) {
+    } else {
         // ===================================================== hidden-layer epilogue warps
         const int wq = warp & 3;
         const int grp = (warp - EPI_WARP0) >> 2;  // column group inside every 64-column slab
@@ -472,6 +536,9 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
         const uint32_t a_row = sbase + pl.a_off + row * 128;
         const uint32_t sw = (uint32_t)(row & 7);
         const uint32_t tlane = tmem_base + ((uint32_t)(32 * wq) << 16);
+        TR_DECL;
+        const int trole = 4 + (warp - EPI_WARP0);
+        TR(trole, 0);
         uint32_t ph_d = 0;                        // bit b: parity of the next completion of D_HID[b]
         for (size_t g = cluster_id; g < ngroups; g += nclusters) {
             for (int l = 0; l < L - 1; ++l) {
@@ -480,9 +547,10 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                 const float* bl = bias_s + pl.bias_off[l];
                 const float slope = sd.prelu[l];
                 const uint32_t t0 = tlane + (uint32_t)(b * pl.d_cols + grp * CW);
-                mbar_wait<false>(bar(B_D_HID + b), (ph_d >> b) & 1);
+                mbar_wait<true>(bar(B_D_HID + b), (ph_d >> b) & 1);
                 ph_d ^= 1u << b;
                 tc_fence_after();
+                TR(trole, 2);
                 uint32_t ra[CW], rb[CW];
                 tmem_ld<CW>(t0, ra);
                 for (int j = 0; j < nsl; j += 2) {
@@ -493,6 +561,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive_cluster(bar(B_SLAB_FULL + j), 0);
+                    if (j == 0) TR(trole, 16);
                     if (j + 1 < nsl) {
                         tmem_ld_wait();
                         if (j + 2 < nsl) tmem_ld<CW>(t0 + 64 * (j + 2), ra);
@@ -501,6 +570,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                         tc_fence_before();
                         __syncwarp();
                         if (lane == 0) mbar_arrive_cluster(bar(B_SLAB_FULL + j + 1), 0);
+                        if (j + 2 >= nsl) TR(trole, 19);
                     }
                 }
             }
@@ -510,7 +580,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
     tc_fence_before();
     __syncthreads();
     if (CG == 2) cluster_sync_all();
-    if (warp == 1) {
+    if (warp == MMA_WARP) {
         tc_fence_after();
         tmem_dealloc<CG>(tmem_base, (uint32_t)pl.tmem_cols);
     }
@@ -578,7 +648,7 @@ cudaError_t launch_one(const HbParticles& p, size_t n, const HbSurDev& sd, const
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(grid);
-    cfg.blockDim = dim3(32 * (EPI_WARP0 + 4 * G));
+    cfg.blockDim = dim3(tc_threads(G));
     cfg.dynamicSmemBytes = smem;
     cfg.stream = s;
     cudaLaunchAttribute at[1];
@@ -625,6 +695,12 @@ int choose_g() {
 }
 
 }  // namespace
+
+#ifdef HB_TC_TRACE
+extern "C" int hb_debug_tc_trace(long long* host, int count) {
+    return (int)cudaMemcpyFromSymbol(host, hb_tc_trace_buf, sizeof(long long) * (size_t)count);
+}
+#endif
 
 bool hb_tc_supported(int prec, int n_linear, const int* widths, char* why, size_t why_len) {
     if (prec != 1 && prec != 2) {
