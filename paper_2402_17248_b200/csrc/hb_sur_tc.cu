@@ -88,6 +88,13 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar, uint32_t rank)
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(bar), "r"(rank));
     asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(remote) : "memory");
 }
+// non-blocking probe (try_wait may suspend the thread for a while when the phase is still open)
+__device__ __forceinline__ uint32_t mbar_test(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                 "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok;
+}
 __device__ __forceinline__ uint32_t mbar_try(uint32_t bar, uint32_t parity) {
     uint32_t ok;
     asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
@@ -396,46 +403,68 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
             TR_DECL;
             uint32_t ph_slab = 0;                    // bit j: parity of the next completion of SLAB_FULL[j]
             uint32_t it = 0;
+            // per-layer constants are fetched one layer ahead: anything issued behind a batch of MMAs waits for
+            // the tensor pipe's queue, so the loads for layer l+1 go out before the MMAs of layer l
+            struct LayerC { uint32_t idesc; int nsl; uint64_t bd, bd_step; };
+            auto layer_consts = [&](int l) {
+                LayerC c;
+                c.idesc = idesc_base | ((uint32_t)(pl.npad[l] >> 3) << 17);
+                c.nsl = pl.nslab[l];
+                c.bd = make_desc(sbase + pl.w_off[l]);
+                c.bd_step = (uint64_t)(pl.w_slab_bytes[l] >> 4);
+                return c;
+            };
+            const LayerC c0 = layer_consts(0);
+            const bool more_than_one = L > 1;
+            // layer 0 of tile `t`: one K = 16 MMA from the compact operand buffers.  It is issued directly behind
+            // the last layer of tile t-1, so that its epilogue runs while the IO warps finish tile t-1.
+            auto issue_l0 = [&](uint32_t t) {
+                // L odd: D[0] is also the output buffer, the IO warps must have read tile t-1 out of it
+                if (last_buf == 0 && t > 0) mbar_wait<true>(bar(B_OUT_READ), (t - 1) & 1);
+                TR(0, 1);
+                mbar_wait<true>(bar(B_A0_FULL + (t & 1)), (t >> 1) & 1);
+                tc_fence_after();
+                TR(0, 2);
+                if (issuer) {
+                    umma<CG, false>(tmem_base, make_desc_l0(sbase + pl.a0_off + (t & 1) * A0_BYTES), w0_desc, c0.idesc);
+                    umma_commit<CG>(more_than_one ? bar(B_D_HID) : bar(B_D_LAST));
+                }
+                __syncwarp();
+                TR(0, 32);
+            };
+            if (cluster_id < ngroups) issue_l0(0);
+            LayerC nxt = layer_consts(more_than_one ? 1 : 0);
             for (size_t g = cluster_id; g < ngroups; g += nclusters, ++it) {
-                for (int l = 0; l < L; ++l) {
+                for (int l = 1; l < L; ++l) {
+                    const LayerC cur = nxt;
+                    nxt = layer_consts(l + 1 < L ? l + 1 : 1);
                     const uint32_t d_tmem = tmem_base + (uint32_t)((l & 1) * pl.d_cols);
-                    const uint32_t idesc = idesc_base | ((uint32_t)(pl.npad[l] >> 3) << 17);
-                    const int nsl = pl.nslab[l];
-                    const uint64_t bd = make_desc(sbase + pl.w_off[l]);
-                    const uint64_t bd_step = (uint64_t)(pl.w_slab_bytes[l] >> 4);
+                    const uint32_t idesc = cur.idesc;
+                    const int nsl = cur.nsl;
+                    const uint64_t bd = cur.bd, bd_step = cur.bd_step;
                     // D[last_buf] still holds the previous tile's outputs until the IO warps have read them
                     if (it > 0 && l == last_buf) mbar_wait<true>(bar(B_OUT_READ), (it - 1) & 1);
-                    if (l == 0) {
-                        TR(0, 1);
-                        mbar_wait<true>(bar(B_A0_FULL + (it & 1)), (it >> 1) & 1);
-                        tc_fence_after();
-                        TR(0, 2);
-                        if (issuer) umma<CG, false>(d_tmem, make_desc_l0(sbase + pl.a0_off + (it & 1) * A0_BYTES), w0_desc, idesc);
-                    } else {
-                        // fully unrolled over the (at most MAX_SLABS) K slabs: every MMA of a layer gets its own
-                        // descriptor registers, so that forming the next slab's descriptors never has to wait for
-                        // an MMA still queued in the tensor pipe to release them (measured: +200 cycles per slab)
-                        uint32_t ready = 0;               // slab j's barrier already seen complete (peeked)
+                    // fully unrolled over the (at most MAX_SLABS) K slabs
+                    uint32_t ready = 0;               // slab j's barrier already seen complete (peeked)
 #pragma unroll
-                        for (int j = 0; j < MAX_SLABS; ++j) {
-                            if (j < nsl) {
-                                if (!ready) mbar_wait<true>(bar(B_SLAB_FULL + j), (ph_slab >> j) & 1);
-                                ph_slab ^= 1u << j;
-                                tc_fence_after();
-                                // peek at the next slab before this slab's MMAs go out: an MMA issue can hold the
-                                // warp for as long as the tensor pipe's queue is full
-                                ready = (j + 1 < nsl) ? mbar_try(bar(B_SLAB_FULL + j + 1), (ph_slab >> (j + 1)) & 1) : 0u;
-                                if (j == 0) TR(0, 17);
-                                if (issuer) {
-                                    // four K = 16 steps inside the 64-wide slab: the start address advances by 32 B
-                                    const uint64_t ad = a_desc0 + (uint64_t)(j * (A_SLAB_BYTES >> 4));
-                                    const uint64_t bj = bd + (uint64_t)j * bd_step;
-                                    if (j == 0) umma<CG, false>(d_tmem, ad, bj, idesc);
-                                    else umma<CG, true>(d_tmem, ad, bj, idesc);
-                                    umma<CG, true>(d_tmem, ad + 2, bj + 2, idesc);
-                                    umma<CG, true>(d_tmem, ad + 4, bj + 4, idesc);
-                                    umma<CG, true>(d_tmem, ad + 6, bj + 6, idesc);
-                                }
+                    for (int j = 0; j < MAX_SLABS; ++j) {
+                        if (j < nsl) {
+                            if (!ready) mbar_wait<true>(bar(B_SLAB_FULL + j), (ph_slab >> j) & 1);
+                            ph_slab ^= 1u << j;
+                            tc_fence_after();
+                            // peek at the next slab before this slab's MMAs go out: whatever the warp issues
+                            // behind a batch of MMAs waits while the tensor pipe's queue is full
+                            ready = (j + 1 < nsl) ? mbar_test(bar(B_SLAB_FULL + j + 1), (ph_slab >> (j + 1)) & 1) : 0u;
+                            if (j == 0) TR(0, 17);
+                            if (issuer) {
+                                // four K = 16 steps inside the 64-wide slab: the start address advances by 32 B
+                                const uint64_t ad = a_desc0 + (uint64_t)(j * (A_SLAB_BYTES >> 4));
+                                const uint64_t bj = bd + (uint64_t)j * bd_step;
+                                if (j == 0) umma<CG, false>(d_tmem, ad, bj, idesc);
+                                else umma<CG, true>(d_tmem, ad, bj, idesc);
+                                umma<CG, true>(d_tmem, ad + 2, bj + 2, idesc);
+                                umma<CG, true>(d_tmem, ad + 4, bj + 4, idesc);
+                                umma<CG, true>(d_tmem, ad + 6, bj + 6, idesc);
                             }
                         }
                     }
@@ -443,6 +472,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                     __syncwarp();
                     TR(0, 32 + l);
                 }
+                if (g + nclusters < ngroups) issue_l0(it + 1);
             }
         }
         __syncwarp();
