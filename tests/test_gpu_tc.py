@@ -135,3 +135,60 @@ def test_config4_tensor_core_per_stage(hb, prec):
     e = rel_err(got, ref)
     print("C4 free-running 2 stages", prec, "err/std:", e)
     assert np.all(np.isfinite(got))
+
+
+# ------------------------------------------------------------------ streamed-weights kernel (hb_sur_tcs.cu)
+@pytest.mark.parametrize("prec", ["bf16", "f16"])
+@pytest.mark.parametrize("H", [128, 512])
+def test_tcs_bringup_identity_net(hb, prec, H, monkeypatch):
+    """identity weights through the streamed kernel: ring blocks, N halves, descriptors, A_FREE protocol"""
+    monkeypatch.setenv("HB_TC_FORCE_STREAM", "1")
+    x = wl.gaussian_bunch(3000, 3, sigma=np.ones(6))
+    got, _ = gpu_push(hb, wl.lattice([identity_net(H, prec)]), x)
+    eps = 2.0 ** -8 if prec == "bf16" else 2.0 ** -11
+    assert np.all(np.isfinite(got))
+    assert np.max(np.abs(got - x) / np.maximum(np.abs(x), 1e-3)) <= 1.01 * eps
+
+
+@pytest.mark.parametrize("prec", ["bf16", "f16"])
+@pytest.mark.parametrize("act,widths", [("relu", [6, 256, 256, 256, 6]), ("tanh", [6, 128, 128, 128, 6]),
+                                        ("tanh", [6, 512, 512, 512, 512, 6]), ("prelu", [6, 300, 300, 6]),
+                                        ("relu", [6, 500, 6]), ("identity", [6, 384, 384, 384, 384, 384, 6])])
+def test_tcs_shapes(hb, prec, act, widths, monkeypatch):
+    """streamed kernel vs the oracle (forced for shapes the resident kernel would take)"""
+    monkeypatch.setenv("HB_TC_FORCE_STREAM", "1")
+    n = 20_000
+    init = "he" if act in ("relu", "prelu") else "xavier"
+    W, b = wl.make_mlp(widths, init, 56, len(widths))
+    rng = np.random.default_rng(7)
+    a = rng.uniform(0.05, 0.3, len(widths) - 2).astype(np.float32) if act == "prelu" else None
+    x = wl.correlated_bunch(n, 42)
+    x64 = x.astype(np.float64)
+    sur = wl.surrogate(widths, W, b, act, x64.mean(axis=1), x64.std(axis=1), rng.normal(size=6),
+                       rng.uniform(0.5, 2.0, 6), prelu_a=a, prec=prec)
+    desc = wl.lattice([sur, wl.monitor()])
+    ref, ref_rec = oracle.push(desc, x)
+    got, rec = gpu_push(hb, desc, x, moments=True)
+    e = rel_err(got, ref)
+    rms = np.sqrt(np.mean((got - ref) ** 2, axis=1)) / ref.std(axis=1)
+    print("streamed shape", widths, act, prec, "max err/std", e.max(), "rms err/std", rms.max())
+    assert np.all(np.isfinite(got))
+    assert e.max() <= TOL[prec]
+    own = oracle.moments(np.ascontiguousarray(got))
+    assert np.allclose(rec[0][:6], own[:6], rtol=1e-9, atol=1e-16)
+
+
+@pytest.mark.parametrize("n", [1, 129, 257, 40_001])
+def test_tcs_tiles_and_tails(hb, n, monkeypatch):
+    monkeypatch.setenv("HB_TC_FORCE_STREAM", "1")
+    widths = [6, 128, 128, 6]
+    W, b = wl.make_mlp(widths, "xavier", 57, 3)
+    z, o = np.zeros(6), np.ones(6)
+    x = wl.gaussian_bunch(max(n, 8), 18, sigma=np.ones(6))[:, :n].copy()
+    desc = wl.lattice([wl.surrogate(widths, W, b, "tanh", z, o, z, o, prec="f16"), wl.monitor()])
+    ref, _ = oracle.push(desc, x)
+    got, rec = gpu_push(hb, desc, x, moments=True)
+    assert np.all(np.isfinite(got))
+    assert np.max(np.abs(got - ref)) <= 2e-2
+    own = oracle.moments(np.ascontiguousarray(got))
+    assert np.allclose(rec[0][:6], own[:6], rtol=1e-9, atol=1e-16)
