@@ -47,14 +47,15 @@ enum : int {
 };
 
 template <int CG, int ACT, bool F16, int G>
-__global__ void __launch_bounds__(tc_threads(G), 1)
+__global__ void __launch_bounds__(tc_threads(G), G == 1 ? 2 : 1)
 hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, const __grid_constant__ TcPlan pl,
                  double* __restrict__ partials) {
     constexpr int THREADS = tc_threads(G);
     // the scheduler favours the highest warp id: the MMA issuer sits on top so that busy epilogue warps on the
     // same scheduler never delay an MMA issue
     constexpr int PROD_WARP = EPI_WARP0 + 4 * G, MMA_WARP = PROD_WARP + 1;
-    constexpr int CW = 64 / G;                       // accumulator columns per epilogue step of one warp
+    static_assert(G == 1 || G == 2, "epilogue warps = 4 x G");
+    constexpr int CW = 32;                           // accumulator columns per epilogue step of one warp
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     // the 128-byte swizzle atoms (8 rows x 128 B) must sit on 1024-byte boundaries of the shared window
     unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
@@ -319,6 +320,9 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                 const int nsl = pl.npad[l] >> 6;
                 const float* bl = bias_s + pl.bias_off[l];
                 const float slope = sd.prelu[l];
+                // this warp's 32-column chunks of the layer: columns 32 * (c * G + grp), c = 0 .. nch-1
+                // (G = 2: one chunk per 64-column slab; G = 1: both chunks of every slab)
+                const int nch = nsl * (2 / G);
                 const uint32_t t0 = tlane + (uint32_t)(b * pl.d_cols + grp * CW);
                 mbar_wait<true>(bar(B_D_HID + b), (ph_d >> b) & 1);
                 ph_d ^= 1u << b;
@@ -326,24 +330,27 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                 TR(trole, 2);
                 uint32_t ra[CW], rb[CW];
                 tmem_ld<CW>(t0, ra);
-                for (int j = 0; j < nsl; j += 2) {
+                for (int c = 0; c < nch; c += 2) {
+                    const int col_a = CW * (c * G + grp), col_b = CW * ((c + 1) * G + grp);
                     tmem_ld_wait();
-                    if (j + 1 < nsl) tmem_ld<CW>(t0 + 64 * (j + 1), rb);
-                    epi_store<CW, ACT, F16>(ra, bl, 64 * j + grp * CW, slope, a_row, sw);
-                    fence_proxy_async();
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive_cluster(bar(B_SLAB_FULL + j), 0);
-                    if (j == 0) TR(trole, 16);
-                    if (j + 1 < nsl) {
-                        tmem_ld_wait();
-                        if (j + 2 < nsl) tmem_ld<CW>(t0 + 64 * (j + 2), ra);
-                        epi_store<CW, ACT, F16>(rb, bl, 64 * (j + 1) + grp * CW, slope, a_row, sw);
+                    if (c + 1 < nch) tmem_ld<CW>(tlane + (uint32_t)(b * pl.d_cols + col_b), rb);
+                    epi_store<CW, ACT, F16>(ra, bl, col_a, slope, a_row, sw);
+                    if (G == 2 || c + 1 >= nch) {           // chunk a closes its slab
                         fence_proxy_async();
                         tc_fence_before();
                         __syncwarp();
-                        if (lane == 0) mbar_arrive_cluster(bar(B_SLAB_FULL + j + 1), 0);
-                        if (j + 2 >= nsl) TR(trole, 19);
+                        if (lane == 0) mbar_arrive_cluster(bar(B_SLAB_FULL + (col_a >> 6)), 0);
+                        if (c == 0) TR(trole, 16);
+                    }
+                    if (c + 1 < nch) {
+                        tmem_ld_wait();
+                        if (c + 2 < nch) tmem_ld<CW>(tlane + (uint32_t)(b * pl.d_cols + CW * ((c + 2) * G + grp)), ra);
+                        epi_store<CW, ACT, F16>(rb, bl, col_b, slope, a_row, sw);
+                        fence_proxy_async();
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive_cluster(bar(B_SLAB_FULL + (col_b >> 6)), 0);
+                        if (c + 2 >= nch) TR(trole, 19);
                     }
                 }
             }
@@ -448,7 +455,7 @@ cudaError_t launch_act(const HbParticles& p, size_t n, const HbSurDev& sd, const
 template <int CG, bool F16>
 cudaError_t launch_g(int g, const HbParticles& p, size_t n, const HbSurDev& sd, const TcPlan& pl, double* partials, int grid,
                      cudaStream_t s) {
-    if (g == 4) return launch_act<CG, F16, 4>(p, n, sd, pl, partials, grid, s);
+    if (g == 1) return launch_act<CG, F16, 1>(p, n, sd, pl, partials, grid, s);
     return launch_act<CG, F16, 2>(p, n, sd, pl, partials, grid, s);
 }
 
@@ -470,10 +477,19 @@ bool use_stream(int n_linear, const int* widths) {
     return !choose_cg(n_linear, widths, pl) && hb_tcs_supported(n_linear, widths);
 }
 
-int choose_g() {
-    // HB_TC_EPI_GROUPS=2|4 : hidden-layer epilogue warps = 4 x groups (tuning hook; default 2)
-    const char* e = getenv("HB_TC_EPI_GROUPS");
-    return (e && e[0] == '4') ? 4 : 2;
+// Launch shape.  Small networks (CTA-pair plan <= 113 KB of shared memory, two accumulators <= 256 TMEM
+// columns) run TWO CTAs per SM with 4 epilogue warps each (G = 1): the second tile's MMAs fill the tensor pipe
+// while the first tile is in its (MUFU- or latency-bound) epilogue.  Everything else: one CTA per SM, G = 2.
+// HB_TC_OCC2=0 : tuning/test hook, disables the two-CTAs-per-SM shape.
+struct TcShape { int cg, g, occ; };
+TcShape choose_shape(int n_linear, const int* widths, TcPlan& pl) {
+    const char* force = getenv("HB_TC_FORCE_CG");
+    const char* occ2 = getenv("HB_TC_OCC2");
+    const bool allow_occ2 = !(occ2 && occ2[0] == '0') && !force;
+    if (allow_occ2 && make_plan(2, n_linear, widths, pl) && (size_t)pl.total + 2048 <= SMEM_LIMIT / 2 && pl.tmem_cols <= 256)
+        return {2, 1, 2};
+    const int cg = choose_cg(n_linear, widths, pl);
+    return {cg, 2, 1};
 }
 
 }  // namespace
@@ -543,17 +559,17 @@ cudaError_t hb_launch_sur_tc(const HbParticles& p, size_t n, const HbSurDev& sd,
                              int sm_count, cudaStream_t s) {
     if (use_stream(sd.n_linear, sd.widths)) return hb_launch_sur_tcs(p, n, sd, partials, nblocks_out, sm_count, s);
     TcPlan pl;
-    const int cg = choose_cg(sd.n_linear, sd.widths, pl);
+    const TcShape sh = choose_shape(sd.n_linear, sd.widths, pl);
+    const int cg = sh.cg, g = sh.g;
     if (cg == 0) return cudaErrorNotSupported;
     const size_t ntiles = (n + TILE_M - 1) / TILE_M;
     const size_t ngroups = (ntiles + cg - 1) / cg;
-    size_t clusters = (size_t)(sm_count / cg);
+    size_t clusters = (size_t)(sm_count / cg) * sh.occ;
     if (clusters > ngroups) clusters = ngroups;
     if (clusters < 1) clusters = 1;
     const int grid = (int)clusters * cg;
     if (nblocks_out) *nblocks_out = grid;
     const bool f16 = sd.prec == 2;
-    const int g = choose_g();
     if (cg == 1) return f16 ? launch_g<1, true>(g, p, n, sd, pl, partials, grid, s) : launch_g<1, false>(g, p, n, sd, pl, partials, grid, s);
     return f16 ? launch_g<2, true>(g, p, n, sd, pl, partials, grid, s) : launch_g<2, false>(g, p, n, sd, pl, partials, grid, s);
 }

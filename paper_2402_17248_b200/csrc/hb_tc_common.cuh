@@ -70,16 +70,24 @@ __device__ __forceinline__ uint32_t mbar_try(uint32_t bar, uint32_t parity) {
                  "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     return ok;
 }
+// try_wait with a suspend-time hint: the thread sleeps in hardware until the phase completes (or the hint
+// expires) instead of spinning through the issue slots of the warps that do the work
+__device__ __forceinline__ uint32_t mbar_try_sleep(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+                 "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar), "r"(parity), "r"(200000u) : "memory");
+    return ok;
+}
 // FAST: latency-critical waiters try a few times before they start reading the clock for the hang guard.
 template <bool FAST>
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     if (FAST) {
 #pragma unroll 1
-        for (int i = 0; i < 64; ++i)
+        for (int i = 0; i < 16; ++i)
             if (mbar_try(bar, parity)) return;
     }
     const long long t0 = clock64();
-    while (!mbar_try(bar, parity)) {
+    while (!mbar_try_sleep(bar, parity)) {
         if (clock64() - t0 > 4000000000LL) {   // ~2 s: a protocol bug must not hang the GPU
             printf("hb_sur_tc: mbarrier timeout (block %d thread %d bar %u parity %u)\n", blockIdx.x, threadIdx.x, bar, parity);
             __trap();
