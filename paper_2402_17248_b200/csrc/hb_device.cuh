@@ -26,24 +26,41 @@ struct HbMomAcc {
     }
 };
 
-// Block-level fixed-order reduction of the 27 accumulators: warp xor-shuffle tree, then warp 0..
-// sums the per-warp values in warp order.  `scratch` : shared, >= (blockDim/32)*27 doubles.
-// All threads of the participating group [tid0, tid0+nthreads) must call; `bar_id` named barrier.
+// Block-level fixed-order reduction of the 27 accumulators.  Inside a warp a reduce-scatter butterfly (step
+// h = 16, 8, .., 1: each lane keeps one half of its values, sends the other half to lane ^ h and adds what it
+// receives) leaves the warp total of moment l in lane l with 31 shuffles instead of 27 x 5; warp 0.. then sums the
+// per-warp values in warp order.  `scratch`: shared, >= (blockDim/32)*27 doubles.  All threads of the
+// participating group [tid0, tid0+nthreads) must call; `bar_id` named barrier.
+// The block's 27 sums go to out_partial[j * HB_MOM_MAX_BLOCKS] (moment-major partials: the finalize kernel then
+// reads every moment's row with consecutive lanes on consecutive addresses).
 __device__ __forceinline__ void hb_block_reduce_moments(HbMomAcc& acc, double* scratch, double* out_partial,
                                                         int tid, int nthreads, int bar_id) {
     const int lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
+    double v[32];
 #pragma unroll
-    for (int i = 0; i < HB_NMOM; ++i) {
-        double v = acc.s[i];
+    for (int i = 0; i < 32; ++i) v[i] = i < HB_NMOM ? acc.s[i] : 0.0;
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        if (lane == 0) scratch[warp * HB_NMOM + i] = v;
+    for (int h = 16; h >= 1; h >>= 1) {
+        const bool upper = (lane & h) != 0;
+#pragma unroll
+        for (int i = 0; i < h; ++i) {
+            if (i + h >= HB_NMOM && h == 16) {          // indices 27..31 are padding: nothing to send or keep
+                const double send = upper ? v[i] : 0.0;
+                const double got = __shfl_xor_sync(0xffffffffu, send, h);
+                v[i] = upper ? 0.0 : v[i] + got;
+            } else {
+                const double keep = upper ? v[i + h] : v[i];
+                const double send = upper ? v[i] : v[i + h];
+                v[i] = keep + __shfl_xor_sync(0xffffffffu, send, h);
+            }
+        }
     }
+    if (lane < HB_NMOM) scratch[warp * HB_NMOM + lane] = v[0];
     asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "r"(nthreads) : "memory");
     if (tid < HB_NMOM) {
-        double v = 0.0;
-        for (int w = 0; w < nwarps; ++w) v += scratch[w * HB_NMOM + tid];
-        out_partial[tid] = v;
+        double t = 0.0;
+        for (int w = 0; w < nwarps; ++w) t += scratch[w * HB_NMOM + tid];
+        out_partial[(size_t)tid * HB_MOM_MAX_BLOCKS] = t;
     }
 }
 

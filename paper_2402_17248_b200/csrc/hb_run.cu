@@ -63,7 +63,7 @@ hb_run_composed_kernel(HbParticles p, size_t n, const __grid_constant__ HbRunMap
         for (int j = 0; j < 6; ++j) p.v[j][i] = out[j];
         if (MOM) acc.add(out[0], out[1], out[2], out[3], out[4], out[5]);
     }
-    if (MOM) hb_block_reduce_moments(acc, red, partials + (size_t)blockIdx.x * HB_NMOM, threadIdx.x, RUN_THREADS, 1);
+    if (MOM) hb_block_reduce_moments(acc, red, partials + blockIdx.x, threadIdx.x, RUN_THREADS, 1);
 }
 
 // ---------------------------------------------------------------------------------- sequential
@@ -168,7 +168,7 @@ hb_run_sequential_kernel(HbParticles p, size_t n, const HbSeqElem* __restrict__ 
         }
     }
     (void)first;
-    if (MOM) hb_block_reduce_moments(acc, red, partials + (size_t)blockIdx.x * HB_NMOM, threadIdx.x, RUN_THREADS, 1);
+    if (MOM) hb_block_reduce_moments(acc, red, partials + blockIdx.x, threadIdx.x, RUN_THREADS, 1);
 }
 
 // ---------------------------------------------------------------------------------- standalone moments
@@ -200,18 +200,29 @@ hb_moments_partials_kernel(HbParticles p, size_t n, const __grid_constant__ HbPi
         for (int j = 0; j < 6; ++j) v[j] = (double)p.v[j][i] - pv.p[j];
         acc.add(v);
     }
-    hb_block_reduce_moments(acc, red, partials + (size_t)blockIdx.x * HB_NMOM, threadIdx.x, RUN_THREADS, 1);
+    hb_block_reduce_moments(acc, red, partials + blockIdx.x, threadIdx.x, RUN_THREADS, 1);
 }
 
-// One block of 27 warps: warp j sums partial[k][j], k = lane, lane+32, ... in a fixed order, then a
-// shuffle tree.  Then threads 0..26 turn the raw sums into the record (means + centred covariance, 1/N).
-__global__ void __launch_bounds__(HB_NMOM * 32, 1)
+// One block of 27 warps: warp j sums partial[j][k] (moment-major), k = lane, lane+32, ... in a fixed order (loads issued eight
+// at a time so that their latencies overlap), then an xor-shuffle tree.  Threads 0..26 turn the raw sums into the
+// record (means + centred covariance, 1/N).
+#define FIN_THREADS (HB_NMOM * 32)
+__global__ void __launch_bounds__(FIN_THREADS, 1)
 hb_moments_finalize_kernel(const double* __restrict__ partials, int nblocks, size_t n,
                            const __grid_constant__ HbPivot pv, double* __restrict__ out) {
     __shared__ double S[HB_NMOM];
     const int j = threadIdx.x >> 5, lane = threadIdx.x & 31;
     double v = 0.0;
-    for (int k = lane; k < nblocks; k += 32) v += partials[(size_t)k * HB_NMOM + j];
+    for (int k0 = lane; k0 < nblocks; k0 += 32 * 8) {
+        double t[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int k = k0 + 32 * u;
+            t[u] = k < nblocks ? __ldcg(partials + (size_t)j * HB_MOM_MAX_BLOCKS + k) : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v += t[u];
+    }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     if (lane == 0) S[j] = v;
@@ -279,6 +290,6 @@ cudaError_t hb_launch_moments_finalize(const double* partials, int nblocks, size
                                        double* d_out27, cudaStream_t s) {
     HbPivot pv;
     for (int j = 0; j < 6; ++j) pv.p[j] = pivot6_host ? pivot6_host[j] : 0.0;
-    hb_moments_finalize_kernel<<<1, HB_NMOM * 32, 0, s>>>(partials, nblocks, n, pv, d_out27);
+    hb_moments_finalize_kernel<<<1, FIN_THREADS, 0, s>>>(partials, nblocks, n, pv, d_out27);
     return cudaGetLastError();
 }

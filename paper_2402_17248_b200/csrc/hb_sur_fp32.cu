@@ -114,7 +114,7 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
     }
     if (MOM) {
         __syncthreads();
-        hb_block_reduce_moments(acc, red, partials + (size_t)blockIdx.x * HB_NMOM, tid, NT, 1);
+        hb_block_reduce_moments(acc, red, partials + blockIdx.x, tid, NT, 1);
     }
 }
 

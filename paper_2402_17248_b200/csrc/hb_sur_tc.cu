@@ -300,7 +300,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
         }
         if (partials) {
             double* red = reinterpret_cast<double*>(smem + pl.red_off);
-            hb_block_reduce_moments(acc, red, partials + (size_t)blockIdx.x * HB_NMOM, tid - 32 * IO_WARP0, 128, 2);
+            hb_block_reduce_moments(acc, red, partials + blockIdx.x, tid - 32 * IO_WARP0, 128, 2);
         }
     } else {
         // ===================================================== hidden-layer epilogue warps

@@ -330,7 +330,7 @@ hb_sur_tcs_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
         }
         if (partials) {
             double* red = reinterpret_cast<double*>(smem + pl.red_off);
-            hb_block_reduce_moments(acc, red, partials + (size_t)blockIdx.x * HB_NMOM, tid, 128, 2);
+            hb_block_reduce_moments(acc, red, partials + blockIdx.x, tid, 128, 2);
         }
     } else if (warp < 12) {
         // ===================================================== hidden-layer epilogue warps
