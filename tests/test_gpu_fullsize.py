@@ -1,0 +1,129 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (-m gpu).
+
+Every step of the path is a per-particle map, so the fp64 oracle can compute any particle of a 1e7 / 1e8
+bunch on its own: the GPU pushes the whole bunch through the C ABI, the oracle pushes a seeded sample of it
+(first tile, last tile, ragged tail, and a spread of particles in between), and the two are compared element by
+element.  The moment records are checked by a property that holds at any size: the record the kernels reduce on
+the device equals the plain fp64 moments (oracle R10) of the very output they wrote.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f16": 2e-2, "bf16": 1.5e-1, "fp32": 1e-5}
+
+
+@pytest.fixture(scope="module")
+def hb():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2402_17248_b200 as hb
+    hb.lib()
+    return hb
+
+
+def sample_indices(n, m=6000, seed=99):
+    rng = np.random.default_rng(seed)
+    edge = np.concatenate([np.arange(0, min(n, 300)), np.arange(max(0, n - 300), n)])
+    mid = rng.integers(0, n, size=m)
+    return np.unique(np.concatenate([edge, mid]))
+
+
+def gpu_push_full(hb, desc, x, prec=None):
+    import torch
+    lat = hb.Lattice.from_description(desc, device=0, prec=prec)
+    c = hb.to_device(x)
+    rec = lat.push_moments(c)
+    torch.cuda.synchronize()
+    out = hb.to_host(c)
+    lat.close()
+    del c
+    torch.cuda.empty_cache()
+    return out, rec.cpu().numpy()
+
+
+def check_moments(rec_last, out):
+    own = oracle.moments(np.ascontiguousarray(out.astype(np.float64)))
+    assert np.allclose(rec_last[:6], own[:6], rtol=1e-9, atol=1e-15)
+    diag = [6, 12, 17, 21, 24, 26]
+    assert np.allclose(rec_last[diag], own[diag], rtol=1e-9)
+    scale = np.sqrt(np.outer(own[diag], own[diag]))[np.triu_indices(6)]
+    assert np.all(np.abs(rec_last[6:] - own[6:]) <= 1e-9 * scale)
+
+
+@pytest.mark.parametrize("prec", ["bf16", "f16"])
+def test_config3_full_size_sampled(hb, prec):
+    """C3, N = 1e7, the bench's headline launch: sampled particles vs the oracle, record vs the output."""
+    desc, x = wl.config3(prec=prec)
+    n = x.shape[1]
+    assert n == 10_000_000
+    out, rec = gpu_push_full(hb, desc, x)
+    idx = sample_indices(n)
+    ref, _ = oracle.push(desc, np.ascontiguousarray(x[:, idx]))
+    assert np.all(np.isfinite(out))
+    std = out.astype(np.float64).std(axis=1)
+    err = np.max(np.abs(out[:, idx].astype(np.float64) - ref), axis=1) / std
+    print("C3 full size", prec, "max err/std on", idx.size, "sampled particles:", err)
+    assert err.max() <= TOL[prec]
+    check_moments(rec[-1], out)
+
+
+def test_config2_full_size_sampled(hb):
+    """conventional run at the size the HBM roofline is quoted on (N = 1e7, 500 elements in one fused pass)"""
+    desc, x = wl.config2(n=10_000_000)
+    out, rec = gpu_push_full(hb, desc, x)
+    idx = sample_indices(x.shape[1])
+    ref, _ = oracle.push(desc, np.ascontiguousarray(x[:, idx]))
+    std = out.astype(np.float64).std(axis=1)
+    err = np.max(np.abs(out[:, idx].astype(np.float64) - ref), axis=1) / std
+    print("C2 lattice N=1e7 max err/std:", err)
+    assert err.max() <= 1e-6
+    check_moments(rec[-1], out)
+
+
+def test_config4_full_size_sampled(hb):
+    """C4, N = 1e7, f16 operands, whole hybrid lattice (2 COORD_T stages + transport + chicane), free running"""
+    desc, x = wl.config4(prec="f16")
+    out, rec = gpu_push_full(hb, desc, x)
+    idx = sample_indices(x.shape[1])
+    ref, _ = oracle.push(desc, np.ascontiguousarray(x[:, idx]))
+    assert np.all(np.isfinite(out))
+    std = out.astype(np.float64).std(axis=1)
+    err = np.max(np.abs(out[:, idx].astype(np.float64) - ref), axis=1) / std
+    print("C4 full size f16 free-running max err/std:", err)
+    assert err.max() <= 5e-2          # two 16-bit stages in a row (per-stage bound 2e-2: test_gpu_tc.py)
+    assert rec.shape[0] == 4
+    check_moments(rec[-1], out)
+
+
+def test_config5_full_size_first_stage_and_run(hb):
+    """C5's bunch (N = 1e8, 2.4 GB) through its first surrogate stage (6-512^4-6 tanh, streamed weights) and
+    first transport section, f16 operands: sampled particles vs the oracle; then the whole 17-segment lattice in
+    bf16 for finiteness and the record property."""
+    desc, x = wl.config5(prec="f16")
+    n = x.shape[1]
+    assert n == 100_000_000
+    first = wl.lattice(desc["elements"][:53])      # surrogate, monitor, 50 elements, monitor
+    assert first["elements"][0]["kind"] == "surrogate" and first["elements"][-1]["kind"] == "monitor"
+    out, rec = gpu_push_full(hb, first, x)
+    idx = sample_indices(n)
+    ref, _ = oracle.push(first, np.ascontiguousarray(x[:, idx]))
+    std = out[:, ::97].astype(np.float64).std(axis=1)
+    err = np.max(np.abs(out[:, idx].astype(np.float64) - ref), axis=1) / std
+    print("C5 N=1e8 stage 1 + run, f16, max err/std:", err)
+    assert err.max() <= TOL["f16"]
+    assert rec.shape[0] == 2
+    del out
+    desc_b, _ = wl.config5(prec="bf16", particles=False)
+    out, rec = gpu_push_full(hb, desc_b, x)
+    assert rec.shape[0] == 17 and np.all(np.isfinite(rec))
+    sub = out[:, ::50]
+    assert np.all(np.isfinite(sub))
+    own = oracle.moments(np.ascontiguousarray(out[:, :5_000_000].astype(np.float64)))
+    assert np.all(np.isfinite(own))
+    # record of the whole bunch vs plain moments of a 5e6-particle prefix: statistical agreement only
+    assert np.allclose(np.sqrt(rec[-1][[6, 17, 24]]), np.sqrt(own[[6, 17, 24]]), rtol=5e-2)
