@@ -32,6 +32,13 @@ import workloads as wl  # noqa: E402
 
 METRIC = "particle-element pushes/s & surrogate particles/s at 1e7; % of HBM/tensor peak"
 L2_FLUSH_BYTES = 256 << 20
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch, from the `ncu --set full` captures summarised in
+# profiles/r1_kernels_v2.md (same commands as there; N = 1e7).  Algorithmic bytes are 480e6 per launch in all three.
+NCU_TRAFFIC = {
+    ("hb_sur_tc_kernel", 10_000_000): 421.3e6,
+    ("hb_sur_tcs_kernel", 10_000_000): 429.0e6,
+    ("hb_run_composed_kernel", 10_000_000): 422.8e6,
+}
 
 
 def peaks():
@@ -44,7 +51,7 @@ def peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks line of B200_PROFILING.md, sampled every 200 ms during the timed region."""
+    """nvidia-smi clocks line of B200_PROFILING.md, sampled every 20 ms during the timed region."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -54,7 +61,7 @@ class ClockSampler:
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                                       "--format=csv,noheader,nounits", "-lms", "200"], stdout=self.f,
+                                       "--format=csv,noheader,nounits", "-lms", "20"], stdout=self.f,
                                       stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
@@ -173,7 +180,7 @@ def oracle_rate(desc, x, budget_s, unit_count):
     oracle.push(desc, x[:, :probe])
     dt = max(time.perf_counter() - t0, 1e-4)
     ns = int(min(n, max(probe, (probe / dt) * budget_s)))
-    ns = min(ns, 1 << 20)
+    ns = min(ns, 1 << 22)
     t0 = time.perf_counter()
     oracle.push(desc, x[:, :ns])
     dt = time.perf_counter() - t0
@@ -271,6 +278,20 @@ def kernel_extras(torch, hb, args, pk, flush, dev):
                     "roofline": {"bound": "alu", "achieved": ach, "peak": fma_peak, "unit": "TFMA/s (fp32)",
                                  "frac": ach / fma_peak, "traffic": None}})
         del x3
+        # (b2) one C5 stage (6-512^4-6 tanh, weights streamed from L2) at N = 1e7
+        desc5, _ = wl.config5(prec="bf16", particles=False)
+        d5 = wl.lattice(desc5["elements"][:2])
+        x5 = wl.gaussian_bunch(n, 5)
+        fl5 = wl.flops_per_particle(d5["elements"][0]["widths"])
+        ms, seg = measure(d5, x5, "sur", True, steps=5)
+        k_ms = float(seg[0])
+        tf = fl5 * n / (k_ms * 1e-3) / 1e12
+        out.append({"kernel": "hb_sur_tcs_kernel<bf16> (streamed weights)", "workload": "one C5 stage 6-512^4-6 tanh, N=%d" % n, "ms": k_ms,
+                    "particle_inferences_per_s": n / (k_ms * 1e-3),
+                    "roofline": {"bound": "tensor", "achieved": tf, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
+                                 "frac": tf / pk["bf16_tflops"], "frac_of_sustained": tf / pk["bf16_tflops_sustained"],
+                                 "traffic": None, "peak_source": pk["source"]}})
+        del x5
         # (c) C4 hybrid lattice (all rows a1-a7 in one push)
         desc4, x4 = wl.config4(prec="bf16", n=n)
         ms, seg = measure(desc4, x4, "c4", True)
@@ -376,15 +397,18 @@ def main():
     if kinds[dom] == "sur":
         per = flops / max(n_sur, 1)
         ach = per * n / (dom_ms * 1e-3) / 1e12
+        widest = max(max(e["widths"][1:-1]) for e in desc["elements"] if e["kind"] == "surrogate")
+        kname = "hb_sur_tcs_kernel" if widest > 256 else "hb_sur_tc_kernel"
         roof = {"bound": "tensor", "achieved": ach, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
-                "frac": ach / pk["bf16_tflops"], "traffic": None, "kernel": "hb_sur_tc_kernel",
+                "frac": ach / pk["bf16_tflops"], "traffic": NCU_TRAFFIC.get((kname, n)), "kernel": kname,
                 "kernel_ms": dom_ms, "peak_source": pk["source"] + " (burst, cuBLAS bf16)",
                 "frac_of_sustained": ach / pk["bf16_tflops_sustained"],
                 "algorithmic_flop_per_particle": per}
     else:
         ach = 48.0 * n / (dom_ms * 1e-3) / 1e9
         roof = {"bound": "hbm", "achieved": ach, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": ach / pk["hbm_gbs"],
-                "traffic": None, "kernel": "hb_run_composed_kernel", "kernel_ms": dom_ms, "peak_source": pk["source"]}
+                "traffic": NCU_TRAFFIC.get(("hb_run_composed_kernel", n)), "kernel": "hb_run_composed_kernel",
+                "kernel_ms": dom_ms, "peak_source": pk["source"]}
 
     line = {
         "metric": METRIC, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
