@@ -88,3 +88,7 @@ size_t hb_tcs_pack_weights(int prec, int n_linear, const int* widths, const floa
                            void* dst, long long* off_bytes, int* kpad, int* npad);
 cudaError_t hb_launch_sur_tcs(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials,
                               int* nblocks_out, int sm_count, cudaStream_t s);
+// two-tiles-in-flight variant of the resident kernel (hb_sur_tc2.cu): same weight image as hb_tc_pack_weights
+bool hb_tc2_supported(int n_linear, const int* widths);
+cudaError_t hb_launch_sur_tc2(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials,
+                              int* nblocks_out, int sm_count, cudaStream_t s);

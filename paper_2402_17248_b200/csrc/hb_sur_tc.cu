@@ -560,6 +560,15 @@ cudaError_t hb_launch_sur_tc(const HbParticles& p, size_t n, const HbSurDev& sd,
     if (use_stream(sd.n_linear, sd.widths)) return hb_launch_sur_tcs(p, n, sd, partials, nblocks_out, sm_count, s);
     TcPlan pl;
     const TcShape sh = choose_shape(sd.n_linear, sd.widths, pl);
+    // HB_TC_TWO_TILES=1 : opt-in to the two-tiles-in-flight kernel (hb_sur_tc2.cu) where its operand ring fits.
+    // Measured slower than this file's pipeline on C3 (3.12 vs 2.63 ms): with an epilogue running under EVERY MMA
+    // phase the MMAs themselves slow from 512 to ~800 cycles per K slab (shared-memory traffic of the operand
+    // stores + proxy fences), which costs more than the exposed first-slab latency it removes.
+    {
+        const char* two = getenv("HB_TC_TWO_TILES");
+        if (sh.cg == 2 && sh.occ == 1 && two && two[0] == '1' && hb_tc2_supported(sd.n_linear, sd.widths))
+            return hb_launch_sur_tc2(p, n, sd, partials, nblocks_out, sm_count, s);
+    }
     const int cg = sh.cg, g = sh.g;
     if (cg == 0) return cudaErrorNotSupported;
     const size_t ntiles = (n + TILE_M - 1) / TILE_M;

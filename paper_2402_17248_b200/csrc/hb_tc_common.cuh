@@ -285,4 +285,26 @@ __device__ __forceinline__ void sts128(uint32_t addr, const uint32_t (&q)[4]) {
     asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(q[0]), "r"(q[1]), "r"(q[2]), "r"(q[3]) : "memory");
 }
 
+// Same step, but into one given 16 KB slab (ring slot): `slab_row` = address of this thread's row in the slab,
+// `ch0` = first 16-byte chunk of the row the CW columns go to, `bl` already points at the first column's bias.
+template <int CW, int ACT, bool F16>
+__device__ __forceinline__ void epi_store_slab(const uint32_t (&r)[CW], const float* __restrict__ bl, uint32_t ch0,
+                                               float slope, uint32_t slab_row, uint32_t sw) {
+    uint32_t q[CW / 2];
+#pragma unroll
+    for (int k = 0; k < CW / 4; ++k) {
+        const float4 b4 = *reinterpret_cast<const float4*>(bl + 4 * k);
+        float v0 = __uint_as_float(r[4 * k]), v1 = __uint_as_float(r[4 * k + 1]);
+        float v2 = __uint_as_float(r[4 * k + 2]), v3 = __uint_as_float(r[4 * k + 3]);
+        add2(v0, v1, b4.x, b4.y);
+        add2(v2, v3, b4.z, b4.w);
+        q[2 * k] = act_pack<ACT, F16>(v0, v1, slope);
+        q[2 * k + 1] = act_pack<ACT, F16>(v2, v3, slope);
+    }
+#pragma unroll
+    for (int k = 0; k < CW / 8; ++k)
+        asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(slab_row + (((ch0 + k) ^ sw) << 4)),
+                     "r"(q[4 * k]), "r"(q[4 * k + 1]), "r"(q[4 * k + 2]), "r"(q[4 * k + 3]) : "memory");
+}
+
 }  // namespace

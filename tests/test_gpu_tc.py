@@ -192,3 +192,30 @@ def test_tcs_tiles_and_tails(hb, n, monkeypatch):
     assert np.max(np.abs(got - ref)) <= 2e-2
     own = oracle.moments(np.ascontiguousarray(got))
     assert np.allclose(rec[0][:6], own[:6], rtol=1e-9, atol=1e-16)
+
+
+# ------------------------------------------------------------------ two-tiles-in-flight kernel (hb_sur_tc2.cu, opt-in)
+@pytest.mark.parametrize("prec", ["bf16", "f16"])
+@pytest.mark.parametrize("act,widths,n", [("relu", [6, 256, 256, 256, 6], 70_000), ("tanh", [6, 192, 192, 6], 20_001),
+                                          ("prelu", [6, 64, 64, 64, 64, 6], 333)])
+def test_tc2_shapes(hb, prec, act, widths, n, monkeypatch):
+    """operand-ring kernel vs the oracle: ring wrap-around, odd tile counts per CTA pair, ragged tails"""
+    monkeypatch.setenv("HB_TC_TWO_TILES", "1")
+    monkeypatch.setenv("HB_TC_FORCE_CG", "2")
+    init = "he" if act in ("relu", "prelu") else "xavier"
+    W, b = wl.make_mlp(widths, init, 58, len(widths))
+    rng = np.random.default_rng(8)
+    a = rng.uniform(0.05, 0.3, len(widths) - 2).astype(np.float32) if act == "prelu" else None
+    x = wl.correlated_bunch(n, 43)
+    x64 = x.astype(np.float64)
+    sur = wl.surrogate(widths, W, b, act, x64.mean(axis=1), x64.std(axis=1), rng.normal(size=6),
+                       rng.uniform(0.5, 2.0, 6), prelu_a=a, prec=prec)
+    desc = wl.lattice([sur, wl.monitor()])
+    ref, _ = oracle.push(desc, x)
+    got, rec = gpu_push(hb, desc, x, moments=True)
+    e = rel_err(got, ref)
+    print("two-tile shape", widths, act, prec, "max err/std", e.max())
+    assert np.all(np.isfinite(got))
+    assert e.max() <= TOL[prec]
+    own = oracle.moments(np.ascontiguousarray(got))
+    assert np.allclose(rec[0][:6], own[:6], rtol=1e-9, atol=1e-16)
