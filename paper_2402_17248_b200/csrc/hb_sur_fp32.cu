@@ -2,18 +2,20 @@
 //
 // One block owns a tile of TP particles.  Activations live in shared memory as [feature][particle]
 // (two ping-pong buffers); the transposed weights W^T [k][n] (packed, zero-padded to 64 outputs, by
-// hb_api.cu) are streamed through a [32][64] shared slab.  Each thread owns a 4-particle x 4-output
-// register tile.  Partial sums of each 32-wide K chunk are formed separately and then added (shorter
+// hb_api.cu) are streamed through a [32][64] shared slab (the next slab is fetched into registers while
+// the current one is multiplied).  Each thread owns a 4-particle x 4-output register tile.  Partial sums of each 32-wide K chunk are formed separately and then added (shorter
 // rounding chains), bias is added last in fp32, tanh is tanhf.
 // Prologue (s->t R6, normalise R8) and epilogue (de-normalise R8, reference R7, t->s R6, moments R10)
 // are fused: hidden activations never touch HBM (data preparation is 1-2 % of the push).
 #include "hb_device.cuh"
 
+#include <cstdlib>
+
 #define KC 32
 #define OC 64
 
 template <int TP, int ACT, bool MOM>
-__global__ void __launch_bounds__((TP / 4) * 16, 1)
+__global__ void __launch_bounds__((TP / 4) * 16, TP == 64 ? 1 : 3)
 hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, int hmax, double* __restrict__ partials) {
     constexpr int NT = (TP / 4) * 16;
     extern __shared__ __align__(16) float smem[];
@@ -52,15 +54,30 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
                 for (int a = 0; a < 4; ++a)
 #pragma unroll
                     for (int b = 0; b < 4; ++b) tot[a][b] = 0.0f;
+                // weight slab of the next K chunk travels global -> registers while this chunk is being multiplied
+                constexpr int PER = (KC * (OC / 4) + NT - 1) / NT;      // float4 per thread and slab
+                float4 pre[PER];
+                auto fetch = [&](int k0) {
+                    const int kk = min(KC, K - k0);
+#pragma unroll
+                    for (int u = 0; u < PER; ++u) {
+                        const int idx = tid + u * NT;
+                        const int k = idx / (OC / 4), c4 = idx % (OC / 4);
+                        pre[u] = k < kk ? __ldg(reinterpret_cast<const float4*>(Wt + (size_t)(k0 + k) * npad + o0) + c4)
+                                        : make_float4(0.f, 0.f, 0.f, 0.f);
+                    }
+                };
+                fetch(0);
                 for (int k0 = 0; k0 < K; k0 += KC) {
                     const int kk = min(KC, K - k0);
                     __syncthreads();          // previous slab consumed; layer input complete
-                    for (int idx = tid; idx < kk * (OC / 4); idx += NT) {
-                        const int k = idx / (OC / 4), c4 = idx % (OC / 4);
-                        reinterpret_cast<float4*>(Ws)[k * (OC / 4) + c4] =
-                            __ldg(reinterpret_cast<const float4*>(Wt + (size_t)(k0 + k) * npad + o0) + c4);
+#pragma unroll
+                    for (int u = 0; u < PER; ++u) {
+                        const int idx = tid + u * NT;
+                        if (idx < KC * (OC / 4)) reinterpret_cast<float4*>(Ws)[idx] = pre[u];
                     }
                     __syncthreads();
+                    if (k0 + KC < K) fetch(k0 + KC);
                     float part[4][4];
 #pragma unroll
                     for (int a = 0; a < 4; ++a)
@@ -144,10 +161,17 @@ cudaError_t hb_launch_sur_fp32(const HbParticles& p, size_t n, const HbSurDev& s
                                int* nblocks_out, int sm_count, cudaStream_t s) {
     int hmax = 64;
     for (int l = 0; l < sd.n_linear; ++l) hmax = hmax > sd.npad32[l] ? hmax : sd.npad32[l];
-    // tile size: two activation buffers of hmax x TP floats must fit beside the weight slab
-    int tp = hmax <= 384 ? 64 : (hmax <= 768 ? 32 : 16);
+    // tile size: two activation buffers of hmax x TP floats beside the weight slab; several blocks per SM when they
+    // fit (independent blocks hide each other's barriers and slab loads): hmax 256 -> TP 32, 72 KB, 3 blocks/SM
+    const char* force = getenv("HB_FP32_TP");
+    int tp = hmax <= 128 ? 64 : (hmax <= 768 ? 32 : 16);
+    if (force) tp = atoi(force) == 64 && hmax <= 384 ? 64 : (atoi(force) == 16 ? 16 : (hmax <= 768 ? 32 : 16));
+    const size_t smem_blk = ((size_t)2 * hmax * tp + KC * OC) * sizeof(float) + 1024;
+    int per_sm = (int)((227 * 1024) / smem_blk);
+    if (per_sm < 1) per_sm = 1;
+    if (per_sm > 4) per_sm = 4;
     const size_t ntiles = (n + tp - 1) / tp;
-    size_t g = (size_t)sm_count * (tp == 64 ? 1 : 1);
+    size_t g = (size_t)sm_count * per_sm;
     if (g > ntiles) g = ntiles;
     if (g < 1) g = 1;
     const int grid = (int)g;
