@@ -285,3 +285,31 @@ def test_stream_ordering_and_inplace(hb):
     got = c.cpu().numpy().astype(np.float64)
     assert rel_err(got, ref).max() <= 2e-6
     lat.close()
+
+
+def test_push_is_capturable_in_a_cuda_graph(hb):
+    """row a7: hb_push_moments only enqueues work on the caller's stream (no host sync, no allocation), so a whole
+    hybrid lattice (runs, tensor-core surrogate, monitors) can be captured once in a CUDA graph and replayed"""
+    import torch
+    desc, x = wl.config1(prec="f16", n=3000)
+    ref, ref_rec = oracle.push(desc, x)
+    lat = hb.Lattice.from_description(desc, device=0)
+    pristine = torch.from_numpy(x).cuda()
+    work = torch.empty_like(pristine)
+    rec = torch.zeros((lat.num_monitors, 27), dtype=torch.float64, device="cuda")
+    work.copy_(pristine)
+    lat.push_moments(work, out=rec)              # warm-up outside the capture (cudaFuncSetAttribute etc.)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        work.copy_(pristine)
+        lat.push_moments(work, out=rec)
+    for _ in range(3):
+        rec.zero_()
+        g.replay()
+    torch.cuda.synchronize()
+    got = work.cpu().numpy().astype(np.float64)
+    assert rel_err(got, ref).max() <= 2e-2
+    own = oracle.moments(np.ascontiguousarray(got))
+    assert np.allclose(rec[-1].cpu().numpy()[:6], own[:6], rtol=1e-9, atol=1e-16)
+    lat.close()
