@@ -299,9 +299,15 @@ def kernel_extras(torch, hb, args, pk, flush, dev):
         kinds = segment_kinds(desc4)
         sur_ms = float(np.mean([t for t, k in zip(seg, kinds) if k == "sur"]))
         run_ms = float(np.mean([t for t, k in zip(seg, kinds) if k == "run"]))
+        # a 6-128^3-6 tanh stage is bound by the special-function unit (16 tanh/clk/SM), not by the tensor pipe:
+        # 384 tanh per particle
+        xu_peak = 148 * 16 * 1.965e9 / 1e12
+        xu_ach = 384.0 * n / (sur_ms * 1e-3) / 1e12
         out.append({"kernel": "C4 whole push (2 surrogate + 2 run kernels + 4 moment finalizes)", "workload": "C4, N=%d" % n,
                     "ms": ms, "particles_per_s": n / (ms * 1e-3), "surrogate_ms": sur_ms, "run_ms": run_ms,
-                    "surrogate_tflops": fl4 * n / (sur_ms * 1e-3) / 1e12, "run_gbs": 48.0 * n / (run_ms * 1e-3) / 1e9})
+                    "surrogate_tflops": fl4 * n / (sur_ms * 1e-3) / 1e12, "run_gbs": 48.0 * n / (run_ms * 1e-3) / 1e9,
+                    "roofline": {"bound": "alu", "achieved": xu_ach, "peak": xu_peak, "unit": "Ttanh/s (MUFU, surrogate kernel)",
+                                 "frac": xu_ach / xu_peak, "traffic": None}})
     return out
 
 
