@@ -248,6 +248,26 @@ def kernel_extras(torch, hb, args, pk, flush, dev):
                     "ms": k_ms, "particle_element_pushes_per_s": 500.0 * n / (k_ms * 1e-3),
                     "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
                                  "frac": gbs / pk["hbm_gbs"], "traffic": None, "peak_source": pk["source"]}})
+    # same kernel at N = 1e8 (2.4 GB per bunch, 4.8 GB of traffic per launch): launch + event overhead (~6 us) no
+    # longer visible beside 730 us of streaming
+    if not args.n:
+        nb = 100_000_000
+        xb = wl.gaussian_bunch(nb, 2)
+        for mom in (False, True):
+            lat = hb.Lattice.from_description(desc2, run_mode="composed", device=dev.index)
+            pristine = torch.from_numpy(xb).to(dev)
+            work = torch.empty_like(pristine)
+            tot, seg, _ = timed_steps(torch, hb, lat, pristine, work, 5, 3, flush, with_moments=mom, segtimes=True)
+            lat.close()
+            del pristine, work
+            k_ms = float(seg[0])
+            gbs = 48.0 * nb / (k_ms * 1e-3) / 1e9
+            out.append({"kernel": "hb_run_composed_kernel" + ("<moments>" if mom else ""),
+                        "workload": "C2 lattice (500 elements, one run), N=%d" % nb, "ms": k_ms,
+                        "particle_element_pushes_per_s": 500.0 * nb / (k_ms * 1e-3),
+                        "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                                     "frac": gbs / pk["hbm_gbs"], "traffic": None, "peak_source": pk["source"]}})
+        del xb
     # sequential (fp64 registers, ALU-bound): 2700 DFMA-class ops per particle
     ms, seg = measure(desc2, x2, "run", False, steps=5, run_mode="sequential")
     k_ms = float(seg[0])
