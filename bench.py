@@ -289,6 +289,14 @@ def kernel_extras(torch, hb, args, pk, flush, dev):
                     "particle_inferences_per_s": n / (k_ms * 1e-3),
                     "roofline": {"bound": "tensor", "achieved": tf, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
                                  "frac": tf / pk["bf16_tflops"], "traffic": None, "peak_source": pk["source"]}})
+        ms, seg = measure(desc3, x3, "sur", True, steps=5, prec="tf32")
+        k_ms = float(seg[0])
+        tf = fl * n / (k_ms * 1e-3) / 1e12
+        out.append({"kernel": "hb_sur_tcs_kernel<tf32>", "workload": "C3, N=%d" % n, "ms": k_ms,
+                    "particle_inferences_per_s": n / (k_ms * 1e-3),
+                    "roofline": {"bound": "tensor", "achieved": tf, "peak": 0.5 * pk["bf16_tflops"], "unit": "TFLOP/s",
+                                 "frac": tf / (0.5 * pk["bf16_tflops"]), "traffic": None,
+                                 "peak_source": pk["source"] + " bf16 x 0.5 (nominal tf32 : bf16 ratio)"}})
         ms, seg = measure(desc3, x3, "sur", True, steps=2, prec="fp32")
         k_ms = float(seg[0])
         fma_peak = 148 * 128 * 1.965e9 / 1e12

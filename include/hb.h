@@ -52,7 +52,10 @@ typedef enum { HB_ELEM_DRIFT = 0, HB_ELEM_QUAD = 1, HB_ELEM_SBEND = 2, HB_ELEM_M
 typedef enum { HB_ACT_IDENTITY = 0, HB_ACT_RELU = 1, HB_ACT_PRELU = 2, HB_ACT_TANH = 3 } hb_act;
 
 /* Arithmetic of the MLP layers.  FP32: CUDA-core FFMA.  BF16/F16/TF32: tcgen05 tensor cores with
- * operands rounded to that type and fp32 accumulation in TMEM. */
+ * operands rounded to that type and fp32 accumulation in TMEM.  Shapes: BF16/F16 any hidden widths <= 256
+ * whose 16-bit weights fit in shared memory (resident kernel), else equal hidden widths <= 512 (weights
+ * streamed from L2); TF32 (half the tensor rate): at least one hidden layer, equal hidden widths <= 256.
+ * Anything else: hb_lattice_finalize returns HB_ERR_UNSUPPORTED -- never a slower fallback. */
 typedef enum { HB_PREC_FP32 = 0, HB_PREC_BF16 = 1, HB_PREC_F16 = 2, HB_PREC_TF32 = 3 } hb_prec;
 
 /* Coordinates the surrogate was trained in.  HB_COORD_S: the net sees (x,px,y,py,t,pt) as is.

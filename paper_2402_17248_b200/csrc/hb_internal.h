@@ -83,7 +83,7 @@ size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float
                           void* dst, long long* off_bytes, int* kpad, int* npad);
 bool hb_tc_supported(int prec, int n_linear, const int* widths, char* why, size_t why_len);
 // streamed-weights variant (hb_sur_tcs.cu): hidden width <= 512, equal hidden widths, weights through an smem ring
-bool hb_tcs_supported(int n_linear, const int* widths);
+bool hb_tcs_supported(int prec, int n_linear, const int* widths);   // prec: hb_prec (1 bf16, 2 f16, 3 tf32)
 size_t hb_tcs_pack_weights(int prec, int n_linear, const int* widths, const float* const* W,
                            void* dst, long long* off_bytes, int* kpad, int* npad);
 cudaError_t hb_launch_sur_tcs(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials,

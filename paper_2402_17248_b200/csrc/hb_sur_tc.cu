@@ -470,11 +470,12 @@ int choose_cg(int n_linear, const int* widths, TcPlan& pl) {
 
 // resident kernel if the weights fit in shared memory, else the streamed kernel (hb_sur_tcs.cu).
 // HB_TC_FORCE_STREAM=1 : test hook, runs shapes the resident kernel could take through the streamed one.
-bool use_stream(int n_linear, const int* widths) {
+bool use_stream(int prec, int n_linear, const int* widths) {
+    if (prec == 3) return hb_tcs_supported(prec, n_linear, widths);       // tf32 operands: streamed kernel only
     const char* force = getenv("HB_TC_FORCE_STREAM");
-    if (force && force[0] == '1' && hb_tcs_supported(n_linear, widths)) return true;
+    if (force && force[0] == '1' && hb_tcs_supported(prec, n_linear, widths)) return true;
     TcPlan pl;
-    return !choose_cg(n_linear, widths, pl) && hb_tcs_supported(n_linear, widths);
+    return !choose_cg(n_linear, widths, pl) && hb_tcs_supported(prec, n_linear, widths);
 }
 
 // Launch shape.  Small networks (CTA-pair plan <= 113 KB of shared memory, two accumulators <= 256 TMEM
@@ -501,12 +502,17 @@ extern "C" int hb_debug_tc_trace(long long* host, int count) {
 #endif
 
 bool hb_tc_supported(int prec, int n_linear, const int* widths, char* why, size_t why_len) {
+    if (prec == 3) {
+        if (hb_tcs_supported(prec, n_linear, widths)) return true;
+        snprintf(why, why_len, "HB_PREC_TF32 runs on the streamed kernel only: at least one hidden layer, equal hidden widths <= 256");
+        return false;
+    }
     if (prec != 1 && prec != 2) {
-        snprintf(why, why_len, "HB_PREC_TF32 has no kernel yet (use HB_PREC_BF16 or HB_PREC_F16)");
+        snprintf(why, why_len, "unknown precision %d", prec);
         return false;
     }
     TcPlan pl;
-    if (!choose_cg(n_linear, widths, pl) && !hb_tcs_supported(n_linear, widths)) {
+    if (!choose_cg(n_linear, widths, pl) && !hb_tcs_supported(prec, n_linear, widths)) {
         snprintf(why, why_len, "no tensor-core schedule for this shape: the weights do not fit resident in shared memory "
                                "and the streamed kernel needs equal hidden widths <= 512");
         return false;
@@ -520,7 +526,7 @@ bool hb_tc_supported(int prec, int n_linear, const int* widths, char* why, size_
 // the 16-byte chunk c of row r sits at chunk position c ^ (r mod 8)).
 size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float* const* W, void* dst,
                           long long* off_bytes, int* kpad, int* npad) {
-    if (use_stream(n_linear, widths)) return hb_tcs_pack_weights(prec, n_linear, widths, W, dst, off_bytes, kpad, npad);
+    if (use_stream(prec, n_linear, widths)) return hb_tcs_pack_weights(prec, n_linear, widths, W, dst, off_bytes, kpad, npad);
     int ksteps[HB_MAX_LINEAR];
     layer_geometry(n_linear, widths, kpad, npad, ksteps);
     size_t total = 0;
@@ -557,7 +563,7 @@ size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float
 
 cudaError_t hb_launch_sur_tc(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials, int* nblocks_out,
                              int sm_count, cudaStream_t s) {
-    if (use_stream(sd.n_linear, sd.widths)) return hb_launch_sur_tcs(p, n, sd, partials, nblocks_out, sm_count, s);
+    if (use_stream(sd.prec, sd.n_linear, sd.widths)) return hb_launch_sur_tcs(p, n, sd, partials, nblocks_out, sm_count, s);
     TcPlan pl;
     const TcShape sh = choose_shape(sd.n_linear, sd.widths, pl);
     // HB_TC_TWO_TILES=1 : opt-in to the two-tiles-in-flight kernel (hb_sur_tc2.cu) where its operand ring fits.

@@ -50,11 +50,15 @@ struct TcsPlan {
     int a_off, ring_off, a0_off, stage_off, bias_base, bar_off, red_off, total;
 };
 
-template <int ACT, bool F16>
+// EL: operand type  0 = bf16, 1 = f16 (kind::f16, 64 elements per 128-byte slab row, K = 16 per MMA),
+//                   2 = tf32 (kind::tf32, 32 elements per slab row, K = 8 per MMA, half the rate; width <= 256)
+template <int ACT, int EL>
 __global__ void __launch_bounds__(S_THREADS, 1)
 hb_sur_tcs_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, const __grid_constant__ TcsPlan pl,
                   double* __restrict__ partials) {
     constexpr int CG = 2;
+    constexpr bool F16 = EL == 1, T32 = EL == 2;
+    constexpr int A0B = T32 ? 2 * A0_BYTES : A0_BYTES;      // layer-0 operand buffer (K = 16 elements per row)
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     const uint32_t sbase = smem_u32(smem);
@@ -83,7 +87,7 @@ hb_sur_tcs_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
             mbar_init(bar(S_W_READY + s), CG);
             mbar_init(bar(S_A_FREE + s), 1);
         }
-        for (int j = 0; j < S_MAX_SLABS; ++j) mbar_init(bar(S_SLAB_FULL + j), 8 * CG);
+        for (int j = 0; j < S_MAX_SLABS; ++j) mbar_init(bar(S_SLAB_FULL + j), (T32 ? 4 : 8) * CG);
         mbar_init(bar(S_D_LAST), 1);
         mbar_init(bar(S_OUT_READ), 4 * CG);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -162,7 +166,7 @@ hb_sur_tcs_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
         // ===================================================== MMA issuer (leader CTA): warp-uniform walk of the
         // schedule, one elected lane issues
         if (rank == 0) {
-            const uint32_t fmt = F16 ? 0u : 1u;
+            const uint32_t fmt = T32 ? 2u : (F16 ? 0u : 1u);
             const uint32_t idesc_base = (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)((TILE_M * CG) >> 4) << 24);
             const uint32_t idesc_h = idesc_base | ((uint32_t)(pl.nh >> 3) << 17);
             const uint32_t idesc_last = idesc_base | ((uint32_t)(16 >> 3) << 17);
@@ -200,12 +204,24 @@ hb_sur_tcs_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
                 {
                     const uint32_t slot = wait_block();
                     if (issuer) {
-                        const uint64_t ad = make_desc_l0(sbase + pl.a0_off + (it & 1) * A0_BYTES);
+                        const uint32_t ab = sbase + pl.a0_off + (it & 1) * A0B;
                         const uint32_t wb = sbase + pl.ring_off + slot * S_BLOCK_BYTES;
-                        umma<CG, false>(d0, ad, make_desc_l0(wb), idesc_h);
-                        umma_commit<CG>(bar(S_D_FULL + 0));
-                        umma<CG, false>(d1, ad, make_desc_l0(wb + (uint32_t)(pl.nh >> 1) * 32u), idesc_h);
-                        umma_commit<CG>(bar(S_D_FULL + 1));
+                        if (T32) {      // K = 16 = two K = 8 MMAs; the second starts two core matrices (256 B) further
+                            const uint64_t ad = make_desc_l0_t32(ab);
+                            const uint64_t w0 = make_desc_l0_t32(wb), w1 = make_desc_l0_t32(wb + (uint32_t)(pl.nh >> 1) * 64u);
+                            umma<CG, false, true>(d0, ad, w0, idesc_h);
+                            umma<CG, true, true>(d0, ad + 16, w0 + 16, idesc_h);
+                            umma_commit<CG>(bar(S_D_FULL + 0));
+                            umma<CG, false, true>(d1, ad, w1, idesc_h);
+                            umma<CG, true, true>(d1, ad + 16, w1 + 16, idesc_h);
+                            umma_commit<CG>(bar(S_D_FULL + 1));
+                        } else {
+                            const uint64_t ad = make_desc_l0(ab);
+                            umma<CG, false>(d0, ad, make_desc_l0(wb), idesc_h);
+                            umma_commit<CG>(bar(S_D_FULL + 0));
+                            umma<CG, false>(d1, ad, make_desc_l0(wb + (uint32_t)(pl.nh >> 1) * 32u), idesc_h);
+                            umma_commit<CG>(bar(S_D_FULL + 1));
+                        }
                     }
                     release_block(slot);
                     __syncwarp();
@@ -223,11 +239,11 @@ hb_sur_tcs_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
                                 if (issuer) {
                                     const uint64_t ad = a_desc0 + (uint64_t)(s * (A_SLAB_BYTES >> 4));
                                     const uint64_t bd = make_desc(sbase + pl.ring_off + slot * S_BLOCK_BYTES);
-                                    if (s == 0) umma<CG, false>(d_tmem, ad, bd, idesc_h);
-                                    else umma<CG, true>(d_tmem, ad, bd, idesc_h);
-                                    umma<CG, true>(d_tmem, ad + 2, bd + 2, idesc_h);
-                                    umma<CG, true>(d_tmem, ad + 4, bd + 4, idesc_h);
-                                    umma<CG, true>(d_tmem, ad + 6, bd + 6, idesc_h);
+                                    if (s == 0) umma<CG, false, T32>(d_tmem, ad, bd, idesc_h);
+                                    else umma<CG, true, T32>(d_tmem, ad, bd, idesc_h);
+                                    umma<CG, true, T32>(d_tmem, ad + 2, bd + 2, idesc_h);
+                                    umma<CG, true, T32>(d_tmem, ad + 4, bd + 4, idesc_h);
+                                    umma<CG, true, T32>(d_tmem, ad + 6, bd + 6, idesc_h);
                                 }
                                 release_block(slot);
                                 // half 1 has read slab s: the epilogue of half 0 may overwrite it
@@ -249,11 +265,11 @@ hb_sur_tcs_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
                             if (issuer) {
                                 const uint64_t ad = a_desc0 + (uint64_t)(s * (A_SLAB_BYTES >> 4));
                                 const uint64_t bd = make_desc(sbase + pl.ring_off + slot * S_BLOCK_BYTES + s * 1024);
-                                if (s == 0) umma<CG, false>(d0, ad, bd, idesc_last);
-                                else umma<CG, true>(d0, ad, bd, idesc_last);
-                                umma<CG, true>(d0, ad + 2, bd + 2, idesc_last);
-                                umma<CG, true>(d0, ad + 4, bd + 4, idesc_last);
-                                umma<CG, true>(d0, ad + 6, bd + 6, idesc_last);
+                                if (s == 0) umma<CG, false, T32>(d0, ad, bd, idesc_last);
+                                else umma<CG, true, T32>(d0, ad, bd, idesc_last);
+                                umma<CG, true, T32>(d0, ad + 2, bd + 2, idesc_last);
+                                umma<CG, true, T32>(d0, ad + 4, bd + 4, idesc_last);
+                                umma<CG, true, T32>(d0, ad + 6, bd + 6, idesc_last);
                             }
                             __syncwarp();
                         }
@@ -294,11 +310,19 @@ hb_sur_tcs_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
 #pragma unroll
                 for (int j = 0; j < 6; ++j) c[j] = p.v[j][i];
             }
-            uint32_t q0[4], q1[4];
-            tc_make_a0_row<F16>(sd, valid, c, q0, q1);
-            const uint32_t dst = a0_row + buf * A0_BYTES;
-            sts128(dst, q0);
-            sts128(dst + 128, q1);
+            if (T32) {   // 8-row groups of 512 B: four K chunks (4 elements each) 128 B apart
+                uint32_t q[4][4];
+                tc_make_a0_row_t32(sd, valid, c, q);
+                const uint32_t dst = sbase + pl.a0_off + buf * A0B + (uint32_t)(row >> 3) * 512 + (uint32_t)(row & 7) * 16;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) sts128(dst + 128 * k, q[k]);
+            } else {
+                uint32_t q0[4], q1[4];
+                tc_make_a0_row<F16>(sd, valid, c, q0, q1);
+                const uint32_t dst = a0_row + buf * A0B;
+                sts128(dst, q0);
+                sts128(dst + 128, q1);
+            }
             fence_proxy_async();
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(bar(S_A0_FULL + buf), 0);
@@ -348,36 +372,39 @@ hb_sur_tcs_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
                 const float slope = sd.prelu[l];
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
-                    const uint32_t t0 = tlane + (uint32_t)(h * 256 + grp * 32);
                     mbar_wait<true>(bar(S_D_FULL + h), (ph_d >> h) & 1);
                     ph_d ^= 1u << h;
                     tc_fence_after();
-                    uint32_t ra[32], rb[32];
-                    tmem_ld32(t0, ra);
-                    for (int j = 0; j < NS2; j += 2) {
-                        tmem_ld_wait();
-                        if (j + 1 < NS2) tmem_ld32(t0 + 64 * (j + 1), rb);
-                        if (h == 0 && l > 0) {        // half 1's MMAs must have read slab j of the current operand
-                            mbar_wait<true>(bar(S_A_FREE + j), (ph_free >> j) & 1);
-                            ph_free ^= 1u << j;
+                    // this warp's 32-column chunks of the half: c = grp, grp + 2, ...  (16-bit operands: chunk c is
+                    // half of slab c / 2; tf32: chunk c is slab c)
+                    const int nchunk = pl.nh >> 5;
+                    auto finish = [&](const uint32_t (&r)[32], int c) {
+                        const int slab_in_half = T32 ? c : (c >> 1);
+                        const int slab = h * NS2 + slab_in_half;
+                        if (h == 0 && l > 0) {        // half 1's MMAs must have read this slab of the current operand
+                            if (T32 || grp == (c & 1)) {   // (every chunk of this warp lies in a different slab)
+                                mbar_wait<true>(bar(S_A_FREE + slab_in_half), (ph_free >> slab_in_half) & 1);
+                                ph_free ^= 1u << slab_in_half;
+                            }
                         }
-                        epi_store<32, ACT, F16>(ra, bl, h * pl.nh + 64 * j + grp * 32, slope, a_row, sw);
+                        if (T32) epi_store_t32<ACT>(r, bl + h * pl.nh + 32 * c, slope, a_row + slab * A_SLAB_BYTES, sw);
+                        else epi_store<32, ACT, F16>(r, bl, h * pl.nh + 32 * c, slope, a_row, sw);
                         fence_proxy_async();
                         tc_fence_before();
                         __syncwarp();
-                        if (lane == 0) mbar_arrive_cluster(bar(S_SLAB_FULL + h * NS2 + j), 0);
-                        if (j + 1 < NS2) {
+                        if (lane == 0) mbar_arrive_cluster(bar(S_SLAB_FULL + slab), 0);
+                    };
+                    uint32_t ra[32], rb[32];
+                    const uint32_t tb = tlane + (uint32_t)(h * 256);
+                    tmem_ld32(tb + 32 * grp, ra);
+                    for (int c = grp; c < nchunk; c += 4) {
+                        tmem_ld_wait();
+                        if (c + 2 < nchunk) tmem_ld32(tb + 32 * (c + 2), rb);
+                        finish(ra, c);
+                        if (c + 2 < nchunk) {
                             tmem_ld_wait();
-                            if (j + 2 < NS2) tmem_ld32(t0 + 64 * (j + 2), ra);
-                            if (h == 0 && l > 0) {
-                                mbar_wait<true>(bar(S_A_FREE + j + 1), (ph_free >> (j + 1)) & 1);
-                                ph_free ^= 1u << (j + 1);
-                            }
-                            epi_store<32, ACT, F16>(rb, bl, h * pl.nh + 64 * (j + 1) + grp * 32, slope, a_row, sw);
-                            fence_proxy_async();
-                            tc_fence_before();
-                            __syncwarp();
-                            if (lane == 0) mbar_arrive_cluster(bar(S_SLAB_FULL + h * NS2 + j + 1), 0);
+                            if (c + 4 < nchunk) tmem_ld32(tb + 32 * (c + 4), ra);
+                            finish(rb, c + 2);
                         }
                     }
                 }
@@ -397,7 +424,8 @@ hb_sur_tcs_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
 // ------------------------------------------------------------------------------- host: plan + packing
 int s_round_up(int v, int m) { return (v + m - 1) / m * m; }
 
-bool make_splan(int n_linear, const int* widths, TcsPlan& pl) {
+bool make_splan(int prec, int n_linear, const int* widths, TcsPlan& pl) {
+    const bool t32 = prec == 3;
     std::memset(&pl, 0, sizeof pl);
     if (n_linear < 2) return false;
     int npad = 0;
@@ -406,12 +434,12 @@ bool make_splan(int n_linear, const int* widths, TcsPlan& pl) {
         if (l == 0) npad = w;
         else if (w != npad) return false;                            // equal (padded) hidden widths only
     }
-    if (npad > 512) return false;
+    if (npad > (t32 ? 256 : 512)) return false;      // operand buffer: 8 slabs of 64 (16-bit) or 32 (tf32) inputs
     pl.n_linear = n_linear;
     pl.npad = npad;
-    pl.ns = npad / 64;
+    pl.ns = npad / (t32 ? 32 : 64);
     pl.nh = npad / 2;
-    pl.blk0_bytes = npad / 2 * 32;
+    pl.blk0_bytes = npad / 2 * (t32 ? 64 : 32);
     pl.hblk_bytes = pl.nh / 2 * 128;
     pl.last_bytes = pl.ns * 1024;
     pl.img_rank_bytes = (long long)pl.blk0_bytes + (long long)(n_linear - 2) * 2 * pl.ns * pl.hblk_bytes + pl.last_bytes;
@@ -426,7 +454,7 @@ bool make_splan(int n_linear, const int* widths, TcsPlan& pl) {
     pl.ring_off = off;
     off += S_RING * S_BLOCK_BYTES;
     pl.a0_off = off;
-    off += 2 * A0_BYTES;
+    off += 2 * (t32 ? 2 * A0_BYTES : A0_BYTES);
     pl.stage_off = off;
     off += IN_STAGES * STAGE_BYTES;
     pl.bias_base = off;
@@ -439,11 +467,11 @@ bool make_splan(int n_linear, const int* widths, TcsPlan& pl) {
     return (size_t)pl.total + 1024 <= SMEM_LIMIT;
 }
 
-template <int ACT, bool F16>
+template <int ACT, int EL>
 cudaError_t s_launch_one(const HbParticles& p, size_t n, const HbSurDev& sd, const TcsPlan& pl, double* partials, int grid,
                          cudaStream_t s) {
     const size_t smem = (size_t)pl.total + 1024;
-    cudaError_t e = cudaFuncSetAttribute(hb_sur_tcs_kernel<ACT, F16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(hb_sur_tcs_kernel<ACT, EL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(grid);
@@ -457,25 +485,25 @@ cudaError_t s_launch_one(const HbParticles& p, size_t n, const HbSurDev& sd, con
     at[0].val.clusterDim.z = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, hb_sur_tcs_kernel<ACT, F16>, p, n, sd, pl, partials);
+    return cudaLaunchKernelEx(&cfg, hb_sur_tcs_kernel<ACT, EL>, p, n, sd, pl, partials);
 }
 
-template <bool F16>
+template <int EL>
 cudaError_t s_launch_act(const HbParticles& p, size_t n, const HbSurDev& sd, const TcsPlan& pl, double* partials, int grid,
                          cudaStream_t s) {
     switch (sd.act) {
-    case 0: return s_launch_one<0, F16>(p, n, sd, pl, partials, grid, s);
-    case 1: return s_launch_one<1, F16>(p, n, sd, pl, partials, grid, s);
-    case 2: return s_launch_one<2, F16>(p, n, sd, pl, partials, grid, s);
-    default: return s_launch_one<3, F16>(p, n, sd, pl, partials, grid, s);
+    case 0: return s_launch_one<0, EL>(p, n, sd, pl, partials, grid, s);
+    case 1: return s_launch_one<1, EL>(p, n, sd, pl, partials, grid, s);
+    case 2: return s_launch_one<2, EL>(p, n, sd, pl, partials, grid, s);
+    default: return s_launch_one<3, EL>(p, n, sd, pl, partials, grid, s);
     }
 }
 
 }  // namespace
 
-bool hb_tcs_supported(int n_linear, const int* widths) {
+bool hb_tcs_supported(int prec, int n_linear, const int* widths) {
     TcsPlan pl;
-    return make_splan(n_linear, widths, pl);
+    return make_splan(prec, n_linear, widths, pl);
 }
 
 // Global image = [rank 0 block sequence | rank 1 block sequence]; a rank's sequence is what its weight producer
@@ -487,7 +515,10 @@ bool hb_tcs_supported(int n_linear, const int* widths) {
 size_t hb_tcs_pack_weights(int prec, int n_linear, const int* widths, const float* const* W, void* dst,
                            long long* off_bytes, int* kpad, int* npad) {
     TcsPlan pl;
-    if (!make_splan(n_linear, widths, pl)) return 0;
+    if (!make_splan(prec, n_linear, widths, pl)) return 0;
+    const bool t32 = prec == 3;
+    const int ks = t32 ? 32 : 64;                    // inputs per slab
+    const int esz = t32 ? 4 : 2;
     for (int l = 0; l < n_linear; ++l) {
         off_bytes[l] = 0;                                    // the kernel walks the block sequence itself
         npad[l] = l == n_linear - 1 ? 16 : pl.npad;
@@ -497,12 +528,21 @@ size_t hb_tcs_pack_weights(int prec, int n_linear, const int* widths, const floa
     if (!dst) return total;
     std::memset(dst, 0, total);
     unsigned char* base = static_cast<unsigned char*>(dst);
-    auto put = [&](size_t byte, float w) {
+    // element e of a 16-byte chunk starting at `chunk_byte`
+    auto put = [&](size_t chunk_byte, int e, float w) {
+        if (t32) {           // tf32: fp32 container, 10 explicit mantissa bits, round to nearest (ties away)
+            unsigned int u;
+            std::memcpy(&u, &w, 4);
+            u = (u + 0x1000u) & 0xffffe000u;
+            std::memcpy(base + chunk_byte + (size_t)e * 4, &u, 4);
+            return;
+        }
         unsigned short bits;
         if (prec == 2) { __half h = __float2half_rn(w); std::memcpy(&bits, &h, 2); }
         else { __nv_bfloat16 h = __float2bfloat16_rn(w); std::memcpy(&bits, &h, 2); }
-        std::memcpy(base + byte, &bits, 2);
+        std::memcpy(base + chunk_byte + (size_t)e * 2, &bits, 2);
     };
+    const int epc = 16 / esz;                        // elements per 16-byte chunk
     const int nh = pl.nh, nq = pl.nh / 2;
     for (int rank = 0; rank < 2; ++rank) {
         const size_t r0 = (size_t)rank * (size_t)pl.img_rank_bytes;
@@ -512,8 +552,9 @@ size_t hb_tcs_pack_weights(int prec, int n_linear, const int* widths, const floa
                 const int o = h * nh + rank * nq + i;
                 if (o >= widths[1]) continue;
                 const int row = h * nq + i;
+                // K = 16 no-swizzle: per 8-row group, K chunk c (epc elements) at c * 128 B
                 for (int k = 0; k < 12; ++k)
-                    put(r0 + (size_t)(row / 8) * 256 + (size_t)(k / 8) * 128 + (size_t)(row % 8) * 16 + (size_t)(k % 8) * 2,
+                    put(r0 + (size_t)(row / 8) * (size_t)(16 / epc * 128) + (size_t)(k / epc) * 128 + (size_t)(row % 8) * 16, k % epc,
                         W[0][(size_t)o * widths[0] + (k % 6)]);
             }
         // hidden layers
@@ -524,10 +565,10 @@ size_t hb_tcs_pack_weights(int prec, int n_linear, const int* widths, const floa
                     for (int i = 0; i < nq; ++i) {
                         const int o = h * nh + rank * nq + i;
                         if (o >= widths[l + 1]) continue;
-                        for (int kk = 0; kk < 64; ++kk) {
-                            const int k = s * 64 + kk;
+                        for (int kk = 0; kk < ks; ++kk) {
+                            const int k = s * ks + kk;
                             if (k >= widths[l]) break;
-                            put(b0 + (size_t)i * 128 + (size_t)(((kk / 8) ^ (i & 7)) << 4) + (size_t)(kk % 8) * 2,
+                            put(b0 + (size_t)i * 128 + (size_t)(((kk / epc) ^ (i & 7)) << 4), kk % epc,
                                 W[l][(size_t)o * widths[l] + k]);
                         }
                     }
@@ -540,8 +581,8 @@ size_t hb_tcs_pack_weights(int prec, int n_linear, const int* widths, const floa
                 const int o = rank * 8 + i;
                 if (o >= widths[l + 1]) continue;
                 for (int k = 0; k < widths[l]; ++k) {
-                    const int s = k / 64, kk = k % 64;
-                    put(b0 + (size_t)s * 1024 + (size_t)i * 128 + (size_t)(((kk / 8) ^ (i & 7)) << 4) + (size_t)(kk % 8) * 2,
+                    const int s = k / ks, kk = k % ks;
+                    put(b0 + (size_t)s * 1024 + (size_t)i * 128 + (size_t)(((kk / epc) ^ (i & 7)) << 4), kk % epc,
                         W[l][(size_t)o * widths[l] + k]);
                 }
             }
@@ -553,7 +594,7 @@ size_t hb_tcs_pack_weights(int prec, int n_linear, const int* widths, const floa
 cudaError_t hb_launch_sur_tcs(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials, int* nblocks_out,
                               int sm_count, cudaStream_t s) {
     TcsPlan pl;
-    if (!make_splan(sd.n_linear, sd.widths, pl)) return cudaErrorNotSupported;
+    if (!make_splan(sd.prec, sd.n_linear, sd.widths, pl)) return cudaErrorNotSupported;
     const size_t ntiles = (n + TILE_M - 1) / TILE_M;
     const size_t ngroups = (ntiles + 1) / 2;
     size_t clusters = (size_t)(sm_count / 2);
@@ -561,5 +602,6 @@ cudaError_t hb_launch_sur_tcs(const HbParticles& p, size_t n, const HbSurDev& sd
     if (clusters < 1) clusters = 1;
     const int grid = (int)clusters * 2;
     if (nblocks_out) *nblocks_out = grid;
-    return sd.prec == 2 ? s_launch_act<true>(p, n, sd, pl, partials, grid, s) : s_launch_act<false>(p, n, sd, pl, partials, grid, s);
+    if (sd.prec == 3) return s_launch_act<2>(p, n, sd, pl, partials, grid, s);
+    return sd.prec == 2 ? s_launch_act<1>(p, n, sd, pl, partials, grid, s) : s_launch_act<0>(p, n, sd, pl, partials, grid, s);
 }

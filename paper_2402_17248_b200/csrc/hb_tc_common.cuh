@@ -117,16 +117,24 @@ __device__ __forceinline__ void tmem_dealloc(uint32_t addr, uint32_t cols) {
     if (CG == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(addr), "r"(cols) : "memory");
     else asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(addr), "r"(cols) : "memory");
 }
-// D[tmem] (+)= A[smem desc] * B[smem desc]
-template <int CG, bool ACC>
+// D[tmem] (+)= A[smem desc] * B[smem desc];  T32: kind::tf32 (32-bit operands, K = 8), else kind::f16 (K = 16)
+template <int CG, bool ACC, bool T32 = false>
 __device__ __forceinline__ void umma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc) {
-    if (CG == 1)
+    if (CG == 1 && !T32)
         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
                      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
                      ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "n"(ACC ? 1 : 0) : "memory");
-    else
+    else if (!T32)
         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
                      "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+                     ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "n"(ACC ? 1 : 0) : "memory");
+    else if (CG == 1)
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                     "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
+                     ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "n"(ACC ? 1 : 0) : "memory");
+    else
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                     "tcgen05.mma.cta_group::2.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
                      ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "n"(ACC ? 1 : 0) : "memory");
 }
 __device__ __forceinline__ bool elect_one() {
@@ -305,6 +313,52 @@ __device__ __forceinline__ void epi_store_slab(const uint32_t (&r)[CW], const fl
     for (int k = 0; k < CW / 8; ++k)
         asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(slab_row + (((ch0 + k) ^ sw) << 4)),
                      "r"(q[4 * k]), "r"(q[4 * k + 1]), "r"(q[4 * k + 2]), "r"(q[4 * k + 3]) : "memory");
+}
+
+// ---- tf32 operands (HB_PREC_TF32): 32-bit elements, 32 per 128-byte slab row, K = 8 per MMA
+__device__ __forceinline__ float to_tf32(float v) {           // round to nearest (ties away), low 13 bits zero
+    uint32_t d;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(d) : "f"(v));
+    return __uint_as_float(d);
+}
+// K-major, no swizzle, 32-bit elements, K = 16 (layer 0): core matrices of 8 rows x 16 bytes (4 elements); the four
+// K chunks of an 8-row group sit 128 B apart (LBO), 8-row groups 512 B apart (SBO).
+__device__ __forceinline__ uint64_t make_desc_l0_t32(uint32_t saddr) {
+    uint64_t d = (uint64_t)((saddr & 0x3FFFFu) >> 4);
+    d |= (uint64_t)(128 >> 4) << 16;
+    d |= (uint64_t)(512 >> 4) << 32;
+    d |= (uint64_t)1 << 46;
+    return d;
+}
+// One hidden-layer epilogue step of one warp for tf32: 32 accumulator columns -> bias, sigma, tf32, one full
+// 128-byte slab row (eight 16-byte chunks, swizzled).
+template <int ACT>
+__device__ __forceinline__ void epi_store_t32(const uint32_t (&r)[32], const float* __restrict__ bl, float slope,
+                                              uint32_t slab_row, uint32_t sw) {
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const float4 b4 = *reinterpret_cast<const float4*>(bl + 4 * k);
+        float v[4] = {__uint_as_float(r[4 * k]) + b4.x, __uint_as_float(r[4 * k + 1]) + b4.y,
+                      __uint_as_float(r[4 * k + 2]) + b4.z, __uint_as_float(r[4 * k + 3]) + b4.w};
+        uint32_t q[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) q[e] = __float_as_uint(to_tf32(hb_activate<ACT, true>(v[e], slope)));
+        asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(slab_row + ((((uint32_t)k) ^ sw) << 4)),
+                     "r"(q[0]), "r"(q[1]), "r"(q[2]), "r"(q[3]) : "memory");
+    }
+}
+// a4 for tf32: the K = 16 layer-0 operand row  hi0..hi5, lo0..lo5, 0, 0, 0, 0  as four 16-byte chunks
+__device__ __forceinline__ void tc_make_a0_row_t32(const HbSurDev& sd, bool valid, const float (&c)[6], uint32_t (&q)[4][4]) {
+    float nin[6] = {0, 0, 0, 0, 0, 0};
+    if (valid) hb_sur_prologue(sd, c[0], c[1], c[2], c[3], c[4], c[5], nin);
+    float e[16];
+#pragma unroll
+    for (int j = 0; j < 6; ++j) { e[j] = to_tf32(nin[j]); e[6 + j] = to_tf32(nin[j] - e[j]); }
+    e[12] = e[13] = e[14] = e[15] = 0.0f;
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) q[k][i] = __float_as_uint(e[4 * k + i]);
 }
 
 }  // namespace

@@ -219,3 +219,44 @@ def test_tc2_shapes(hb, prec, act, widths, n, monkeypatch):
     assert e.max() <= TOL[prec]
     own = oracle.moments(np.ascontiguousarray(got))
     assert np.allclose(rec[0][:6], own[:6], rtol=1e-9, atol=1e-16)
+
+
+# ------------------------------------------------------------------ HB_PREC_TF32 (kind::tf32 on the streamed kernel)
+def test_tf32_bringup_identity_net(hb):
+    """identity weights, tf32 operands: output = input rounded to 10 explicit mantissa bits (layouts, descriptors)"""
+    x = wl.gaussian_bunch(3000, 3, sigma=np.ones(6))
+    got, _ = gpu_push(hb, wl.lattice([identity_net(128, "tf32")]), x)
+    assert np.all(np.isfinite(got))
+    assert np.max(np.abs(got - x) / np.maximum(np.abs(x), 1e-3)) <= 1.01 * 2.0 ** -11
+
+
+@pytest.mark.parametrize("act,widths,n", [("relu", [6, 256, 256, 256, 6], 20_000), ("tanh", [6, 128, 128, 128, 6], 20_000),
+                                          ("prelu", [6, 100, 100, 6], 257), ("tanh", [6, 192, 6], 1),
+                                          ("identity", [6, 64, 64, 64, 64, 64, 6], 40_001)])
+def test_tf32_shapes(hb, act, widths, n):
+    init = "he" if act in ("relu", "prelu") else "xavier"
+    W, b = wl.make_mlp(widths, init, 59, len(widths))
+    rng = np.random.default_rng(9)
+    a = rng.uniform(0.05, 0.3, len(widths) - 2).astype(np.float32) if act == "prelu" else None
+    x = wl.correlated_bunch(max(n, 8), 44)[:, :n].copy()
+    full = wl.correlated_bunch(max(n, 8), 44).astype(np.float64)
+    sur = wl.surrogate(widths, W, b, act, full.mean(axis=1), full.std(axis=1), rng.normal(size=6),
+                       rng.uniform(0.5, 2.0, 6), prelu_a=a, prec="tf32")
+    desc = wl.lattice([sur, wl.monitor()])
+    ref, _ = oracle.push(desc, x)
+    got, rec = gpu_push(hb, desc, x, moments=True)
+    scale = np.maximum(ref.std(axis=1), np.abs(sur["out_std"]) * 0.2) if n > 1 else np.abs(sur["out_std"])
+    e = np.max(np.abs(got - ref), axis=1) / scale
+    print("tf32 shape", widths, act, "max err/std", e.max())
+    assert np.all(np.isfinite(got))
+    assert e.max() <= 2e-2
+    own = oracle.moments(np.ascontiguousarray(got))
+    assert np.allclose(rec[0][:6], own[:6], rtol=1e-9, atol=1e-16)
+
+
+def test_tf32_unsupported_shapes_fail_loudly(hb):
+    """tf32 needs the streamed kernel's shape (equal hidden widths <= 256); anything else is an error, never a fallback"""
+    W, b = wl.make_mlp([6, 512, 512, 6], "xavier", 60, 3)
+    z, o = np.zeros(6), np.ones(6)
+    with pytest.raises(Exception):
+        hb.Lattice.from_description(wl.lattice([wl.surrogate([6, 512, 512, 6], W, b, "tanh", z, o, z, o, prec="tf32")]), device=0)
