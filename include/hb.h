@@ -165,6 +165,13 @@ const char *hb_status_string(hb_status s);
 const char *hb_last_error(void); /* thread-local message of the last failing call on this thread */
 const char *hb_version(void);
 
+/* Which kernel a surrogate stage of this shape runs on (host-only query, no device needed; the same decision
+ * hb_lattice_finalize takes): "fp32-ffma", "tcgen05-resident" (16-bit weights resident in shared memory),
+ * "tcgen05-streamed" (weights streamed from L2; also every HB_PREC_TF32 stage), or NULL when the shape has no
+ * schedule (hb_lattice_finalize would return HB_ERR_UNSUPPORTED; reason in hb_last_error()).
+ * widths: n_linear + 1 entries, 6, H_1, ..., 6.  The returned string is static. */
+const char *hb_surrogate_kernel(hb_prec prec, int n_linear, const int *widths);
+
 #ifdef __cplusplus
 }
 #endif

@@ -22,7 +22,7 @@ EXPORTED_SYMBOLS = [
     "hb_lattice_finalize", "hb_lattice_num_monitors", "hb_lattice_num_launches", "hb_lattice_ref_bg_out",
     "hb_push", "hb_push_moments", "hb_moments", "hb_moments_scratch_bytes", "hb_lattice_destroy",
     "hb_lattice_enable_timing", "hb_lattice_get_timing",
-    "hb_status_string", "hb_last_error", "hb_version",
+    "hb_status_string", "hb_last_error", "hb_version", "hb_surrogate_kernel",
 ]
 
 
@@ -87,6 +87,8 @@ def lib():
     L.hb_status_string.argtypes = [c_int]
     L.hb_last_error.restype = c_char_p
     L.hb_version.restype = c_char_p
+    L.hb_surrogate_kernel.restype = c_char_p
+    L.hb_surrogate_kernel.argtypes = [c_int, c_int, POINTER(c_int)]
     for name in EXPORTED_SYMBOLS:
         getattr(L, name)
     _lib = L
@@ -104,6 +106,13 @@ def hb_last_error() -> str:
 
 def hb_version() -> str:
     return lib().hb_version().decode()
+
+
+def hb_surrogate_kernel(prec, widths):
+    """kernel a stage of this shape runs on ("fp32-ffma" | "tcgen05-resident" | "tcgen05-streamed"), None if unsupported"""
+    w = (c_int * len(widths))(*[int(v) for v in widths])
+    r = lib().hb_surrogate_kernel(PRECS[prec] if isinstance(prec, str) else int(prec), len(widths) - 1, w)
+    return None if r is None else r.decode()
 
 
 def _check(status, where):

@@ -218,6 +218,17 @@ const char* hb_status_string(hb_status s) {
 const char* hb_last_error(void) { return g_err.c_str(); }
 const char* hb_version(void) { return "hb 0.1 (sm_100a)"; }
 
+const char* hb_surrogate_kernel(hb_prec prec, int n_linear, const int* widths) {
+    if (!widths || n_linear < 1 || n_linear > HB_MAX_LINEAR) { fail(HB_ERR_INVALID_ARG, "n_linear / widths"); return nullptr; }
+    if (widths[0] != 6 || widths[n_linear] != 6) { fail(HB_ERR_INVALID_ARG, "widths[0] and widths[last] must be 6"); return nullptr; }
+    for (int l = 1; l < n_linear; ++l)
+        if (widths[l] < 1 || widths[l] > HB_MAX_WIDTH) { fail(HB_ERR_INVALID_ARG, "hidden width out of range"); return nullptr; }
+    if (prec == HB_PREC_FP32) return "fp32-ffma";
+    char why[256];
+    if (!hb_tc_supported((int)prec, n_linear, widths, why, sizeof why)) { fail(HB_ERR_UNSUPPORTED, "tensor-core surrogate: %s", why); return nullptr; }
+    return hb_tc_kernel_kind((int)prec, n_linear, widths) == 2 ? "tcgen05-streamed" : "tcgen05-resident";
+}
+
 hb_status hb_lattice_create(double kin, double rest, hb_lattice** out) {
     if (!out) return fail(HB_ERR_INVALID_ARG, "out is NULL");
     *out = nullptr;
@@ -399,6 +410,7 @@ static hb_status build_surrogate(hb_lattice* lat, const SurHost& s, double bg_in
         if (st != HB_OK) return st;
         sd.wtc = dw;
         sd.btc = (const float*)db;
+        sd.tc_kind = hb_tc_kernel_kind(s.prec, s.n_linear, s.widths.data());   // the image above is this kernel's
         seg.tc = true;
     }
     return HB_OK;

@@ -56,6 +56,7 @@ struct HbSurDev {             // passed by value to the surrogate kernels
     int btc_off[HB_MAX_LINEAR];
     int kpad[HB_MAX_LINEAR];  // padded fan-in  (multiple of 64 elements; layer 0: 64)
     int npadtc[HB_MAX_LINEAR];// padded fan-out (multiple of 16; hidden: multiple of 64)
+    int tc_kind;              // which tensor-core kernel the image was packed for (hb_tc_kernel_kind, fixed at finalize)
 };
 
 struct HbParticles {
@@ -92,3 +93,5 @@ cudaError_t hb_launch_sur_tcs(const HbParticles& p, size_t n, const HbSurDev& sd
 bool hb_tc2_supported(int n_linear, const int* widths);
 cudaError_t hb_launch_sur_tc2(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials,
                               int* nblocks_out, int sm_count, cudaStream_t s);
+// 0: no tensor-core schedule for this shape, 1: weights resident (hb_sur_tc.cu), 2: weights streamed (hb_sur_tcs.cu)
+int hb_tc_kernel_kind(int prec, int n_linear, const int* widths);

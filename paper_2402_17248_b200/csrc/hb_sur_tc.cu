@@ -501,6 +501,14 @@ extern "C" int hb_debug_tc_trace(long long* host, int count) {
 }
 #endif
 
+int hb_tc_kernel_kind(int prec, int n_linear, const int* widths) {
+    if (prec < 1 || prec > 3) return 0;
+    if (use_stream(prec, n_linear, widths)) return 2;
+    if (prec == 3) return 0;
+    TcPlan pl;
+    return choose_cg(n_linear, widths, pl) ? 1 : 0;
+}
+
 bool hb_tc_supported(int prec, int n_linear, const int* widths, char* why, size_t why_len) {
     if (prec == 3) {
         if (hb_tcs_supported(prec, n_linear, widths)) return true;
@@ -563,7 +571,7 @@ size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float
 
 cudaError_t hb_launch_sur_tc(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials, int* nblocks_out,
                              int sm_count, cudaStream_t s) {
-    if (use_stream(sd.prec, sd.n_linear, sd.widths)) return hb_launch_sur_tcs(p, n, sd, partials, nblocks_out, sm_count, s);
+    if (sd.tc_kind == 2) return hb_launch_sur_tcs(p, n, sd, partials, nblocks_out, sm_count, s);
     TcPlan pl;
     const TcShape sh = choose_shape(sd.n_linear, sd.widths, pl);
     // HB_TC_TWO_TILES=1 : opt-in to the two-tiles-in-flight kernel (hb_sur_tc2.cu) where its operand ring fits.

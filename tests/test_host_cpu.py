@@ -88,3 +88,25 @@ def test_shard_ranges_cover_everything():
             assert r[0][0] == 0 and r[-1][1] == n
             assert all(a[1] == b[0] for a, b in zip(r[:-1], r[1:]))
             assert max(b - a for a, b in r) - min(b - a for a, b in r) <= 1
+
+
+def test_surrogate_kernel_dispatch_is_a_host_decision(hb, monkeypatch):
+    """which kernel a shape runs on (the decision hb_lattice_finalize takes) -- BASELINE.json's five configs and the
+    edges of each kernel's envelope; unsupported shapes are an error with a reason, never a fallback"""
+    for k in ("HB_TC_FORCE_STREAM", "HB_TC_FORCE_CG", "HB_TC_OCC2", "HB_TC_TWO_TILES"):
+        monkeypatch.delenv(k, raising=False)
+    K = hb.hb_surrogate_kernel
+    assert K("fp32", [6, 64, 64, 6]) == "fp32-ffma"                       # C1 as specified
+    assert K("bf16", [6, 64, 64, 6]) == "tcgen05-resident"
+    assert K("bf16", [6, 256, 256, 256, 6]) == "tcgen05-resident"         # C3: 272 KB of weights over a CTA pair
+    assert K("f16", [6, 128, 128, 128, 6]) == "tcgen05-resident"          # C4
+    assert K("bf16", [6, 512, 512, 512, 512, 6]) == "tcgen05-streamed"    # C5: 1.55 MB of weights
+    assert K("bf16", [6] + [256] * 8 + [6]) == "tcgen05-streamed"         # too deep to stay resident
+    assert K("bf16", [6, 6]) == "tcgen05-resident"                        # no hidden layer
+    assert K("tf32", [6, 256, 256, 256, 6]) == "tcgen05-streamed"
+    assert K("tf32", [6, 512, 512, 6]) is None and "TF32" in hb.hb_last_error()
+    assert K("bf16", [6, 900, 900, 900, 900, 900, 6]) is None             # NEXT-1 widths: no schedule yet
+    assert K("bf16", [6, 512, 300, 512, 6]) is None                       # streamed kernel: equal widths only
+    assert K("bf16", [6, 1025, 6]) is None and K("bf16", [5, 8, 6]) is None
+    monkeypatch.setenv("HB_TC_FORCE_STREAM", "1")
+    assert K("bf16", [6, 256, 256, 256, 6]) == "tcgen05-streamed"
