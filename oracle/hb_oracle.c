@@ -107,6 +107,22 @@ void orc_quad(double *x, double *px, double *y, double *py, double *t, double *p
     }
 }
 
+/* R3b (NEXT-2): thick axisymmetric linear (plasma) lens, length L, strength k [m^-2]:
+ * x'' = -k x and y'' = -k y, i.e. k > 0 focuses BOTH planes (k < 0 defocuses both, k = 0 is a drift);
+ * longitudinally a drift.  The paper sets k from the beam moments with an expression of its ref. [31] that it
+ * does not print: here k is an input. */
+void orc_plens(double *x, double *px, double *y, double *py, double *t, double *pt,
+               long n, double L, double k, double bg0)
+{
+    long i;
+#pragma omp parallel for schedule(static)
+    for (i = 0; i < n; ++i) {
+        quad_plane(&x[i], &px[i], L, k);
+        quad_plane(&y[i], &py[i], L, k);
+        t[i] = t[i] + L * pt[i] / (bg0 * bg0);
+    }
+}
+
 /* R4: sector bend, arc length L, bend angle theta (signed), rho = L/theta. */
 void orc_sbend(double *x, double *px, double *y, double *py, double *t, double *pt,
                long n, double L, double theta, double bg0)

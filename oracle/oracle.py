@@ -78,6 +78,11 @@ def quad(c, L, k, bg0):
                    ctypes.c_double(bg0))
 
 
+def plens(c, L, k, bg0):
+    lib().orc_plens(*_rows(c), ctypes.c_long(c.shape[1]), ctypes.c_double(L), ctypes.c_double(k),
+                    ctypes.c_double(bg0))
+
+
 def sbend(c, L, theta, bg0):
     lib().orc_sbend(*_rows(c), ctypes.c_long(c.shape[1]), ctypes.c_double(L), ctypes.c_double(theta),
                     ctypes.c_double(bg0))
@@ -151,6 +156,8 @@ class Tracker:
             drift(c, el["L"], self.bg)
         elif kind == "quad":
             quad(c, el["L"], el["k"], self.bg)
+        elif kind == "plens":
+            plens(c, el["L"], el["k"], self.bg)
         elif kind == "sbend":
             sbend(c, el["L"], el["theta"], self.bg)
         elif kind == "monitor":

@@ -486,3 +486,57 @@ def test_config4_physical_no_nans():
     lat, x = wl.config4(n=2048)
     c, rec = oracle.push(lat, x)
     assert np.all(np.isfinite(c)) and rec.shape == (4, 27) and np.all(np.isfinite(rec))
+
+
+# ------------------------------------------------------------------------------ R3b plasma lens (NEXT-2)
+@pytest.mark.parametrize("k", [3.0, -3.0, 250.0])
+def test_plens_matrix_closed_form(k):
+    """x'' = -k x in BOTH planes: the textbook harmonic-oscillator transfer matrix, twice; t as in a drift"""
+    L = 0.05
+    M = jacobian([wl.plens(L, k)])
+    w = math.sqrt(abs(k))
+    foc = np.array([[math.cos(w * L), math.sin(w * L) / w], [-w * math.sin(w * L), math.cos(w * L)]])
+    dfc = np.array([[math.cosh(w * L), math.sinh(w * L) / w], [w * math.sinh(w * L), math.cosh(w * L)]])
+    E = np.eye(6)
+    E[0:2, 0:2] = E[2:4, 2:4] = foc if k > 0 else dfc
+    E[4, 5] = L / BG0 ** 2
+    assert np.allclose(M, E, rtol=0, atol=1e-14)
+    assert np.max(np.abs(M.T @ S6 @ M - S6)) < 1e-13 * max(1.0, np.max(np.abs(M)) ** 2)
+
+
+def test_plens_is_a_quad_in_x_and_the_opposite_quad_in_y():
+    """cross pin against the (separately pinned) quadrupole: lens(k) = quad(+k) in x = quad(-k) in y"""
+    L, k = 0.07, 11.0
+    P, Qp, Qm = jacobian([wl.plens(L, k)]), jacobian([wl.quad(L, k)]), jacobian([wl.quad(L, -k)])
+    assert np.array_equal(P[0:2, 0:2], Qp[0:2, 0:2]) and np.array_equal(P[2:4, 2:4], Qm[2:4, 2:4])
+    assert np.array_equal(P[4:6, :], Qp[4:6, :])
+    assert P[1, 0] < 0 and P[3, 2] < 0                       # focuses both planes for k > 0
+
+
+def test_plens_limits_inverse_and_thin_lens():
+    assert np.array_equal(jacobian([wl.plens(0.3, 0.0)]), jacobian([wl.drift(0.3)]))
+    assert np.allclose(jacobian([wl.plens(0.02, 9.0), wl.plens(-0.02, 9.0)]), np.eye(6), atol=1e-15)
+    # thin-lens limit: L -> 0 at fixed integrated strength kL = 1/f: kick px -= x/f, no displacement
+    f, L = 2.0, 1e-7
+    M = jacobian([wl.plens(L, 1.0 / (f * L))])
+    assert abs(M[1, 0] + 1.0 / f) < 1e-6 and abs(M[0, 0] - 1.0) < 1e-6 and abs(M[0, 1]) < 1e-6
+    # a quarter betatron period images (x, px) -> (px / w, -w x)
+    w = 5.0
+    M = jacobian([wl.plens(math.pi / (2 * w), w * w)])
+    assert np.allclose(M[0:2, 0:2], [[0.0, 1.0 / w], [-w, 0.0]], atol=1e-15)
+
+
+def test_plens_8_particles_brute_force_and_axisymmetry():
+    c = rand_coords(8, 5)
+    L, k = 0.05, 40.0
+    ref = jacobian([wl.plens(L, k)]) @ c
+    got = c.copy()
+    oracle.Tracker(LAT).apply(wl.plens(L, k), got)
+    assert np.allclose(got, ref, rtol=1e-13, atol=1e-20)
+    # axisymmetric: rotating the transverse plane by any angle commutes with the lens (not true for a quadrupole)
+    a = 0.7
+    R = np.eye(6)
+    R[np.ix_([0, 2], [0, 2])] = [[math.cos(a), -math.sin(a)], [math.sin(a), math.cos(a)]]
+    R[np.ix_([1, 3], [1, 3])] = [[math.cos(a), -math.sin(a)], [math.sin(a), math.cos(a)]]
+    P, Q = jacobian([wl.plens(L, k)]), jacobian([wl.quad(L, k)])
+    assert np.allclose(R @ P, P @ R, atol=1e-14) and not np.allclose(R @ Q, Q @ R, atol=1e-3)
