@@ -44,8 +44,11 @@ typedef enum {
 } hb_status;
 
 /* Conventional elements (formulas R2-R4).  MONITOR is the identity map that emits one
- * 27-double moment record (R10) and splits runs (R5, G17). */
-typedef enum { HB_ELEM_DRIFT = 0, HB_ELEM_QUAD = 1, HB_ELEM_SBEND = 2, HB_ELEM_MONITOR = 3 } hb_elem_kind;
+ * 27-double moment record (R10) and splits runs (R5, G17).  PLENS: thick axisymmetric linear (plasma) lens
+ * (R3b): x'' = -k x and y'' = -k y, k > 0 focuses both planes; the paper sets k from the
+ * moments of the previous monitor with an expression it does not print -- here the caller supplies k
+ * (read the record, build the next lattice). */
+typedef enum { HB_ELEM_DRIFT = 0, HB_ELEM_QUAD = 1, HB_ELEM_SBEND = 2, HB_ELEM_MONITOR = 3, HB_ELEM_PLENS = 5 } hb_elem_kind;
 
 /* Activation sigma of Eq. 3: identity; ReLU Eq. 1; PReLU Eq. 2, one learned
  * slope per activation layer (G9); tanh (the "sigmoidal function" of P:90; BASELINE configs 1,4,5). */
@@ -97,7 +100,8 @@ hb_status hb_lattice_create(double ref_kinetic_energy_MeV, double rest_energy_Me
 
 /* Append a conventional element.  length_m: DRIFT any finite value (negative allowed: the
  * drift(L) o drift(-L) identity test needs it); QUAD, SBEND >= 0; MONITOR ignored.
- * param: QUAD k [1/m^2] (k > 0 focuses x, R3); SBEND bend angle [rad], signed (R4); else ignored.
+ * param: QUAD k [1/m^2] (k > 0 focuses x, R3); PLENS k [1/m^2] (k > 0 focuses x and y, R3b); SBEND bend angle
+ * [rad], signed (R4); else ignored.
  * Errors: finalized lattice -> STATE; non-finite or negative QUAD/SBEND length -> INVALID_ARG. */
 hb_status hb_lattice_add_element(hb_lattice *lat, hb_elem_kind kind, double length_m, double param);
 

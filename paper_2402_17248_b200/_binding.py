@@ -11,7 +11,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libhb.so")
 
-ELEM_KINDS = {"drift": 0, "quad": 1, "sbend": 2, "monitor": 3}
+ELEM_KINDS = {"drift": 0, "quad": 1, "sbend": 2, "monitor": 3, "plens": 5}
 ACTS = {"identity": 0, "relu": 1, "prelu": 2, "tanh": 3}
 PRECS = {"fp32": 0, "bf16": 1, "f16": 2, "tf32": 3}
 COORDS = {"s": 0, "t": 1}
@@ -279,8 +279,8 @@ class Lattice:
             k = el["kind"]
             if k == "drift":
                 lat.add_element("drift", el["L"])
-            elif k == "quad":
-                lat.add_element("quad", el["L"], el["k"])
+            elif k in ("quad", "plens"):
+                lat.add_element(k, el["L"], el["k"])
             elif k == "sbend":
                 lat.add_element("sbend", el["L"], el["theta"])
             elif k == "monitor":

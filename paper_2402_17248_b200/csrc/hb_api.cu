@@ -96,7 +96,7 @@ Mat6 elem_matrix(const Elem& e, double bg) {
     const double r56 = L / (bg * bg);
     if (e.kind == HB_ELEM_DRIFT) {
         M.m[0][1] = L; M.m[2][3] = L; M.m[4][5] = r56;
-    } else if (e.kind == HB_ELEM_QUAD) {
+    } else if (e.kind == HB_ELEM_QUAD || e.kind == HB_ELEM_PLENS) {
         const double k = e.param, w = std::sqrt(std::fabs(k)), ph = w * L;
         // focusing plane: [cos, sin/w; -w sin, cos]; defocusing: [cosh, sinh/w; w sinh, cosh]
         double f[4], d[4];
@@ -105,7 +105,7 @@ Mat6 elem_matrix(const Elem& e, double bg) {
         d[1] = ph < 1e-6 ? L * (1.0 + ph * ph / 6.0) : std::sinh(ph) / w;
         d[2] = w * std::sinh(ph); d[3] = d[0];
         const double* X = k >= 0 ? f : d;
-        const double* Y = k >= 0 ? d : f;
+        const double* Y = e.kind == HB_ELEM_PLENS ? X : (k >= 0 ? d : f);     // lens: same sign in both planes (R3b)
         M.m[0][0] = X[0]; M.m[0][1] = X[1]; M.m[1][0] = X[2]; M.m[1][1] = X[3];
         M.m[2][2] = Y[0]; M.m[2][3] = Y[1]; M.m[3][2] = Y[2]; M.m[3][3] = Y[3];
         M.m[4][5] = r56;
@@ -130,10 +130,10 @@ HbSeqElem seq_elem(const Elem& e, double bg) {
     const Mat6 M = elem_matrix(e, bg);
     HbSeqElem s;
     std::memset(&s, 0, sizeof s);
-    s.kind = e.kind;
+    s.kind = e.kind == HB_ELEM_PLENS ? (int)HB_ELEM_QUAD : e.kind;   // the device applies a lens as two 2x2 planes + t
     if (e.kind == HB_ELEM_DRIFT) {
         s.a[0] = e.L; s.a[1] = M.m[4][5];
-    } else if (e.kind == HB_ELEM_QUAD) {
+    } else if (e.kind == HB_ELEM_QUAD || e.kind == HB_ELEM_PLENS) {
         s.a[0] = M.m[0][0]; s.a[1] = M.m[0][1]; s.a[2] = M.m[1][0]; s.a[3] = M.m[1][1];
         s.a[4] = M.m[2][2]; s.a[5] = M.m[2][3]; s.a[6] = M.m[3][2]; s.a[7] = M.m[3][3];
         s.a[8] = M.m[4][5];
@@ -247,12 +247,13 @@ hb_status hb_lattice_create(double kin, double rest, hb_lattice** out) {
 hb_status hb_lattice_add_element(hb_lattice* lat, hb_elem_kind kind, double L, double param) {
     if (!lat) return fail(HB_ERR_INVALID_ARG, "lattice is NULL");
     if (lat->finalized) return fail(HB_ERR_STATE, "lattice already finalized");
-    if ((int)kind < 0 || (int)kind > HB_ELEM_MONITOR) return fail(HB_ERR_INVALID_ARG, "unknown element kind %d", (int)kind);
+    if (((int)kind < 0 || (int)kind > HB_ELEM_MONITOR) && kind != HB_ELEM_PLENS)
+        return fail(HB_ERR_INVALID_ARG, "unknown element kind %d", (int)kind);
     Elem e{(int)kind, 0.0, 0.0, -1};
     if (kind != HB_ELEM_MONITOR) {
         if (!std::isfinite(L)) return fail(HB_ERR_INVALID_ARG, "length must be finite");
         if (kind != HB_ELEM_DRIFT && (!std::isfinite(param) || L < 0.0))
-            return fail(HB_ERR_INVALID_ARG, "quad/sbend need a finite parameter and length >= 0");
+            return fail(HB_ERR_INVALID_ARG, "quad/plens/sbend need a finite parameter and length >= 0");
         e.L = L;
         e.param = kind == HB_ELEM_DRIFT ? 0.0 : param;
     }
@@ -465,7 +466,7 @@ hb_status hb_lattice_finalize(hb_lattice* lat, int device) {
             s.monitor = -1;
             s.seq_off = (int)seq.size();
             Mat6 M = mat_identity();
-            while (i < lat->elems.size() && lat->elems[i].kind <= HB_ELEM_SBEND) {
+            while (i < lat->elems.size() && (lat->elems[i].kind <= HB_ELEM_SBEND || lat->elems[i].kind == HB_ELEM_PLENS)) {
                 M = mat_mul(elem_matrix(lat->elems[i], bg), M);
                 seq.push_back(seq_elem(lat->elems[i], bg));
                 ++i;

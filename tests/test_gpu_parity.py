@@ -313,3 +313,54 @@ def test_push_is_capturable_in_a_cuda_graph(hb):
     own = oracle.moments(np.ascontiguousarray(got))
     assert np.allclose(rec[-1].cpu().numpy()[:6], own[:6], rtol=1e-9, atol=1e-16)
     lat.close()
+
+
+# ------------------------------------------------------------------ NEXT-2: plasma lens + moments -> host feedback
+@pytest.mark.parametrize("mode,tol", [("composed", 1e-6), ("sequential", 1e-6)])
+def test_plasma_lens_runs(hb, mode, tol):
+    """thick axisymmetric lens (R3b) inside fused runs: focusing, defocusing, zero strength, between other elements"""
+    els = [wl.drift(0.3), wl.plens(0.05, 40.0), wl.drift(0.2), wl.quad(0.1, 1.2), wl.plens(0.02, -15.0),
+           wl.sbend(0.5, 0.02), wl.plens(0.1, 0.0), wl.plens(0.03, 400.0), wl.drift(0.1), wl.monitor()]
+    desc = wl.lattice(els)
+    x = wl.gaussian_bunch(100_003, 21)
+    ref, ref_rec = oracle.push(desc, x)
+    got, rec = gpu_push(hb, desc, x, run_mode=mode, moments=True)
+    assert rel_err(got, ref).max() <= tol
+    diag = [6, 12, 17, 21, 24, 26]
+    assert np.allclose(rec[0][diag], ref_rec[0][diag], rtol=1e-4)
+
+
+def lens_strength_from_record(rec):
+    """a caller-side rule (the paper's own expression is in its ref. [31], not in the paper): matched focusing for
+    the measured beam, k = (eps/sigma^2)^2 averaged over the two planes, times a fixed factor"""
+    sxx, sxpx, spxpx = rec[6], rec[7], rec[12]
+    syy, sypy, spypy = rec[17], rec[18], rec[21]
+    ex2, ey2 = sxx * spxpx - sxpx ** 2, syy * spypy - sypy ** 2
+    return 50.0 * 0.5 * (ex2 / sxx ** 2 + ey2 / syy ** 2)
+
+
+def test_moments_to_host_feedback_sets_the_lens(hb):
+    """the paper's in-situ lens setting: push a stage, read the moment record on the host, set the strength
+    of the following plasma lens from it, push the transport -- on the GPU and in the oracle, same rule"""
+    import torch
+    desc1, x = wl.config1(prec="fp32", n=50_000)
+    stage = wl.lattice(desc1["elements"][:8])                      # FODO cell | monitor | surrogate | monitor
+    ref1, ref_rec1 = oracle.push(stage, x)
+    k_ref = lens_strength_from_record(ref_rec1[-1])
+    gap_ref = wl.lattice([wl.drift(0.1), wl.plens(0.02, k_ref), wl.drift(0.1), wl.monitor()])
+    ref2, ref_rec2 = oracle.push(gap_ref, ref1.astype(np.float32))
+
+    lat1 = hb.Lattice.from_description(stage, device=0)
+    c = hb.to_device(x)
+    rec1 = lat1.push_moments(c)
+    torch.cuda.synchronize()                                       # the per-stage device -> host sync the paper has
+    k_gpu = lens_strength_from_record(rec1[-1].cpu().numpy())
+    assert abs(k_gpu - k_ref) <= 1e-4 * abs(k_ref) and k_gpu > 0
+    lat2 = hb.Lattice.from_description(wl.lattice([wl.drift(0.1), wl.plens(0.02, k_gpu), wl.drift(0.1), wl.monitor()]), device=0)
+    rec2 = lat2.push_moments(c)
+    torch.cuda.synchronize()
+    got = hb.to_host(c).astype(np.float64)
+    assert rel_err(got, ref2).max() <= 2e-5
+    diag = [6, 12, 17, 21, 24, 26]
+    assert np.allclose(rec2[-1].cpu().numpy()[diag], ref_rec2[-1][diag], rtol=1e-4)
+    lat1.close(); lat2.close()
