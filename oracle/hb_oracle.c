@@ -76,6 +76,28 @@ void orc_drift(double *x, double *px, double *y, double *py, double *t, double *
     }
 }
 
+/* R2x (NEXT-3): drift of length L WITHOUT the paraxial / first-order expansion of R2.  In the coordinates
+ * of R1 the total momentum and energy of a particle, in units of p0 and p0 c, are
+ *     E/(p0 c) = 1/beta0 - pt,      pz = sqrt( (1/beta0 - pt)^2 - 1/(beta0 gamma0)^2 - px^2 - py^2 )
+ * (pz: longitudinal momentum / p0).  A free particle moves on a straight line with slopes px/pz, py/pz and takes the
+ * time L (E/(p0 c))/pz (in units of 1/c) to advance by L in s, the reference L/beta0:
+ *     x' = x + L px/pz,   y' = y + L py/pz,   t' = t + L ( (1/beta0 - pt)/pz - 1/beta0 ).
+ * First order in (px, py, pt) this is R2. */
+void orc_drift_exact(double *x, double *px, double *y, double *py, double *t, double *pt,
+                     long n, double L, double bg0)
+{
+    long i;
+    const double g0 = sqrt(1.0 + bg0 * bg0), b0 = bg0 / g0;
+#pragma omp parallel for schedule(static)
+    for (i = 0; i < n; ++i) {
+        const double e = 1.0 / b0 - pt[i];
+        const double pz = sqrt(e * e - 1.0 / (bg0 * bg0) - px[i] * px[i] - py[i] * py[i]);
+        x[i] = x[i] + L * px[i] / pz;
+        y[i] = y[i] + L * py[i] / pz;
+        t[i] = t[i] + L * (e / pz - 1.0 / b0);
+    }
+}
+
 /* one transverse plane of a thick quadrupole, R3 */
 static void quad_plane(double *u, double *pu, double L, double k_plane)
 {

@@ -73,6 +73,10 @@ def drift(c, L, bg0):
     lib().orc_drift(*_rows(c), ctypes.c_long(c.shape[1]), ctypes.c_double(L), ctypes.c_double(bg0))
 
 
+def drift_exact(c, L, bg0):
+    lib().orc_drift_exact(*_rows(c), ctypes.c_long(c.shape[1]), ctypes.c_double(L), ctypes.c_double(bg0))
+
+
 def quad(c, L, k, bg0):
     lib().orc_quad(*_rows(c), ctypes.c_long(c.shape[1]), ctypes.c_double(L), ctypes.c_double(k),
                    ctypes.c_double(bg0))
@@ -154,6 +158,8 @@ class Tracker:
         kind = el["kind"]
         if kind == "drift":
             drift(c, el["L"], self.bg)
+        elif kind == "drift_exact":
+            drift_exact(c, el["L"], self.bg)
         elif kind == "quad":
             quad(c, el["L"], el["k"], self.bg)
         elif kind == "plens":

@@ -540,3 +540,64 @@ def test_plens_8_particles_brute_force_and_axisymmetry():
     R[np.ix_([1, 3], [1, 3])] = [[math.cos(a), -math.sin(a)], [math.sin(a), math.cos(a)]]
     P, Q = jacobian([wl.plens(L, k)]), jacobian([wl.quad(L, k)])
     assert np.allclose(R @ P, P @ R, atol=1e-14) and not np.allclose(R @ Q, Q @ R, atol=1e-3)
+
+
+# ------------------------------------------------------------------------------ R2x exact drift (NEXT-3)
+def test_exact_drift_is_straight_line_geometry_and_time_of_flight():
+    """independent of the formula in the oracle: build the particle's velocity vector from (px, py, pt), fly it in a
+    straight line until it has advanced by L in s, compare position and arrival time"""
+    g0, bg0, b0 = oracle.reference(1000.0, wl.ELECTRON_MEV)[0], BG0, BG0 / math.sqrt(1 + BG0 ** 2)
+    rng = np.random.default_rng(3)
+    c = np.ascontiguousarray(rng.standard_normal((6, 64)) * np.array([1e-3, 2e-2, 1e-3, 2e-2, 1e-3, 5e-2])[:, None])
+    L = 3.7
+    got = c.copy()
+    oracle.Tracker(LAT).apply(wl.drift_exact(L), got)
+    for i in range(c.shape[1]):
+        x, px, y, py, t, pt = c[:, i]
+        gamma = g0 - pt * bg0                          # E = E0 - pt p0 c  (R1)
+        p = math.sqrt(gamma ** 2 - 1.0) / bg0          # |p| / p0
+        pz = math.sqrt(p * p - px * px - py * py)
+        beta = math.sqrt(1.0 - 1.0 / gamma ** 2)
+        path = L * p / pz                              # length of the straight line
+        assert abs(got[0, i] - (x + path * px / p)) < 1e-14 and abs(got[2, i] - (y + path * py / p)) < 1e-14
+        assert abs(got[4, i] - (t + path / beta - L / b0)) < 1e-12    # c (T - T_ref)
+        assert got[1, i] == px and got[3, i] == py and got[5, i] == pt
+
+
+def test_exact_drift_first_order_is_r2_and_it_is_symplectic():
+    L = 0.9
+    # Jacobian by central differences about the reference particle -> the matrix of R2
+    h = 1e-6
+    J = np.zeros((6, 6))
+    for j in range(6):
+        cp, cm = np.zeros((6, 1)), np.zeros((6, 1))
+        cp[j], cm[j] = h, -h
+        oracle.Tracker(LAT).apply(wl.drift_exact(L), cp)
+        oracle.Tracker(LAT).apply(wl.drift_exact(L), cm)
+        J[:, j] = (cp[:, 0] - cm[:, 0]) / (2 * h)
+    assert np.allclose(J, jacobian([wl.drift(L)]), atol=1e-9)
+    # ... and about a far-off-axis, off-momentum particle it is still a symplectic map
+    c0 = np.array([2e-3, 3e-2, -1e-3, -2e-2, 5e-4, 4e-2])
+    for j in range(6):
+        cp, cm = c0.reshape(6, 1).copy(), c0.reshape(6, 1).copy()
+        cp[j] += h; cm[j] -= h
+        oracle.Tracker(LAT).apply(wl.drift_exact(L), cp)
+        oracle.Tracker(LAT).apply(wl.drift_exact(L), cm)
+        J[:, j] = (cp[:, 0] - cm[:, 0]) / (2 * h)
+    assert np.max(np.abs(J.T @ S6 @ J - S6)) < 1e-8
+    assert not np.allclose(J, jacobian([wl.drift(L)]), atol=1e-6)        # it does differ from R2 there
+
+
+def test_exact_drift_composes_and_inverts():
+    c = rand_coords(32, 9, scale=np.array([1e-3, 1e-2, 1e-3, 1e-2, 1e-3, 1e-2]))
+    a, b = c.copy(), c.copy()
+    tr = oracle.Tracker(LAT)
+    tr.apply(wl.drift_exact(0.4), a); tr.apply(wl.drift_exact(0.6), a)
+    tr.apply(wl.drift_exact(1.0), b)
+    assert np.allclose(a, b, rtol=0, atol=1e-15)
+    tr.apply(wl.drift_exact(-1.0), b)
+    assert np.allclose(b, c, rtol=0, atol=1e-15)
+    # the reference particle stays the reference particle
+    z = np.zeros((6, 1))
+    tr.apply(wl.drift_exact(5.0), z)
+    assert np.all(z == 0.0)

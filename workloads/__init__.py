@@ -91,6 +91,7 @@ def surrogate(widths, W, b, act, in_mean, in_std, out_mean, out_std, coord="s",
 
 # ------------------------------------------------------------------------------ lattices
 def drift(L): return {"kind": "drift", "L": float(L)}
+def drift_exact(L): return {"kind": "drift_exact", "L": float(L)}
 def quad(L, k): return {"kind": "quad", "L": float(L), "k": float(k)}
 def sbend(L, theta): return {"kind": "sbend", "L": float(L), "theta": float(theta)}
 def plens(L, k): return {"kind": "plens", "L": float(L), "k": float(k)}
