@@ -118,7 +118,7 @@ def build_workload(name, prec, n):
 
 def count_work(desc):
     n_sur = sum(1 for e in desc["elements"] if e["kind"] == "surrogate")
-    n_el = sum(1 for e in desc["elements"] if e["kind"] in ("drift", "quad", "sbend", "plens"))
+    n_el = sum(1 for e in desc["elements"] if e["kind"] in ("drift", "quad", "sbend", "plens", "drift_exact"))
     flops = sum(wl.flops_per_particle(e["widths"]) for e in desc["elements"] if e["kind"] == "surrogate")
     return n_sur, n_el, flops
 

@@ -47,8 +47,12 @@ typedef enum {
  * 27-double moment record (R10) and splits runs (R5, G17).  PLENS: thick axisymmetric linear (plasma) lens
  * (R3b): x'' = -k x and y'' = -k y, k > 0 focuses both planes; the paper sets k from the
  * moments of the previous monitor with an expression it does not print -- here the caller supplies k
- * (read the record, build the next lattice). */
-typedef enum { HB_ELEM_DRIFT = 0, HB_ELEM_QUAD = 1, HB_ELEM_SBEND = 2, HB_ELEM_MONITOR = 3, HB_ELEM_PLENS = 5 } hb_elem_kind;
+ * (read the record, build the next lattice).
+ * DRIFT_EXACT: drift without the paraxial expansion of R2 (R2x: x += L px/pz, t += L((1/beta0 - pt)/pz - 1/beta0),
+ * pz = sqrt(1 - 2 pt/beta0 + pt^2 - px^2 - py^2)); non-linear, so a run that contains one is always applied
+ * element by element in fp64 registers (the SEQUENTIAL kernel), whatever the run mode. */
+typedef enum { HB_ELEM_DRIFT = 0, HB_ELEM_QUAD = 1, HB_ELEM_SBEND = 2, HB_ELEM_MONITOR = 3, HB_ELEM_PLENS = 5,
+               HB_ELEM_DRIFT_EXACT = 6 } hb_elem_kind;
 
 /* Activation sigma of Eq. 3: identity; ReLU Eq. 1; PReLU Eq. 2, one learned
  * slope per activation layer (G9); tanh (the "sigmoidal function" of P:90; BASELINE configs 1,4,5). */

@@ -11,7 +11,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libhb.so")
 
-ELEM_KINDS = {"drift": 0, "quad": 1, "sbend": 2, "monitor": 3, "plens": 5}
+ELEM_KINDS = {"drift": 0, "quad": 1, "sbend": 2, "monitor": 3, "plens": 5, "drift_exact": 6}
 ACTS = {"identity": 0, "relu": 1, "prelu": 2, "tanh": 3}
 PRECS = {"fp32": 0, "bf16": 1, "f16": 2, "tf32": 3}
 COORDS = {"s": 0, "t": 1}
@@ -277,8 +277,8 @@ class Lattice:
         lat = cls(desc["kinetic_MeV"], desc["rest_MeV"])
         for el in desc["elements"]:
             k = el["kind"]
-            if k == "drift":
-                lat.add_element("drift", el["L"])
+            if k in ("drift", "drift_exact"):
+                lat.add_element(k, el["L"])
             elif k in ("quad", "plens"):
                 lat.add_element(k, el["L"], el["k"])
             elif k == "sbend":

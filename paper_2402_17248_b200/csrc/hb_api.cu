@@ -56,6 +56,7 @@ struct Segment {
     int type;
     HbRunMap map;          // SEG_RUN composed
     int seq_off, seq_cnt;  // SEG_RUN sequential: range in d_seq
+    bool nonlinear;        // SEG_RUN holds a non-linear element: no composed map, always the fp64 sequential kernel
     HbSurDev sd;           // SEG_SUR
     bool tc;               // SEG_SUR: tensor-core kernel
     int monitor;           // record index written after this segment, -1 = none
@@ -94,7 +95,7 @@ Mat6 elem_matrix(const Elem& e, double bg) {
     Mat6 M = mat_identity();
     const double L = e.L;
     const double r56 = L / (bg * bg);
-    if (e.kind == HB_ELEM_DRIFT) {
+    if (e.kind == HB_ELEM_DRIFT || e.kind == HB_ELEM_DRIFT_EXACT) {   // (exact drift: its linearisation, unused)
         M.m[0][1] = L; M.m[2][3] = L; M.m[4][5] = r56;
     } else if (e.kind == HB_ELEM_QUAD || e.kind == HB_ELEM_PLENS) {
         const double k = e.param, w = std::sqrt(std::fabs(k)), ph = w * L;
@@ -131,7 +132,10 @@ HbSeqElem seq_elem(const Elem& e, double bg) {
     HbSeqElem s;
     std::memset(&s, 0, sizeof s);
     s.kind = e.kind == HB_ELEM_PLENS ? (int)HB_ELEM_QUAD : e.kind;   // the device applies a lens as two 2x2 planes + t
-    if (e.kind == HB_ELEM_DRIFT) {
+    if (e.kind == HB_ELEM_DRIFT_EXACT) {
+        s.kind = 3;
+        s.a[0] = e.L; s.a[1] = std::sqrt(1.0 + bg * bg) / bg;      // 1/beta0
+    } else if (e.kind == HB_ELEM_DRIFT) {
         s.a[0] = e.L; s.a[1] = M.m[4][5];
     } else if (e.kind == HB_ELEM_QUAD || e.kind == HB_ELEM_PLENS) {
         s.a[0] = M.m[0][0]; s.a[1] = M.m[0][1]; s.a[2] = M.m[1][0]; s.a[3] = M.m[1][1];
@@ -247,15 +251,15 @@ hb_status hb_lattice_create(double kin, double rest, hb_lattice** out) {
 hb_status hb_lattice_add_element(hb_lattice* lat, hb_elem_kind kind, double L, double param) {
     if (!lat) return fail(HB_ERR_INVALID_ARG, "lattice is NULL");
     if (lat->finalized) return fail(HB_ERR_STATE, "lattice already finalized");
-    if (((int)kind < 0 || (int)kind > HB_ELEM_MONITOR) && kind != HB_ELEM_PLENS)
+    if (((int)kind < 0 || (int)kind > HB_ELEM_MONITOR) && kind != HB_ELEM_PLENS && kind != HB_ELEM_DRIFT_EXACT)
         return fail(HB_ERR_INVALID_ARG, "unknown element kind %d", (int)kind);
     Elem e{(int)kind, 0.0, 0.0, -1};
     if (kind != HB_ELEM_MONITOR) {
         if (!std::isfinite(L)) return fail(HB_ERR_INVALID_ARG, "length must be finite");
-        if (kind != HB_ELEM_DRIFT && (!std::isfinite(param) || L < 0.0))
+        if (kind != HB_ELEM_DRIFT && kind != HB_ELEM_DRIFT_EXACT && (!std::isfinite(param) || L < 0.0))
             return fail(HB_ERR_INVALID_ARG, "quad/plens/sbend need a finite parameter and length >= 0");
         e.L = L;
-        e.param = kind == HB_ELEM_DRIFT ? 0.0 : param;
+        e.param = (kind == HB_ELEM_DRIFT || kind == HB_ELEM_DRIFT_EXACT) ? 0.0 : param;
     }
     lat->elems.push_back(e);
     return HB_OK;
@@ -466,7 +470,9 @@ hb_status hb_lattice_finalize(hb_lattice* lat, int device) {
             s.monitor = -1;
             s.seq_off = (int)seq.size();
             Mat6 M = mat_identity();
-            while (i < lat->elems.size() && (lat->elems[i].kind <= HB_ELEM_SBEND || lat->elems[i].kind == HB_ELEM_PLENS)) {
+            while (i < lat->elems.size() && (lat->elems[i].kind <= HB_ELEM_SBEND || lat->elems[i].kind == HB_ELEM_PLENS ||
+                                             lat->elems[i].kind == HB_ELEM_DRIFT_EXACT)) {
+                s.nonlinear = s.nonlinear || lat->elems[i].kind == HB_ELEM_DRIFT_EXACT;
                 M = mat_mul(elem_matrix(lat->elems[i], bg), M);
                 seq.push_back(seq_elem(lat->elems[i], bg));
                 ++i;
@@ -578,9 +584,9 @@ static hb_status push_impl(hb_lattice* lat, float* x, float* px, float* y, float
             int nblocks = 0;
             cudaError_t e = cudaSuccess;
             if (g.type == SEG_RUN) {
-                if (lat->run_mode == HB_RUN_COMPOSED) e = hb_launch_run_composed(p, n, g.map, partials, &nblocks, s);
+                if (lat->run_mode == HB_RUN_COMPOSED && !g.nonlinear) e = hb_launch_run_composed(p, n, g.map, partials, &nblocks, s);
                 else e = hb_launch_run_sequential(p, n, lat->d_seq + g.seq_off, g.seq_cnt,
-                                                  lat->run_mode == HB_RUN_SEQUENTIAL_FP32, partials, &nblocks, s);
+                                                  lat->run_mode == HB_RUN_SEQUENTIAL_FP32 && !g.nonlinear, partials, &nblocks, s);
             } else if (g.type == SEG_SUR) {
                 e = g.tc ? hb_launch_sur_tc(p, n, g.sd, partials, &nblocks, lat->sm_count, s)
                          : hb_launch_sur_fp32(p, n, g.sd, partials, &nblocks, lat->sm_count, s);

@@ -73,7 +73,7 @@ struct SeqElemT { T a[10]; int kind; };
 
 template <typename T>
 __device__ __forceinline__ void seq_apply(const SeqElemT<T>& e, T (&v)[6]) {
-    // v = (x, px, y, py, t, pt); pt never changes (R2-R4)
+    // v = (x, px, y, py, t, pt); pt never changes (R2-R4, R2x)
     if (e.kind == 0) {                 // drift R2
         v[0] = fma(e.a[0], v[1], v[0]);
         v[2] = fma(e.a[0], v[3], v[2]);
@@ -85,6 +85,14 @@ __device__ __forceinline__ void seq_apply(const SeqElemT<T>& e, T (&v)[6]) {
         v[2] = fma(e.a[4], y, e.a[5] * py);
         v[3] = fma(e.a[6], y, e.a[7] * py);
         v[4] = fma(e.a[8], v[5], v[4]);
+    } else if (e.kind == 3) {          // exact drift R2x (non-linear): a0 = L, a1 = 1/beta0
+        // pz^2 = (1/beta0 - pt)^2 - 1/(beta0 gamma0)^2 - px^2 - py^2 = 1 - 2 pt/beta0 + pt^2 - px^2 - py^2
+        const T px = v[1], py = v[3], pt = v[5];
+        const T pz2 = fma(pt, pt - T(2) * e.a[1], T(1)) - fma(px, px, py * py);
+        const T ipz = T(1) / sqrt(pz2);
+        v[0] = fma(e.a[0] * ipz, px, v[0]);
+        v[2] = fma(e.a[0] * ipz, py, v[2]);
+        v[4] = fma(e.a[0], fma(e.a[1] - pt, ipz, -e.a[1]), v[4]);
     } else {                           // sector bend R4
         const T x = v[0], px = v[1], d = v[5];
         v[0] = fma(e.a[0], x, fma(e.a[1], px, e.a[4] * d));

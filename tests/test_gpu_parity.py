@@ -364,3 +364,22 @@ def test_moments_to_host_feedback_sets_the_lens(hb):
     diag = [6, 12, 17, 21, 24, 26]
     assert np.allclose(rec2[-1].cpu().numpy()[diag], ref_rec2[-1][diag], rtol=1e-4)
     lat1.close(); lat2.close()
+
+
+# ------------------------------------------------------------------ NEXT-3: non-linear map in sequential mode
+@pytest.mark.parametrize("mode", ["composed", "sequential", "sequential_fp32"])
+def test_exact_drift_runs_in_fp64_registers_whatever_the_mode(hb, mode):
+    """a run holding a non-linear element (exact drift R2x) has no composed matrix: it always goes element by element
+    through the fp64 sequential kernel; large divergences and momentum offsets make the non-linearity matter"""
+    sig = np.array([1e-3, 2e-2, 1e-3, 2e-2, 1e-3, 3e-2])
+    x = wl.gaussian_bunch(70_001, 23, sigma=sig)
+    els = [wl.drift_exact(0.8), wl.quad(0.1, 1.2), wl.drift_exact(1.5), wl.plens(0.02, 30.0), wl.drift_exact(-0.3),
+           wl.sbend(0.5, 0.02), wl.drift(0.2), wl.monitor()]
+    desc = wl.lattice(els)
+    ref, ref_rec = oracle.push(desc, x)
+    lin, _ = oracle.push(wl.lattice([wl.drift(e["L"]) if e["kind"] == "drift_exact" else e for e in els]), x)
+    assert rel_err(lin, ref).max() > 1e-3                      # the paraxial drift is visibly different here
+    got, rec = gpu_push(hb, desc, x, run_mode=mode, moments=True)
+    assert rel_err(got, ref).max() <= 1e-6
+    diag = [6, 12, 17, 21, 24, 26]
+    assert np.allclose(rec[0][diag], ref_rec[0][diag], rtol=1e-4)
