@@ -98,6 +98,76 @@ void orc_drift_exact(double *x, double *px, double *y, double *py, double *t, do
     }
 }
 
+/* R3x (NEXT-3, "chromatic effects"): thick quadrupole whose focusing depends on the particle's momentum.
+ * With 1+delta = |p|/p0 = sqrt((1/beta0 - pt)^2 - 1/(beta0 gamma0)^2) and e = E/(p0 c) = 1/beta0 - pt, the paraxial
+ * Hamiltonian of the quadrupole for an off-momentum particle is
+ *     H = -(1+delta) + (px^2 + py^2)/(2(1+delta)) + k (x^2 - y^2)/2 - pt/beta0
+ * so  x' = px/(1+delta), px' = -k x  (omega^2 = k/(1+delta): "k -> k/(1+delta)"),  y likewise with -k, and
+ *     t' = dH/dpt = e/(1+delta) - 1/beta0 + e (px^2 + py^2) / (2 (1+delta)^3).
+ * chr_plane advances one plane over L and returns  integral_0^L p(s)^2 ds  (closed form of the harmonic motion). */
+static double chr_plane(double *u, double *pu, double L, double k_plane, double d1 /* 1+delta */)
+{
+    const double u0 = *u, p0 = *pu;
+    double A = p0, B, I;
+    if (k_plane > 0.0) {
+        const double w = sqrt(k_plane / d1), c = cos(w * L), sn = sin(w * L);
+        B = -w * d1 * u0;                         /* p(s) = A cos(ws) + B sin(ws) */
+        *u = c * u0 + sn / (w * d1) * p0;
+        *pu = B * sn + A * c;
+        I = 0.5 * (A * A + B * B) * L + (A * A - B * B) * sin(2.0 * w * L) / (4.0 * w)
+            + A * B * (1.0 - cos(2.0 * w * L)) / (2.0 * w);
+    } else if (k_plane < 0.0) {
+        const double w = sqrt(-k_plane / d1), c = cosh(w * L), sn = sinh(w * L);
+        B = w * d1 * u0;                          /* p(s) = A cosh(ws) + B sinh(ws) */
+        *u = c * u0 + sn / (w * d1) * p0;
+        *pu = B * sn + A * c;
+        I = 0.5 * (A * A - B * B) * L + (A * A + B * B) * sinh(2.0 * w * L) / (4.0 * w)
+            + A * B * (cosh(2.0 * w * L) - 1.0) / (2.0 * w);
+    } else {
+        *u = u0 + L * p0 / d1;
+        I = p0 * p0 * L;
+    }
+    return I;
+}
+
+void orc_quad_chromatic(double *x, double *px, double *y, double *py, double *t, double *pt,
+                        long n, double L, double k, double bg0)
+{
+    long i;
+    const double g0 = sqrt(1.0 + bg0 * bg0), b0 = bg0 / g0;
+#pragma omp parallel for schedule(static)
+    for (i = 0; i < n; ++i) {
+        const double e = 1.0 / b0 - pt[i];
+        const double d1 = sqrt(e * e - 1.0 / (bg0 * bg0));
+        const double Ix = chr_plane(&x[i], &px[i], L, k, d1);
+        const double Iy = chr_plane(&y[i], &py[i], L, -k, d1);
+        t[i] = t[i] + L * (e / d1 - 1.0 / b0) + e * (Ix + Iy) / (2.0 * d1 * d1 * d1);
+    }
+}
+
+/* R5x (NEXT-3): thin multipole kick of order m (1 = dipole, 2 = quadrupole, 3 = sextupole, ...) with integrated
+ * normal / skew strengths kn, ks [m^-(m-1)]:  px - i py  -=  (kn + i ks) (x + i y)^(m-1) / (m-1)!   (the usual complex
+ * form; m = 2, ks = 0:  px -= kn x,  py += kn y,  the thin limit of R3).  Positions and (t, pt) unchanged. */
+void orc_multipole(double *x, double *px, double *y, double *py, double *t, double *pt,
+                   long n, int m, double kn, double ks)
+{
+    long i;
+    int j;
+    double fact = 1.0;
+    (void)t; (void)pt;
+    for (j = 2; j < m; ++j) fact *= (double)j;
+#pragma omp parallel for schedule(static) private(j)
+    for (i = 0; i < n; ++i) {
+        double zr = 1.0, zi = 0.0;                /* (x + i y)^(m-1) */
+        for (j = 1; j < m; ++j) {
+            const double r = zr * x[i] - zi * y[i], im = zr * y[i] + zi * x[i];
+            zr = r; zi = im;
+        }
+        px[i] = px[i] - (kn * zr - ks * zi) / fact;
+        py[i] = py[i] + (kn * zi + ks * zr) / fact;
+    }
+}
+
 /* one transverse plane of a thick quadrupole, R3 */
 static void quad_plane(double *u, double *pu, double L, double k_plane)
 {

@@ -77,6 +77,16 @@ def drift_exact(c, L, bg0):
     lib().orc_drift_exact(*_rows(c), ctypes.c_long(c.shape[1]), ctypes.c_double(L), ctypes.c_double(bg0))
 
 
+def quad_chromatic(c, L, k, bg0):
+    lib().orc_quad_chromatic(*_rows(c), ctypes.c_long(c.shape[1]), ctypes.c_double(L), ctypes.c_double(k),
+                             ctypes.c_double(bg0))
+
+
+def multipole(c, order, kn, ks):
+    lib().orc_multipole(*_rows(c), ctypes.c_long(c.shape[1]), ctypes.c_int(int(order)), ctypes.c_double(kn),
+                        ctypes.c_double(ks))
+
+
 def quad(c, L, k, bg0):
     lib().orc_quad(*_rows(c), ctypes.c_long(c.shape[1]), ctypes.c_double(L), ctypes.c_double(k),
                    ctypes.c_double(bg0))
@@ -160,6 +170,10 @@ class Tracker:
             drift(c, el["L"], self.bg)
         elif kind == "drift_exact":
             drift_exact(c, el["L"], self.bg)
+        elif kind == "quad_chromatic":
+            quad_chromatic(c, el["L"], el["k"], self.bg)
+        elif kind == "multipole":
+            multipole(c, el["order"], el["kn"], el["ks"])
         elif kind == "quad":
             quad(c, el["L"], el["k"], self.bg)
         elif kind == "plens":

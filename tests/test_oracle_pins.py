@@ -601,3 +601,71 @@ def test_exact_drift_composes_and_inverts():
     z = np.zeros((6, 1))
     tr.apply(wl.drift_exact(5.0), z)
     assert np.all(z == 0.0)
+
+
+# ------------------------------------------------------------------------------ R3x chromatic quad, R5x multipole (NEXT-3)
+def fd_jacobian(el, c0, h=1e-6):
+    J = np.zeros((6, 6))
+    for j in range(6):
+        cp, cm = np.array(c0, float).reshape(6, 1), np.array(c0, float).reshape(6, 1)
+        cp[j] += h; cm[j] -= h
+        oracle.Tracker(LAT).apply(el, cp)
+        oracle.Tracker(LAT).apply(el, cm)
+        J[:, j] = (cp[:, 0] - cm[:, 0]) / (2 * h)
+    return J
+
+
+@pytest.mark.parametrize("k", [1.2, -1.2, 0.0])
+def test_chromatic_quad_on_momentum_is_r3_and_off_momentum_rescales_k(k):
+    L = 0.4
+    M = fd_jacobian(wl.quad_chromatic(L, k), np.zeros(6))
+    assert np.allclose(M, jacobian([wl.quad(L, k)]), atol=1e-9)          # at pt = 0 it is the quadrupole of R3
+    # off momentum: the transverse 4x4 is the R3 matrix of strength k/(1+delta) with px measured in units of p0(1+delta)
+    pt = 0.05
+    b0 = BG0 / math.sqrt(1 + BG0 ** 2)
+    d1 = math.sqrt((1 / b0 - pt) ** 2 - 1 / BG0 ** 2)
+    c0 = np.array([0, 0, 0, 0, 0, pt])
+    J = fd_jacobian(wl.quad_chromatic(L, k), c0)
+    Q = jacobian([wl.quad(L, k / d1)])
+    S = np.diag([1, d1, 1, d1])                                          # (x, px) -> (x, px/(1+delta)) and back
+    assert np.allclose(J[:4, :4], S @ Q[:4, :4] @ np.linalg.inv(S), atol=1e-8)
+
+
+def test_chromatic_quad_is_symplectic_including_the_time_of_flight_term():
+    """a wrong or missing betatron term in t breaks M^T S M = S through the (t, x..py) couplings"""
+    c0 = np.array([2e-3, 1e-2, -1e-3, -2e-2, 3e-4, 4e-2])
+    for k in (2.0, -2.0):
+        J = fd_jacobian(wl.quad_chromatic(0.7, k), c0)
+        assert np.max(np.abs(J.T @ S6 @ J - S6)) < 2e-8
+        assert abs(J[4, 0]) > 1e-6 and abs(J[4, 3]) > 1e-6               # the couplings are really there
+
+
+def test_chromatic_quad_zero_strength_on_axis_is_the_exact_drift():
+    c = np.zeros((6, 5)); c[5] = [-0.1, -0.01, 0.0, 0.02, 0.2]
+    a, b = c.copy(), c.copy()
+    oracle.Tracker(LAT).apply(wl.quad_chromatic(1.3, 0.0), a)
+    oracle.Tracker(LAT).apply(wl.drift_exact(1.3), b)
+    assert np.allclose(a, b, rtol=0, atol=1e-15)                          # px = py = 0: pure time of flight
+
+
+def test_multipole_kicks():
+    c = rand_coords(16, 4, scale=np.array([1e-2, 1e-3, 1e-2, 1e-3, 1e-3, 1e-3]))
+    x, y = c[0].copy(), c[2].copy()
+    # quadrupole kick = thin limit of R3
+    got = c.copy(); oracle.Tracker(LAT).apply(wl.multipole(2, 0.8), got)
+    assert np.allclose(got[1], c[1] - 0.8 * x) and np.allclose(got[3], c[3] + 0.8 * y)
+    L = 1e-7
+    assert np.allclose(fd_jacobian(wl.multipole(2, 0.8), np.zeros(6)), jacobian([wl.quad(L, 0.8 / L)]), atol=2e-6)
+    # sextupole: px -= kn (x^2 - y^2)/2, py += kn x y; skew quadrupole: px -= -ks y ... from the complex form
+    got = c.copy(); oracle.Tracker(LAT).apply(wl.multipole(3, 5.0), got)
+    assert np.allclose(got[1], c[1] - 5.0 * (x * x - y * y) / 2) and np.allclose(got[3], c[3] + 5.0 * x * y)
+    got = c.copy(); oracle.Tracker(LAT).apply(wl.multipole(2, 0.0, 0.3), got)
+    assert np.allclose(got[1], c[1] + 0.3 * y) and np.allclose(got[3], c[3] + 0.3 * x)
+    # dipole kick is a constant; positions, t, pt never change; every kick is symplectic (derives from a potential)
+    got = c.copy(); oracle.Tracker(LAT).apply(wl.multipole(1, 1e-3, 2e-3), got)
+    assert np.allclose(got[1], c[1] - 1e-3) and np.allclose(got[3], c[3] + 2e-3)
+    for el in (wl.multipole(3, 5.0, -2.0), wl.multipole(4, 40.0, 10.0)):
+        J = fd_jacobian(el, [3e-3, 0, -2e-3, 0, 0, 0], h=1e-5)
+        assert np.max(np.abs(J.T @ S6 @ J - S6)) < 1e-7
+        got = c.copy(); oracle.Tracker(LAT).apply(el, got)
+        assert np.array_equal(got[[0, 2, 4, 5]], c[[0, 2, 4, 5]])

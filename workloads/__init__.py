@@ -92,6 +92,8 @@ def surrogate(widths, W, b, act, in_mean, in_std, out_mean, out_std, coord="s",
 # ------------------------------------------------------------------------------ lattices
 def drift(L): return {"kind": "drift", "L": float(L)}
 def drift_exact(L): return {"kind": "drift_exact", "L": float(L)}
+def quad_chromatic(L, k): return {"kind": "quad_chromatic", "L": float(L), "k": float(k)}
+def multipole(order, kn, ks=0.0): return {"kind": "multipole", "order": int(order), "kn": float(kn), "ks": float(ks)}
 def quad(L, k): return {"kind": "quad", "L": float(L), "k": float(k)}
 def sbend(L, theta): return {"kind": "sbend", "L": float(L), "theta": float(theta)}
 def plens(L, k): return {"kind": "plens", "L": float(L), "k": float(k)}
