@@ -118,7 +118,7 @@ def build_workload(name, prec, n):
 
 def count_work(desc):
     n_sur = sum(1 for e in desc["elements"] if e["kind"] == "surrogate")
-    n_el = sum(1 for e in desc["elements"] if e["kind"] in ("drift", "quad", "sbend", "plens", "drift_exact"))
+    n_el = sum(1 for e in desc["elements"] if e["kind"] in ("drift", "quad", "sbend", "plens", "drift_exact", "quad_chromatic", "multipole"))
     flops = sum(wl.flops_per_particle(e["widths"]) for e in desc["elements"] if e["kind"] == "surrogate")
     return n_sur, n_el, flops
 
@@ -277,6 +277,14 @@ def kernel_extras(torch, hb, args, pk, flush, dev):
                 "particle_element_pushes_per_s": 500.0 * n / (k_ms * 1e-3),
                 "roofline": {"bound": "alu", "achieved": ach, "peak": dp_peak, "unit": "TFMA/s (fp64)", "frac": ach / dp_peak,
                              "traffic": None}})
+    # non-linear run (NEXT-3): 100 chromatic FODO cells = 300 exact drifts + 200 chromatic quadrupoles, always on the
+    # fp64 sequential kernel (sin/cos/sqrt per particle and element: ALU/MUFU-bound, no closed-form FMA count)
+    cell = [wl.drift_exact(0.25), wl.quad_chromatic(0.1, 1.2), wl.drift_exact(0.5), wl.quad_chromatic(0.1, -1.2), wl.drift_exact(0.25)]
+    descn = wl.lattice(cell * 100 + [wl.monitor()])
+    ms, seg = measure(descn, x2, "run", True, steps=3)
+    k_ms = float(seg[0])
+    out.append({"kernel": "hb_run_sequential_kernel<double> (non-linear elements)", "workload": "100 chromatic FODO cells, N=%d" % n,
+                "ms": k_ms, "particle_element_pushes_per_s": 500.0 * n / (k_ms * 1e-3)})
     del x2
     # (b) surrogate C3 in f16 (same instruction, same rate) and fp32 FFMA
     if args.workload == "C3":

@@ -50,9 +50,11 @@ typedef enum {
  * (read the record, build the next lattice).
  * DRIFT_EXACT: drift without the paraxial expansion of R2 (R2x: x += L px/pz, t += L((1/beta0 - pt)/pz - 1/beta0),
  * pz = sqrt(1 - 2 pt/beta0 + pt^2 - px^2 - py^2)); non-linear, so a run that contains one is always applied
- * element by element in fp64 registers (the SEQUENTIAL kernel), whatever the run mode. */
+ * element by element in fp64 registers (the SEQUENTIAL kernel), whatever the run mode.
+ * QUAD_CHROMATIC (R3x): thick quadrupole with momentum-dependent focusing, omega^2 = k/(1+delta), and the betatron
+ * term in the time of flight.  MULTIPOLE (R5x): thin kick, added with hb_lattice_add_multipole.  Both non-linear. */
 typedef enum { HB_ELEM_DRIFT = 0, HB_ELEM_QUAD = 1, HB_ELEM_SBEND = 2, HB_ELEM_MONITOR = 3, HB_ELEM_PLENS = 5,
-               HB_ELEM_DRIFT_EXACT = 6 } hb_elem_kind;
+               HB_ELEM_DRIFT_EXACT = 6, HB_ELEM_QUAD_CHROMATIC = 7, HB_ELEM_MULTIPOLE = 8 } hb_elem_kind;
 
 /* Activation sigma of Eq. 3: identity; ReLU Eq. 1; PReLU Eq. 2, one learned
  * slope per activation layer (G9); tanh (the "sigmoidal function" of P:90; BASELINE configs 1,4,5). */
@@ -108,6 +110,11 @@ hb_status hb_lattice_create(double ref_kinetic_energy_MeV, double rest_energy_Me
  * [rad], signed (R4); else ignored.
  * Errors: finalized lattice -> STATE; non-finite or negative QUAD/SBEND length -> INVALID_ARG. */
 hb_status hb_lattice_add_element(hb_lattice *lat, hb_elem_kind kind, double length_m, double param);
+
+/* Append a thin multipole kick (R5x) of order m (1 dipole, 2 quadrupole, 3 sextupole, ... <= 8) with integrated normal
+ * and skew strengths kn, ks [m^-(m-1)]:  px - i py -= (kn + i ks)(x + i y)^(m-1)/(m-1)!.  Non-linear for m > 2: the run
+ * that holds it is applied element by element in fp64 registers.  Errors as hb_lattice_add_element. */
+hb_status hb_lattice_add_multipole(hb_lattice *lat, int order, double kn, double ks);
 
 /* Append a surrogate stage; deep-copies every host array of *desc.
  * Errors: widths[0] != 6 or widths[last] != 6, H outside [1,1024], std <= 0, non-finite values,

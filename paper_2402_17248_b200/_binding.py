@@ -11,14 +11,15 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libhb.so")
 
-ELEM_KINDS = {"drift": 0, "quad": 1, "sbend": 2, "monitor": 3, "plens": 5, "drift_exact": 6}
+ELEM_KINDS = {"drift": 0, "quad": 1, "sbend": 2, "monitor": 3, "plens": 5, "drift_exact": 6, "quad_chromatic": 7}
 ACTS = {"identity": 0, "relu": 1, "prelu": 2, "tanh": 3}
 PRECS = {"fp32": 0, "bf16": 1, "f16": 2, "tf32": 3}
 COORDS = {"s": 0, "t": 1}
 RUN_MODES = {"composed": 0, "sequential": 1, "sequential_fp32": 2}
 
 EXPORTED_SYMBOLS = [
-    "hb_lattice_create", "hb_lattice_add_element", "hb_lattice_add_surrogate", "hb_lattice_set_run_mode",
+    "hb_lattice_create", "hb_lattice_add_element", "hb_lattice_add_multipole", "hb_lattice_add_surrogate",
+    "hb_lattice_set_run_mode",
     "hb_lattice_finalize", "hb_lattice_num_monitors", "hb_lattice_num_launches", "hb_lattice_ref_bg_out",
     "hb_push", "hb_push_moments", "hb_moments", "hb_moments_scratch_bytes", "hb_lattice_destroy",
     "hb_lattice_enable_timing", "hb_lattice_get_timing",
@@ -69,6 +70,7 @@ def lib():
     fp = POINTER(c_float)
     L.hb_lattice_create.argtypes = [c_double, c_double, POINTER(c_void_p)]
     L.hb_lattice_add_element.argtypes = [c_void_p, c_int, c_double, c_double]
+    L.hb_lattice_add_multipole.argtypes = [c_void_p, c_int, c_double, c_double]
     L.hb_lattice_add_surrogate.argtypes = [c_void_p, POINTER(_SurrogateDesc)]
     L.hb_lattice_set_run_mode.argtypes = [c_void_p, c_int]
     L.hb_lattice_finalize.argtypes = [c_void_p, c_int]
@@ -124,6 +126,10 @@ def hb_lattice_create(ref_kinetic_energy_MeV: float, rest_energy_MeV: float):
     h = c_void_p()
     _check(lib().hb_lattice_create(ref_kinetic_energy_MeV, rest_energy_MeV, ctypes.byref(h)), "hb_lattice_create")
     return h
+
+
+def hb_lattice_add_multipole(lat, order: int, kn: float, ks: float = 0.0):
+    _check(lib().hb_lattice_add_multipole(lat, int(order), float(kn), float(ks)), "hb_lattice_add_multipole")
 
 
 def hb_lattice_add_element(lat, kind, length_m: float = 0.0, param: float = 0.0):
@@ -279,8 +285,10 @@ class Lattice:
             k = el["kind"]
             if k in ("drift", "drift_exact"):
                 lat.add_element(k, el["L"])
-            elif k in ("quad", "plens"):
+            elif k in ("quad", "plens", "quad_chromatic"):
                 lat.add_element(k, el["L"], el["k"])
+            elif k == "multipole":
+                hb_lattice_add_multipole(lat._h, el["order"], el["kn"], el["ks"])
             elif k == "sbend":
                 lat.add_element("sbend", el["L"], el["theta"])
             elif k == "monitor":

@@ -36,7 +36,16 @@ struct Elem {
     int kind;        // hb_elem_kind, or 4 = surrogate
     double L, param;
     int sur;         // index into surrogates
+    double p2 = 0.0; // MULTIPOLE: skew strength (L = order, param = normal strength)
 };
+
+bool is_conventional(int kind) {
+    return kind <= HB_ELEM_SBEND || kind == HB_ELEM_PLENS || kind == HB_ELEM_DRIFT_EXACT ||
+           kind == HB_ELEM_QUAD_CHROMATIC || kind == HB_ELEM_MULTIPOLE;
+}
+bool is_nonlinear(int kind) {
+    return kind == HB_ELEM_DRIFT_EXACT || kind == HB_ELEM_QUAD_CHROMATIC || kind == HB_ELEM_MULTIPOLE;
+}
 
 struct SurHost {
     int n_linear;
@@ -97,7 +106,9 @@ Mat6 elem_matrix(const Elem& e, double bg) {
     const double r56 = L / (bg * bg);
     if (e.kind == HB_ELEM_DRIFT || e.kind == HB_ELEM_DRIFT_EXACT) {   // (exact drift: its linearisation, unused)
         M.m[0][1] = L; M.m[2][3] = L; M.m[4][5] = r56;
-    } else if (e.kind == HB_ELEM_QUAD || e.kind == HB_ELEM_PLENS) {
+    } else if (e.kind == HB_ELEM_MULTIPOLE) {
+        // identity (thin; the run it sits in is never composed)
+    } else if (e.kind == HB_ELEM_QUAD || e.kind == HB_ELEM_PLENS || e.kind == HB_ELEM_QUAD_CHROMATIC) {
         const double k = e.param, w = std::sqrt(std::fabs(k)), ph = w * L;
         // focusing plane: [cos, sin/w; -w sin, cos]; defocusing: [cosh, sinh/w; w sinh, cosh]
         double f[4], d[4];
@@ -132,7 +143,16 @@ HbSeqElem seq_elem(const Elem& e, double bg) {
     HbSeqElem s;
     std::memset(&s, 0, sizeof s);
     s.kind = e.kind == HB_ELEM_PLENS ? (int)HB_ELEM_QUAD : e.kind;   // the device applies a lens as two 2x2 planes + t
-    if (e.kind == HB_ELEM_DRIFT_EXACT) {
+    if (e.kind == HB_ELEM_QUAD_CHROMATIC) {
+        s.kind = 4;
+        s.a[0] = e.L; s.a[1] = e.param; s.a[2] = std::sqrt(1.0 + bg * bg) / bg;
+    } else if (e.kind == HB_ELEM_MULTIPOLE) {
+        s.kind = 5;
+        const int m = (int)e.L;
+        double fact = 1.0;
+        for (int j = 2; j < m; ++j) fact *= j;
+        s.a[0] = e.param / fact; s.a[1] = e.p2 / fact; s.a[2] = (double)m;
+    } else if (e.kind == HB_ELEM_DRIFT_EXACT) {
         s.kind = 3;
         s.a[0] = e.L; s.a[1] = std::sqrt(1.0 + bg * bg) / bg;      // 1/beta0
     } else if (e.kind == HB_ELEM_DRIFT) {
@@ -251,7 +271,9 @@ hb_status hb_lattice_create(double kin, double rest, hb_lattice** out) {
 hb_status hb_lattice_add_element(hb_lattice* lat, hb_elem_kind kind, double L, double param) {
     if (!lat) return fail(HB_ERR_INVALID_ARG, "lattice is NULL");
     if (lat->finalized) return fail(HB_ERR_STATE, "lattice already finalized");
-    if (((int)kind < 0 || (int)kind > HB_ELEM_MONITOR) && kind != HB_ELEM_PLENS && kind != HB_ELEM_DRIFT_EXACT)
+    if (kind == HB_ELEM_MULTIPOLE) return fail(HB_ERR_INVALID_ARG, "use hb_lattice_add_multipole for a multipole kick");
+    if (((int)kind < 0 || (int)kind > HB_ELEM_MONITOR) && kind != HB_ELEM_PLENS && kind != HB_ELEM_DRIFT_EXACT &&
+        kind != HB_ELEM_QUAD_CHROMATIC)
         return fail(HB_ERR_INVALID_ARG, "unknown element kind %d", (int)kind);
     Elem e{(int)kind, 0.0, 0.0, -1};
     if (kind != HB_ELEM_MONITOR) {
@@ -261,6 +283,17 @@ hb_status hb_lattice_add_element(hb_lattice* lat, hb_elem_kind kind, double L, d
         e.L = L;
         e.param = (kind == HB_ELEM_DRIFT || kind == HB_ELEM_DRIFT_EXACT) ? 0.0 : param;
     }
+    lat->elems.push_back(e);
+    return HB_OK;
+}
+
+hb_status hb_lattice_add_multipole(hb_lattice* lat, int order, double kn, double ks) {
+    if (!lat) return fail(HB_ERR_INVALID_ARG, "lattice is NULL");
+    if (lat->finalized) return fail(HB_ERR_STATE, "lattice already finalized");
+    if (order < 1 || order > 8) return fail(HB_ERR_INVALID_ARG, "multipole order must be 1..8");
+    if (!std::isfinite(kn) || !std::isfinite(ks)) return fail(HB_ERR_INVALID_ARG, "multipole strengths must be finite");
+    Elem e{(int)HB_ELEM_MULTIPOLE, (double)order, kn, -1};
+    e.p2 = ks;
     lat->elems.push_back(e);
     return HB_OK;
 }
@@ -470,9 +503,8 @@ hb_status hb_lattice_finalize(hb_lattice* lat, int device) {
             s.monitor = -1;
             s.seq_off = (int)seq.size();
             Mat6 M = mat_identity();
-            while (i < lat->elems.size() && (lat->elems[i].kind <= HB_ELEM_SBEND || lat->elems[i].kind == HB_ELEM_PLENS ||
-                                             lat->elems[i].kind == HB_ELEM_DRIFT_EXACT)) {
-                s.nonlinear = s.nonlinear || lat->elems[i].kind == HB_ELEM_DRIFT_EXACT;
+            while (i < lat->elems.size() && is_conventional(lat->elems[i].kind)) {
+                s.nonlinear = s.nonlinear || is_nonlinear(lat->elems[i].kind);
                 M = mat_mul(elem_matrix(lat->elems[i], bg), M);
                 seq.push_back(seq_elem(lat->elems[i], bg));
                 ++i;

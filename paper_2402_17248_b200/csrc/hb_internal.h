@@ -20,6 +20,8 @@ struct HbRunMap {             // composed run: v' = M v (row-major 6x6, fp32, bu
 //  kind 1 quad  : a0..a3 = x-plane 2x2 (row-major), a4..a7 = y-plane 2x2, a8 = L/(bg)^2
 //  kind 2 sbend : a0..a3 = x-plane 2x2, a4 = R16, a5 = R26, a6 = L (y drift), a7 = R51, a8 = R52, a9 = R56
 //  kind 3 exact drift (non-linear, R2x) : a0 = L, a1 = 1/beta0
+//  kind 4 chromatic quad (non-linear, R3x) : a0 = L, a1 = k, a2 = 1/beta0
+//  kind 5 thin multipole kick (non-linear for m > 2, R5x) : a0 = kn/(m-1)!, a1 = ks/(m-1)!, a2 = m
 struct HbSeqElem {
     double a[10];
     int kind;

@@ -73,7 +73,7 @@ struct SeqElemT { T a[10]; int kind; };
 
 template <typename T>
 __device__ __forceinline__ void seq_apply(const SeqElemT<T>& e, T (&v)[6]) {
-    // v = (x, px, y, py, t, pt); pt never changes (R2-R4, R2x)
+    // v = (x, px, y, py, t, pt); pt never changes (R2-R5x)
     if (e.kind == 0) {                 // drift R2
         v[0] = fma(e.a[0], v[1], v[0]);
         v[2] = fma(e.a[0], v[3], v[2]);
@@ -93,6 +93,42 @@ __device__ __forceinline__ void seq_apply(const SeqElemT<T>& e, T (&v)[6]) {
         v[0] = fma(e.a[0] * ipz, px, v[0]);
         v[2] = fma(e.a[0] * ipz, py, v[2]);
         v[4] = fma(e.a[0], fma(e.a[1] - pt, ipz, -e.a[1]), v[4]);
+    } else if (e.kind == 4) {          // chromatic thick quad R3x (non-linear): a0 = L, a1 = k, a2 = 1/beta0
+        const T L = e.a[0], k = e.a[1], pt = v[5];
+        const T en = e.a[2] - pt;                                   // E / (p0 c)
+        const T d1 = sqrt(fma(pt, pt - T(2) * e.a[2], T(1)));       // 1 + delta = |p| / p0
+        T I = T(0);                                                 // integral of px^2 + py^2 over the element
+#pragma unroll
+        for (int pl = 0; pl < 2; ++pl) {
+            const T kp = pl == 0 ? k : -k;
+            const T u0 = v[2 * pl], p0 = v[2 * pl + 1];
+            if (kp > T(0)) {
+                const T w = sqrt(kp / d1), c = cos(w * L), sn = sin(w * L), B = -w * d1 * u0;
+                v[2 * pl] = fma(c, u0, sn / (w * d1) * p0);
+                v[2 * pl + 1] = fma(B, sn, p0 * c);
+                I += T(0.5) * (p0 * p0 + B * B) * L + (p0 * p0 - B * B) * sin(T(2) * w * L) / (T(4) * w) +
+                     p0 * B * (T(1) - cos(T(2) * w * L)) / (T(2) * w);
+            } else if (kp < T(0)) {
+                const T w = sqrt(-kp / d1), c = cosh(w * L), sn = sinh(w * L), B = w * d1 * u0;
+                v[2 * pl] = fma(c, u0, sn / (w * d1) * p0);
+                v[2 * pl + 1] = fma(B, sn, p0 * c);
+                I += T(0.5) * (p0 * p0 - B * B) * L + (p0 * p0 + B * B) * sinh(T(2) * w * L) / (T(4) * w) +
+                     p0 * B * (cosh(T(2) * w * L) - T(1)) / (T(2) * w);
+            } else {
+                v[2 * pl] = fma(L / d1, p0, u0);
+                I += p0 * p0 * L;
+            }
+        }
+        v[4] += L * (en / d1 - e.a[2]) + en * I / (T(2) * d1 * d1 * d1);
+    } else if (e.kind == 5) {          // thin multipole kick R5x: a0 = kn/(m-1)!, a1 = ks/(m-1)!, a2 = m
+        const int m = (int)e.a[2];
+        T zr = T(1), zi = T(0);
+        for (int j = 1; j < m; ++j) {
+            const T r = zr * v[0] - zi * v[2], im = zr * v[2] + zi * v[0];
+            zr = r; zi = im;
+        }
+        v[1] -= e.a[0] * zr - e.a[1] * zi;
+        v[3] += e.a[0] * zi + e.a[1] * zr;
     } else {                           // sector bend R4
         const T x = v[0], px = v[1], d = v[5];
         v[0] = fma(e.a[0], x, fma(e.a[1], px, e.a[4] * d));

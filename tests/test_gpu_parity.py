@@ -383,3 +383,43 @@ def test_exact_drift_runs_in_fp64_registers_whatever_the_mode(hb, mode):
     assert rel_err(got, ref).max() <= 1e-6
     diag = [6, 12, 17, 21, 24, 26]
     assert np.allclose(rec[0][diag], ref_rec[0][diag], rtol=1e-4)
+
+
+def test_chromatic_quads_and_multipole_kicks(hb):
+    """the rest of NEXT-3: a chromatic FODO cell (exact drifts + momentum-dependent quadrupoles) with sextupole /
+    octupole / skew kicks, wide momentum spread, against the oracle; and the first-order limit on the device:
+    on-momentum, small amplitudes -> the linear cell of the composed kernel"""
+    sig = np.array([1e-3, 1e-3, 1e-3, 1e-3, 1e-3, 3e-2])
+    x = wl.gaussian_bunch(60_007, 29, sigma=sig)
+    els = [wl.drift_exact(0.25), wl.quad_chromatic(0.1, 1.2), wl.multipole(3, 20.0, -5.0), wl.drift_exact(0.5),
+           wl.quad_chromatic(0.1, -1.2), wl.multipole(4, 3e3, 1e3), wl.multipole(1, 1e-5, -2e-5), wl.drift_exact(0.25),
+           wl.quad_chromatic(0.2, 0.0), wl.multipole(2, 0.1, 0.05), wl.monitor()]
+    desc = wl.lattice(els)
+    ref, ref_rec = oracle.push(desc, x)
+    got, rec = gpu_push(hb, desc, x, run_mode="composed", moments=True)
+    assert np.all(np.isfinite(got))
+    assert rel_err(got, ref).max() <= 1e-6
+    diag = [6, 12, 17, 21, 24, 26]
+    assert np.allclose(rec[0][diag], ref_rec[0][diag], rtol=1e-4)
+    # chromaticity is visible: the linear cell differs at the per-cent level for this momentum spread
+    lin_els = wl.fodo_cell(1.2) + [wl.drift(0.2), wl.monitor()]
+    lin, _ = oracle.push(wl.lattice(lin_els), x)
+    assert rel_err(lin, ref).max() > 1e-2
+    # first-order limit on the device
+    small = wl.gaussian_bunch(10_000, 31, sigma=np.array([1e-6, 1e-7, 1e-6, 1e-7, 1e-6, 1e-9]))
+    chrom = [wl.drift_exact(0.25), wl.quad_chromatic(0.1, 1.2), wl.drift_exact(0.5), wl.quad_chromatic(0.1, -1.2),
+             wl.drift_exact(0.25)]
+    a, _ = gpu_push(hb, wl.lattice(chrom), small, moments=False)
+    b, _ = gpu_push(hb, wl.lattice(wl.fodo_cell(1.2)), small, moments=False)
+    assert np.max(np.abs(a - b) / b.std(axis=1)[:, None]) <= 2e-6
+
+
+def test_multipole_validation(hb):
+    h = hb.hb_lattice_create(1000.0, wl.ELECTRON_MEV)
+    hb.hb_lattice_add_multipole(h, 3, 1.0, 0.0)
+    for bad in ((0, 1.0, 0.0), (9, 1.0, 0.0), (2, float("nan"), 0.0)):
+        with pytest.raises(hb.HbError):
+            hb.hb_lattice_add_multipole(h, *bad)
+    with pytest.raises(hb.HbError):
+        hb.hb_lattice_add_element(h, 8, 0.0, 1.0)          # a multipole needs its own call
+    hb.hb_lattice_destroy(h)
