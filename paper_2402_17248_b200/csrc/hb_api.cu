@@ -618,7 +618,7 @@ static hb_status push_impl(hb_lattice* lat, float* x, float* px, float* y, float
             if (g.type == SEG_RUN) {
                 if (lat->run_mode == HB_RUN_COMPOSED && !g.nonlinear) e = hb_launch_run_composed(p, n, g.map, partials, &nblocks, s);
                 else e = hb_launch_run_sequential(p, n, lat->d_seq + g.seq_off, g.seq_cnt,
-                                                  lat->run_mode == HB_RUN_SEQUENTIAL_FP32 && !g.nonlinear, partials, &nblocks, s);
+                                                  lat->run_mode == HB_RUN_SEQUENTIAL_FP32, g.nonlinear, partials, &nblocks, s);
             } else if (g.type == SEG_SUR) {
                 e = g.tc ? hb_launch_sur_tc(p, n, g.sd, partials, &nblocks, lat->sm_count, s)
                          : hb_launch_sur_fp32(p, n, g.sd, partials, &nblocks, lat->sm_count, s);

@@ -71,7 +71,7 @@ struct HbParticles {
 cudaError_t hb_launch_run_composed(const HbParticles& p, size_t n, const HbRunMap& map,
                                    double* partials, int* nblocks_out, cudaStream_t s);
 cudaError_t hb_launch_run_sequential(const HbParticles& p, size_t n, const HbSeqElem* d_elems, int count,
-                                     bool fp32_regs, double* partials, int* nblocks_out, cudaStream_t s);
+                                     bool fp32_regs, bool nonlinear, double* partials, int* nblocks_out, cudaStream_t s);
 cudaError_t hb_launch_moments_partials(const HbParticles& p, size_t n, const double* pivot6_host,
                                        double* partials, int* nblocks_out, cudaStream_t s);
 // fixed-order sum of `nblocks` partials -> 27-double record (pivot added back to the means)

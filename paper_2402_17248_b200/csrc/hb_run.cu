@@ -71,7 +71,8 @@ hb_run_composed_kernel(HbParticles p, size_t n, const __grid_constant__ HbRunMap
 template <typename T>
 struct SeqElemT { T a[10]; int kind; };
 
-template <typename T>
+// NL: the run holds non-linear elements (kinds 3-5); the linear-only instantiation keeps the lean three-way branch
+template <typename T, bool NL>
 __device__ __forceinline__ void seq_apply(const SeqElemT<T>& e, T (&v)[6]) {
     // v = (x, px, y, py, t, pt); pt never changes (R2-R5x)
     if (e.kind == 0) {                 // drift R2
@@ -85,7 +86,7 @@ __device__ __forceinline__ void seq_apply(const SeqElemT<T>& e, T (&v)[6]) {
         v[2] = fma(e.a[4], y, e.a[5] * py);
         v[3] = fma(e.a[6], y, e.a[7] * py);
         v[4] = fma(e.a[8], v[5], v[4]);
-    } else if (e.kind == 3) {          // exact drift R2x (non-linear): a0 = L, a1 = 1/beta0
+    } else if (NL && e.kind == 3) {    // exact drift R2x (non-linear): a0 = L, a1 = 1/beta0
         // pz^2 = (1/beta0 - pt)^2 - 1/(beta0 gamma0)^2 - px^2 - py^2 = 1 - 2 pt/beta0 + pt^2 - px^2 - py^2
         const T px = v[1], py = v[3], pt = v[5];
         const T pz2 = fma(pt, pt - T(2) * e.a[1], T(1)) - fma(px, px, py * py);
@@ -93,7 +94,7 @@ __device__ __forceinline__ void seq_apply(const SeqElemT<T>& e, T (&v)[6]) {
         v[0] = fma(e.a[0] * ipz, px, v[0]);
         v[2] = fma(e.a[0] * ipz, py, v[2]);
         v[4] = fma(e.a[0], fma(e.a[1] - pt, ipz, -e.a[1]), v[4]);
-    } else if (e.kind == 4) {          // chromatic thick quad R3x (non-linear): a0 = L, a1 = k, a2 = 1/beta0
+    } else if (NL && e.kind == 4) {    // chromatic thick quad R3x (non-linear): a0 = L, a1 = k, a2 = 1/beta0
         const T L = e.a[0], k = e.a[1], pt = v[5];
         const T en = e.a[2] - pt;                                   // E / (p0 c)
         const T d1 = sqrt(fma(pt, pt - T(2) * e.a[2], T(1)));       // 1 + delta = |p| / p0
@@ -120,7 +121,7 @@ __device__ __forceinline__ void seq_apply(const SeqElemT<T>& e, T (&v)[6]) {
             }
         }
         v[4] += L * (en / d1 - e.a[2]) + en * I / (T(2) * d1 * d1 * d1);
-    } else if (e.kind == 5) {          // thin multipole kick R5x: a0 = kn/(m-1)!, a1 = ks/(m-1)!, a2 = m
+    } else if (NL && e.kind == 5) {    // thin multipole kick R5x: a0 = kn/(m-1)!, a1 = ks/(m-1)!, a2 = m
         const int m = (int)e.a[2];
         T zr = T(1), zi = T(0);
         for (int j = 1; j < m; ++j) {
@@ -138,7 +139,7 @@ __device__ __forceinline__ void seq_apply(const SeqElemT<T>& e, T (&v)[6]) {
     }
 }
 
-template <typename T, bool MOM>
+template <typename T, bool MOM, bool NL>
 __global__ void __launch_bounds__(RUN_THREADS, 2)
 hb_run_sequential_kernel(HbParticles p, size_t n, const HbSeqElem* __restrict__ elems, int count,
                          double* __restrict__ partials) {
@@ -185,7 +186,7 @@ hb_run_sequential_kernel(HbParticles p, size_t n, const HbSeqElem* __restrict__ 
             for (int i = 0; i < m; ++i) {
                 const SeqElemT<T> e = se[i];
 #pragma unroll
-                for (int k = 0; k < 4; ++k) seq_apply(e, v[k]);
+                for (int k = 0; k < 4; ++k) seq_apply<T, NL>(e, v[k]);
             }
         }
         if (active && !tail) {
@@ -307,15 +308,18 @@ cudaError_t hb_launch_run_composed(const HbParticles& p, size_t n, const HbRunMa
 }
 
 cudaError_t hb_launch_run_sequential(const HbParticles& p, size_t n, const HbSeqElem* d_elems, int count,
-                                     bool fp32_regs, double* partials, int* nblocks_out, cudaStream_t s) {
+                                     bool fp32_regs, bool nonlinear, double* partials, int* nblocks_out, cudaStream_t s) {
     const int grid = run_grid(n, partials != nullptr);
     if (nblocks_out) *nblocks_out = grid;
-    if (fp32_regs) {
-        if (partials) hb_run_sequential_kernel<float, true><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
-        else hb_run_sequential_kernel<float, false><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
+    if (nonlinear) {          // non-linear elements: fp64 registers only
+        if (partials) hb_run_sequential_kernel<double, true, true><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
+        else hb_run_sequential_kernel<double, false, true><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
+    } else if (fp32_regs) {
+        if (partials) hb_run_sequential_kernel<float, true, false><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
+        else hb_run_sequential_kernel<float, false, false><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
     } else {
-        if (partials) hb_run_sequential_kernel<double, true><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
-        else hb_run_sequential_kernel<double, false><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
+        if (partials) hb_run_sequential_kernel<double, true, false><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
+        else hb_run_sequential_kernel<double, false, false><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
     }
     return cudaGetLastError();
 }
