@@ -157,6 +157,17 @@ hb_status hb_push(hb_lattice *lat, float *x, float *px, float *y, float *py, flo
 hb_status hb_push_moments(hb_lattice *lat, float *x, float *px, float *y, float *py, float *t, float *pt,
                           size_t n, double *d_moments, void *cuda_stream);
 
+/* Push a bunch that lives in HOST memory (six arrays of n floats; page-locked memory makes the copies asynchronous).
+ * The library stages it through device buffers it owns (allocated at the first call, kept until destroy) in `chunks`
+ * pieces through a three-stage pipeline (internal copy-in, compute and copy-out streams, three staging slots): the
+ * host->device copy of piece i+1 and the device->host copy of piece i-1 overlap the kernels of piece i.  Every particle goes through exactly the kernels of hb_push_moments; the
+ * moment partials of all pieces are summed by the same finalize kernel, so each record is the record of the whole
+ * bunch.  In place: the host arrays hold the result on return.  h_moments: host, num_monitors x 27 doubles, or NULL.
+ * chunks: 1..8.  SYNCHRONOUS (returns when the result is in host memory); n = 0 is a no-op (NaN records).
+ * Errors: as hb_push_moments (the 16-byte alignment requirement does not apply to host arrays). */
+hb_status hb_push_host(hb_lattice *lat, float *x, float *px, float *y, float *py, float *t, float *pt,
+                       size_t n, double *h_moments, int chunks);
+
 /* Standalone moments of a bunch (R10).  pivot: 6 HOST doubles subtracted before accumulation (any
  * value near the bunch centre; NULL = zeros); the result does not depend on it beyond rounding.
  * d_out27: DEVICE, 27 doubles.  d_scratch: DEVICE scratch of hb_moments_scratch_bytes() bytes. */

@@ -21,7 +21,7 @@ EXPORTED_SYMBOLS = [
     "hb_lattice_create", "hb_lattice_add_element", "hb_lattice_add_multipole", "hb_lattice_add_surrogate",
     "hb_lattice_set_run_mode",
     "hb_lattice_finalize", "hb_lattice_num_monitors", "hb_lattice_num_launches", "hb_lattice_ref_bg_out",
-    "hb_push", "hb_push_moments", "hb_moments", "hb_moments_scratch_bytes", "hb_lattice_destroy",
+    "hb_push", "hb_push_moments", "hb_push_host", "hb_moments", "hb_moments_scratch_bytes", "hb_lattice_destroy",
     "hb_lattice_enable_timing", "hb_lattice_get_timing",
     "hb_status_string", "hb_last_error", "hb_version", "hb_surrogate_kernel",
 ]
@@ -79,6 +79,7 @@ def lib():
     L.hb_lattice_ref_bg_out.argtypes = [c_void_p, POINTER(c_double)]
     L.hb_push.argtypes = [c_void_p] + [c_void_p] * 6 + [c_size_t, c_void_p]
     L.hb_push_moments.argtypes = [c_void_p] + [c_void_p] * 6 + [c_size_t, c_void_p, c_void_p]
+    L.hb_push_host.argtypes = [c_void_p] + [c_void_p] * 6 + [c_size_t, c_void_p, c_int]
     L.hb_moments.argtypes = [c_void_p] * 6 + [c_size_t, POINTER(c_double), c_void_p, c_void_p, c_void_p]
     L.hb_moments_scratch_bytes.restype = c_size_t
     L.hb_moments_scratch_bytes.argtypes = []
@@ -206,6 +207,11 @@ def hb_push(lat, x, px, y, py, t, pt, n: int, cuda_stream: int = 0):
 
 def hb_push_moments(lat, x, px, y, py, t, pt, n: int, d_moments: int, cuda_stream: int = 0):
     _check(lib().hb_push_moments(lat, x, px, y, py, t, pt, n, d_moments, cuda_stream), "hb_push_moments")
+
+
+def hb_push_host(lat, x, px, y, py, t, pt, n: int, h_moments: int, chunks: int = 4):
+    """x..pt, h_moments: HOST addresses (h_moments may be 0)"""
+    _check(lib().hb_push_host(lat, x, px, y, py, t, pt, n, h_moments, int(chunks)), "hb_push_host")
 
 
 def hb_moments_scratch_bytes() -> int:
@@ -341,6 +347,17 @@ class Lattice:
             out = torch.empty((m, 27), dtype=torch.float64, device=rows[0].device)
         hb_push_moments(self._h, *[r.data_ptr() for r in rows], n, out.data_ptr(), _stream(rows[0].device))
         return out
+
+    def push_host(self, host_coords, chunks=4, moments=True):
+        """host_coords: CPU float32 tensor or numpy array [6, n] (C-contiguous rows; pinned memory overlaps the copies);
+        pushed in place through hb_push_host; returns the [num_monitors, 27] records (numpy) or None"""
+        import numpy as np
+        rows = [host_coords[j] for j in range(6)]
+        n = int(rows[0].shape[0])
+        ptrs = [int(r.data_ptr()) if hasattr(r, "data_ptr") else int(r.ctypes.data) for r in rows]
+        rec = np.empty((self.num_monitors, 27), dtype=np.float64) if (moments and self.num_monitors) else None
+        hb_push_host(self._h, *ptrs, n, 0 if rec is None else rec.ctypes.data, chunks)
+        return rec
 
     def enable_timing(self, on=True):
         hb_lattice_enable_timing(self._h, on)

@@ -223,6 +223,13 @@ struct hb_lattice {
     bool timing = false;
     bool timing_valid = false;
     std::vector<cudaEvent_t> events;   // segs.size() + 1 when timing is on
+    // hb_push_host: staging owned by the library, allocated at the first call and kept
+    size_t host_chunk_cap = 0;         // particles per staging slot
+    float* d_stage[3] = {nullptr, nullptr, nullptr};   // three staging slots: copy-in / compute / copy-out in flight
+    double* d_host_partials = nullptr; // n_monitors partial buffers (one row range per chunk)
+    double* d_host_records = nullptr;  // n_monitors x 27
+    cudaStream_t host_streams[3] = {nullptr, nullptr, nullptr};   // copy-in, compute, copy-out
+    cudaEvent_t host_events[9] = {};   // per slot: copied in, computed, copied out
 };
 
 extern "C" {
@@ -583,6 +590,40 @@ static hb_status check_arrays(const float* const a[6], size_t n) {
     return HB_OK;
 }
 
+// Enqueue every segment of the lattice for the particles p[0..n) on stream s.
+//   host_partials == nullptr : moment partials go to lat->d_partials and each record is finalized at once into d_moments
+//   host_partials != nullptr : (hb_push_host, one call per chunk) the partials of monitor m go to rows
+//                              [row_off, row_off + blocks) of host_partials + m * 27 * HB_MOM_MAX_BLOCKS; no finalize
+static hb_status enqueue_segments(hb_lattice* lat, const HbParticles& p, size_t n, bool want_moments, double* d_moments,
+                                  double* host_partials, size_t row_off, bool timing, cudaStream_t s) {
+    hb_status st = HB_OK;
+    for (size_t k = 0; k < lat->segs.size() && st == HB_OK; ++k) {
+        const Segment& g = lat->segs[k];
+        const bool mom = want_moments && g.monitor >= 0;
+        double* partials = nullptr;
+        if (mom) partials = host_partials ? host_partials + (size_t)g.monitor * HB_NMOM * HB_MOM_MAX_BLOCKS + row_off : lat->d_partials;
+        int nblocks = 0;
+        cudaError_t e = cudaSuccess;
+        if (g.type == SEG_RUN) {
+            if (lat->run_mode == HB_RUN_COMPOSED && !g.nonlinear) e = hb_launch_run_composed(p, n, g.map, partials, &nblocks, s);
+            else e = hb_launch_run_sequential(p, n, lat->d_seq + g.seq_off, g.seq_cnt,
+                                              lat->run_mode == HB_RUN_SEQUENTIAL_FP32, g.nonlinear, partials, &nblocks, s);
+        } else if (g.type == SEG_SUR) {
+            e = g.tc ? hb_launch_sur_tc(p, n, g.sd, partials, &nblocks, lat->sm_count, s)
+                     : hb_launch_sur_fp32(p, n, g.sd, partials, &nblocks, lat->sm_count, s);
+        } else if (mom) {
+            e = hb_launch_moments_partials(p, n, nullptr, partials, &nblocks, s);
+        }
+        if (e != cudaSuccess) { st = fail(HB_ERR_CUDA, "kernel launch (segment %zu): %s", k, cudaGetErrorString(e)); break; }
+        if (mom && !host_partials) {
+            e = hb_launch_moments_finalize(partials, nblocks, n, nullptr, d_moments + (size_t)g.monitor * HB_NMOM, s);
+            if (e != cudaSuccess) st = fail(HB_ERR_CUDA, "moments finalize: %s", cudaGetErrorString(e));
+        }
+        if (timing) cudaEventRecord(lat->events[k + 1], s);
+    }
+    return st;
+}
+
 static hb_status push_impl(hb_lattice* lat, float* x, float* px, float* y, float* py, float* t, float* pt, size_t n,
                            double* d_moments, bool want_moments, void* stream) {
     if (!lat) return fail(HB_ERR_INVALID_ARG, "lattice is NULL");
@@ -609,29 +650,7 @@ static hb_status push_impl(hb_lattice* lat, float* x, float* px, float* y, float
         const bool timing = lat->timing && lat->events.size() == lat->segs.size() + 1;
         lat->timing_valid = false;
         if (timing) cudaEventRecord(lat->events[0], s);
-        for (size_t k = 0; k < lat->segs.size() && st == HB_OK; ++k) {
-            const Segment& g = lat->segs[k];
-            const bool mom = want_moments && g.monitor >= 0;
-            double* partials = mom ? lat->d_partials : nullptr;
-            int nblocks = 0;
-            cudaError_t e = cudaSuccess;
-            if (g.type == SEG_RUN) {
-                if (lat->run_mode == HB_RUN_COMPOSED && !g.nonlinear) e = hb_launch_run_composed(p, n, g.map, partials, &nblocks, s);
-                else e = hb_launch_run_sequential(p, n, lat->d_seq + g.seq_off, g.seq_cnt,
-                                                  lat->run_mode == HB_RUN_SEQUENTIAL_FP32, g.nonlinear, partials, &nblocks, s);
-            } else if (g.type == SEG_SUR) {
-                e = g.tc ? hb_launch_sur_tc(p, n, g.sd, partials, &nblocks, lat->sm_count, s)
-                         : hb_launch_sur_fp32(p, n, g.sd, partials, &nblocks, lat->sm_count, s);
-            } else if (mom) {
-                e = hb_launch_moments_partials(p, n, nullptr, partials, &nblocks, s);
-            }
-            if (e != cudaSuccess) { st = fail(HB_ERR_CUDA, "kernel launch (segment %zu): %s", k, cudaGetErrorString(e)); break; }
-            if (mom) {
-                e = hb_launch_moments_finalize(partials, nblocks, n, nullptr, d_moments + (size_t)g.monitor * HB_NMOM, s);
-                if (e != cudaSuccess) st = fail(HB_ERR_CUDA, "moments finalize: %s", cudaGetErrorString(e));
-            }
-            if (timing) cudaEventRecord(lat->events[k + 1], s);
-        }
+        st = enqueue_segments(lat, p, n, want_moments, d_moments, nullptr, 0, timing, s);
         if (timing && st == HB_OK) lat->timing_valid = true;
     }
     if (prev != lat->device) cudaSetDevice(prev);
@@ -645,6 +664,112 @@ hb_status hb_push(hb_lattice* lat, float* x, float* px, float* y, float* py, flo
 hb_status hb_push_moments(hb_lattice* lat, float* x, float* px, float* y, float* py, float* t, float* pt, size_t n,
                           double* d_moments, void* stream) {
     return push_impl(lat, x, px, y, py, t, pt, n, d_moments, true, stream);
+}
+
+// ---- host-resident bunch: H2D, push, D2H pipelined in chunks over two internal streams ------------------------
+hb_status hb_push_host(hb_lattice* lat, float* x, float* px, float* y, float* py, float* t, float* pt, size_t n,
+                       double* h_moments, int chunks) {
+    if (!lat) return fail(HB_ERR_INVALID_ARG, "lattice is NULL");
+    if (!lat->finalized) return fail(HB_ERR_STATE, "lattice not finalized");
+    if (chunks < 1 || chunks > HB_MOM_MAX_BLOCKS / HB_MOM_GRID_MAX)
+        return fail(HB_ERR_INVALID_ARG, "chunks must be 1..%d", HB_MOM_MAX_BLOCKS / HB_MOM_GRID_MAX);
+    float* host[6] = {x, px, y, py, t, pt};
+    if (n > 0) {
+        const float* arr[6] = {x, px, y, py, t, pt};
+        for (int j = 0; j < 6; ++j)
+            if (!arr[j]) return fail(HB_ERR_INVALID_ARG, "particle array %d is NULL", j);
+        const size_t bytes = n * sizeof(float);
+        for (int j = 0; j < 6; ++j)
+            for (int k = j + 1; k < 6; ++k) {
+                const uintptr_t a0 = (uintptr_t)arr[j], b0 = (uintptr_t)arr[k];
+                if (a0 < b0 + bytes && b0 < a0 + bytes) return fail(HB_ERR_INVALID_ARG, "particle arrays %d and %d overlap", j, k);
+            }
+    }
+    const bool want = h_moments != nullptr && lat->n_monitors > 0;
+    if (n == 0) {
+        if (want) std::memset(h_moments, 0xff, (size_t)lat->n_monitors * HB_NMOM * sizeof(double));   // NaN records
+        return HB_OK;
+    }
+    int prev = 0;
+    HB_CUDA(cudaGetDevice(&prev));
+    if (prev != lat->device) HB_CUDA(cudaSetDevice(lat->device));
+    // particles per chunk: whole 256-particle tile pairs, 16-byte aligned device rows
+    size_t chunk_n = (n + (size_t)chunks - 1) / (size_t)chunks;
+    chunk_n = (chunk_n + 255) / 256 * 256;
+    hb_status st = HB_OK;
+    // ---- resources, once (and again if a larger chunk is asked for)
+    if (!lat->host_streams[0]) {
+        for (int i = 0; i < 3 && st == HB_OK; ++i)
+            if (cudaStreamCreateWithFlags(&lat->host_streams[i], cudaStreamNonBlocking) != cudaSuccess)
+                st = fail(HB_ERR_CUDA, "stream creation failed");
+        for (int i = 0; i < 9 && st == HB_OK; ++i)
+            if (cudaEventCreateWithFlags(&lat->host_events[i], cudaEventDisableTiming) != cudaSuccess)
+                st = fail(HB_ERR_CUDA, "event creation failed");
+        if (st == HB_OK && lat->n_monitors > 0) {
+            void* d = nullptr;
+            st = upload(lat, nullptr, (size_t)lat->n_monitors * HB_NMOM * HB_MOM_MAX_BLOCKS * sizeof(double), &d);
+            lat->d_host_partials = (double*)d;
+            if (st == HB_OK) st = upload(lat, nullptr, (size_t)lat->n_monitors * HB_NMOM * sizeof(double), &d);
+            lat->d_host_records = (double*)d;
+        }
+    }
+    if (st == HB_OK && chunk_n > lat->host_chunk_cap) {
+        for (int i = 0; i < 3 && st == HB_OK; ++i) {
+            void* d = nullptr;
+            st = upload(lat, nullptr, 6 * chunk_n * sizeof(float), &d);     // (a smaller old buffer stays in d_bufs)
+            lat->d_stage[i] = (float*)d;
+        }
+        if (st == HB_OK) lat->host_chunk_cap = chunk_n;
+    }
+    if (st == HB_OK) {
+        // three-stage pipeline over three staging slots: the copy engine of each direction and the SMs each work
+        // on a different piece; events hand a slot from stage to stage
+        cudaStream_t sin = lat->host_streams[0], scmp = lat->host_streams[1], sout = lat->host_streams[2];
+        cudaEvent_t* ev_in = lat->host_events;          // [slot] piece copied in
+        cudaEvent_t* ev_k = lat->host_events + 3;       // [slot] piece computed
+        cudaEvent_t* ev_out = lat->host_events + 6;     // [slot] piece copied out (slot free again)
+        cudaError_t e = cudaSuccess;
+        if (want)        // rows a piece does not write must read as zero in the finalize
+            e = cudaMemsetAsync(lat->d_host_partials, 0, (size_t)lat->n_monitors * HB_NMOM * HB_MOM_MAX_BLOCKS * sizeof(double), scmp);
+        size_t off = 0;
+        int pieces = 0;
+        for (int c = 0; c < chunks && off < n && st == HB_OK && e == cudaSuccess; ++c, ++pieces) {
+            const size_t nc = n - off < chunk_n ? n - off : chunk_n;
+            const int slot = c % 3;
+            float* base = lat->d_stage[slot];
+            HbParticles p;
+            if (c >= 3) e = cudaStreamWaitEvent(sin, ev_out[slot], 0);
+            for (int j = 0; j < 6 && e == cudaSuccess; ++j) {
+                p.v[j] = base + (size_t)j * lat->host_chunk_cap;
+                e = cudaMemcpyAsync(p.v[j], host[j] + off, nc * sizeof(float), cudaMemcpyHostToDevice, sin);
+            }
+            if (e == cudaSuccess) e = cudaEventRecord(ev_in[slot], sin);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(scmp, ev_in[slot], 0);
+            if (e != cudaSuccess) break;
+            st = enqueue_segments(lat, p, nc, want, nullptr, want ? lat->d_host_partials : nullptr,
+                                  (size_t)c * HB_MOM_GRID_MAX, false, scmp);
+            if (st != HB_OK) break;
+            e = cudaEventRecord(ev_k[slot], scmp);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(sout, ev_k[slot], 0);
+            for (int j = 0; j < 6 && e == cudaSuccess; ++j)
+                e = cudaMemcpyAsync(host[j] + off, p.v[j], nc * sizeof(float), cudaMemcpyDeviceToHost, sout);
+            if (e == cudaSuccess) e = cudaEventRecord(ev_out[slot], sout);
+            off += nc;
+        }
+        if (e == cudaSuccess && st == HB_OK && want) {
+            for (int m = 0; m < lat->n_monitors && e == cudaSuccess; ++m)
+                e = hb_launch_moments_finalize(lat->d_host_partials + (size_t)m * HB_NMOM * HB_MOM_MAX_BLOCKS,
+                                               pieces * HB_MOM_GRID_MAX, n, nullptr, lat->d_host_records + (size_t)m * HB_NMOM, scmp);
+            if (e == cudaSuccess)
+                e = cudaMemcpyAsync(h_moments, lat->d_host_records, (size_t)lat->n_monitors * HB_NMOM * sizeof(double),
+                                    cudaMemcpyDeviceToHost, scmp);
+        }
+        const cudaError_t e1 = cudaStreamSynchronize(sin), e2 = cudaStreamSynchronize(scmp), e3 = cudaStreamSynchronize(sout);
+        if (e == cudaSuccess) e = e1 != cudaSuccess ? e1 : (e2 != cudaSuccess ? e2 : e3);
+        if (e != cudaSuccess && st == HB_OK) st = fail(HB_ERR_CUDA, "hb_push_host: %s", cudaGetErrorString(e));
+    }
+    if (prev != lat->device) cudaSetDevice(prev);
+    return st;
 }
 
 size_t hb_moments_scratch_bytes(void) { return (size_t)HB_MOM_MAX_BLOCKS * HB_NMOM * sizeof(double); }
@@ -703,6 +828,10 @@ hb_status hb_lattice_destroy(hb_lattice* lat) {
         cudaSetDevice(lat->device);
         cudaDeviceSynchronize();
         for (auto& ev : lat->events) cudaEventDestroy(ev);
+        for (int i = 0; i < 9; ++i)
+            if (lat->host_events[i]) cudaEventDestroy(lat->host_events[i]);
+        for (int i = 0; i < 3; ++i)
+            if (lat->host_streams[i]) cudaStreamDestroy(lat->host_streams[i]);
         for (void* p : lat->d_bufs) cudaFree(p);
         cudaSetDevice(prev);
     }

@@ -8,7 +8,8 @@
 #define HB_MAX_LINEAR 12      // L_0 .. L_l, l <= 11 hidden layers
 #define HB_MAX_WIDTH 1024
 #define HB_NMOM 27            // 6 first + 21 second moments
-#define HB_MOM_MAX_BLOCKS 2368  // 148 SMs x 16: upper bound on blocks that write moment partials
+#define HB_MOM_GRID_MAX 592    // 148 SMs x 4: most blocks one launch writes moment partials from
+#define HB_MOM_MAX_BLOCKS 4736  // rows of a partials buffer: 8 launches (hb_push_host: one per chunk) x HB_MOM_GRID_MAX
 
 // ---- conventional runs -------------------------------------------------------------------
 struct HbRunMap {             // composed run: v' = M v (row-major 6x6, fp32, built in fp64 on the host)

@@ -291,7 +291,7 @@ static int run_grid(size_t n, bool moments) {
     const size_t nq = (n >> 2) + ((n & 3) ? 1 : 0);
     size_t blocks = (nq + RUN_THREADS - 1) / RUN_THREADS;
     if (blocks < 1) blocks = 1;
-    const size_t cap = moments ? HB_MOM_MAX_BLOCKS / 4 : 148 * 32;   // moments: 592 = 148 x 4 (2 resident x 2 waves)
+    const size_t cap = moments ? HB_MOM_GRID_MAX : 148 * 32;   // moments: 592 = 148 x 4 (2 resident x 2 waves)
     if (blocks > cap) blocks = cap;
     return (int)blocks;
 }

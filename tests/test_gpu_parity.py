@@ -423,3 +423,56 @@ def test_multipole_validation(hb):
     with pytest.raises(hb.HbError):
         hb.hb_lattice_add_element(h, 8, 0.0, 1.0)          # a multipole needs its own call
     hb.hb_lattice_destroy(h)
+
+
+# ------------------------------------------------------------------ hb_push_host: host-resident bunch, chunked pipeline
+@pytest.mark.parametrize("chunks", [1, 2, 3, 8])
+@pytest.mark.parametrize("n", [1, 255, 70_001])
+def test_push_host_equals_device_push(hb, chunks, n):
+    """the host entry point runs the same kernels piece by piece: coordinates bit-identical to hb_push_moments on the
+    whole bunch, records equal up to the summation order of the partials"""
+    import torch
+    desc, x = wl.config1(prec="f16", n=max(n, 8))
+    x = np.ascontiguousarray(x[:, :n])
+    lat = hb.Lattice.from_description(desc, device=0)
+    c = hb.to_device(x)
+    rec_dev = lat.push_moments(c)
+    torch.cuda.synchronize()
+    dev = hb.to_host(c)
+    host = torch.from_numpy(x.copy()).pin_memory()
+    rec_host = lat.push_host(host, chunks=chunks)
+    assert np.array_equal(host.numpy(), dev)
+    r = rec_dev.cpu().numpy()
+    assert np.allclose(rec_host[:, :6], r[:, :6], rtol=1e-12, atol=1e-18)
+    if n > 1:
+        diag = [6, 12, 17, 21, 24, 26]
+        assert np.allclose(rec_host[:, diag], r[:, diag], rtol=1e-10)
+    # pageable numpy memory works too (copies are then synchronous), and so does a second call on the same lattice
+    again = x.copy()
+    rec2 = lat.push_host(again, chunks=chunks)
+    assert np.array_equal(again, dev) and np.allclose(rec2[:, :6], r[:, :6], rtol=1e-12, atol=1e-18)
+    lat.close()
+
+
+def test_push_host_vs_oracle_and_errors(hb):
+    import torch
+    desc, x = wl.config4(prec="f16", n=120_000)
+    ref, ref_rec = oracle.push(desc, x)
+    lat = hb.Lattice.from_description(desc, device=0)
+    host = torch.from_numpy(x.copy()).pin_memory()
+    rec = lat.push_host(host, chunks=4)
+    got = host.numpy().astype(np.float64)
+    assert rel_err(got, ref).max() <= 5e-2
+    own = oracle.moments(np.ascontiguousarray(got))
+    assert np.allclose(rec[-1][:6], own[:6], rtol=1e-9, atol=1e-16)
+    diag = [6, 12, 17, 21, 24, 26]
+    assert np.allclose(rec[-1][diag], own[diag], rtol=1e-9)
+    assert lat.push_host(host, chunks=2, moments=False) is None
+    with pytest.raises(hb.HbError):
+        lat.push_host(host, chunks=0)
+    with pytest.raises(hb.HbError):
+        lat.push_host(host, chunks=9)
+    empty = np.zeros((6, 0), np.float32)
+    r0 = lat.push_host(empty, chunks=1)
+    assert np.all(np.isnan(r0))
+    lat.close()
