@@ -650,7 +650,7 @@ static hb_status push_impl(hb_lattice* lat, float* x, float* px, float* y, float
         const bool timing = lat->timing && lat->events.size() == lat->segs.size() + 1;
         lat->timing_valid = false;
         if (timing) cudaEventRecord(lat->events[0], s);
-        st = enqueue_segments(lat, p, n, want_moments, d_moments, nullptr, 0, timing, s);
+        if (st == HB_OK) st = enqueue_segments(lat, p, n, want_moments, d_moments, nullptr, 0, timing, s);
         if (timing && st == HB_OK) lat->timing_valid = true;
     }
     if (prev != lat->device) cudaSetDevice(prev);
