@@ -476,3 +476,38 @@ def test_push_host_vs_oracle_and_errors(hb):
     r0 = lat.push_host(empty, chunks=1)
     assert np.all(np.isnan(r0))
     lat.close()
+
+
+def test_lens_optimisation_loop_on_the_gpu(hb):
+    """NEXT-4 in miniature (the paper's headline use is an optimiser around the beamline): Nelder-Mead
+    over the strengths of two plasma lenses, every objective evaluation = one lattice build + one hb_push_moments of
+    a 1e5-particle bunch on the GPU; the optimum is then checked with the fp64 oracle"""
+    import torch
+    from scipy.optimize import minimize
+    x = wl.gaussian_bunch(100_000, 37, sigma=np.array([1e-3, 1e-3, 1e-3, 1e-3, 1e-3, 1e-3]))
+    c0 = torch.from_numpy(x).cuda()
+    work = torch.empty_like(c0)
+
+    def line(k):
+        return wl.lattice([wl.drift(0.5), wl.plens(0.05, k[0]), wl.drift(1.0), wl.plens(0.05, k[1]), wl.drift(0.7), wl.monitor()])
+
+    evals = []
+
+    def objective(k):
+        lat = hb.Lattice.from_description(line(k), device=0)
+        work.copy_(c0)
+        rec = lat.push_moments(work).cpu().numpy()[-1]
+        lat.close()
+        evals.append(1)
+        return float(rec[6] + rec[17])                 # sigma_x^2 + sigma_y^2 at the end of the line
+
+    start = np.array([1.0, 1.0])
+    f0 = objective(start)
+    res = minimize(objective, start, method="Nelder-Mead", options={"xatol": 1e-3, "fatol": 1e-12, "maxfev": 200})
+    assert res.fun < 0.2 * f0 and len(evals) > 20          # the lenses really focus the beam
+    ref, ref_rec = oracle.push(line(res.x), x)
+    f_ref = ref_rec[-1][6] + ref_rec[-1][17]
+    assert abs(res.fun - f_ref) <= 1e-4 * f_ref            # the GPU objective at the optimum is the oracle's
+    for dk in ([0.3, 0.0], [0.0, -0.3]):                   # and it is a (local) minimum of the oracle's objective too
+        _, r2 = oracle.push(line(res.x + np.array(dk)), x)
+        assert r2[-1][6] + r2[-1][17] >= f_ref * (1 - 1e-6)
