@@ -63,7 +63,9 @@ typedef enum { HB_ACT_IDENTITY = 0, HB_ACT_RELU = 1, HB_ACT_PRELU = 2, HB_ACT_TA
 /* Arithmetic of the MLP layers.  FP32: CUDA-core FFMA.  BF16/F16/TF32: tcgen05 tensor cores with
  * operands rounded to that type and fp32 accumulation in TMEM.  Shapes: BF16/F16 any hidden widths <= 256
  * whose 16-bit weights fit in shared memory (resident kernel), else equal hidden widths <= 512 (weights
- * streamed from L2); TF32 (half the tensor rate): at least one hidden layer, equal hidden widths <= 256.
+ * streamed from L2), else equal hidden widths <= 1024 (one launch per layer, activations through a 2-4 GB global
+ * scratch allocated at finalize; bunches up to 3.3e7 particles per push); TF32 (half the tensor rate): at least one
+ * hidden layer, equal hidden widths <= 256.
  * Anything else: hb_lattice_finalize returns HB_ERR_UNSUPPORTED -- never a slower fallback. */
 typedef enum { HB_PREC_FP32 = 0, HB_PREC_BF16 = 1, HB_PREC_F16 = 2, HB_PREC_TF32 = 3 } hb_prec;
 
@@ -193,7 +195,8 @@ const char *hb_version(void);
 
 /* Which kernel a surrogate stage of this shape runs on (host-only query, no device needed; the same decision
  * hb_lattice_finalize takes): "fp32-ffma", "tcgen05-resident" (16-bit weights resident in shared memory),
- * "tcgen05-streamed" (weights streamed from L2; also every HB_PREC_TF32 stage), or NULL when the shape has no
+ * "tcgen05-streamed" (weights streamed from L2; also every HB_PREC_TF32 stage), "tcgen05-layered" (hidden widths
+ * 513..1024: one launch per layer, activations through a global scratch the lattice owns), or NULL when the shape has no
  * schedule (hb_lattice_finalize would return HB_ERR_UNSUPPORTED; reason in hb_last_error()).
  * widths: n_linear + 1 entries, 6, H_1, ..., 6.  The returned string is static. */
 const char *hb_surrogate_kernel(hb_prec prec, int n_linear, const int *widths);

@@ -257,7 +257,8 @@ const char* hb_surrogate_kernel(hb_prec prec, int n_linear, const int* widths) {
     if (prec == HB_PREC_FP32) return "fp32-ffma";
     char why[256];
     if (!hb_tc_supported((int)prec, n_linear, widths, why, sizeof why)) { fail(HB_ERR_UNSUPPORTED, "tensor-core surrogate: %s", why); return nullptr; }
-    return hb_tc_kernel_kind((int)prec, n_linear, widths) == 2 ? "tcgen05-streamed" : "tcgen05-resident";
+    const int kind = hb_tc_kernel_kind((int)prec, n_linear, widths);
+    return kind == 3 ? "tcgen05-layered" : (kind == 2 ? "tcgen05-streamed" : "tcgen05-resident");
 }
 
 hb_status hb_lattice_create(double kin, double rest, hb_lattice** out) {
@@ -456,6 +457,12 @@ static hb_status build_surrogate(hb_lattice* lat, const SurHost& s, double bg_in
         sd.wtc = dw;
         sd.btc = (const float*)db;
         sd.tc_kind = hb_tc_kernel_kind(s.prec, s.n_linear, s.widths.data());   // the image above is this kernel's
+        if (sd.tc_kind == 3) {      // wide net: activations of a chunk round-trip through global scratch
+            void* da = nullptr;
+            st = upload(lat, nullptr, hb_tcw_scratch_bytes(s.n_linear, s.widths.data()), &da);
+            if (st != HB_OK) return st;
+            sd.act_scratch = (unsigned char*)da;
+        }
         seg.tc = true;
     }
     return HB_OK;
@@ -609,8 +616,9 @@ static hb_status enqueue_segments(hb_lattice* lat, const HbParticles& p, size_t 
             else e = hb_launch_run_sequential(p, n, lat->d_seq + g.seq_off, g.seq_cnt,
                                               lat->run_mode == HB_RUN_SEQUENTIAL_FP32, g.nonlinear, partials, &nblocks, s);
         } else if (g.type == SEG_SUR) {
-            e = g.tc ? hb_launch_sur_tc(p, n, g.sd, partials, &nblocks, lat->sm_count, s)
-                     : hb_launch_sur_fp32(p, n, g.sd, partials, &nblocks, lat->sm_count, s);
+            if (g.tc && g.sd.tc_kind == 3) e = hb_launch_sur_tcw(p, n, g.sd, partials, host_partials != nullptr, &nblocks, lat->sm_count, s);
+            else e = g.tc ? hb_launch_sur_tc(p, n, g.sd, partials, &nblocks, lat->sm_count, s)
+                          : hb_launch_sur_fp32(p, n, g.sd, partials, &nblocks, lat->sm_count, s);
         } else if (mom) {
             e = hb_launch_moments_partials(p, n, nullptr, partials, &nblocks, s);
         }

@@ -61,6 +61,7 @@ struct HbSurDev {             // passed by value to the surrogate kernels
     int kpad[HB_MAX_LINEAR];  // padded fan-in  (multiple of 64 elements; layer 0: 64)
     int npadtc[HB_MAX_LINEAR];// padded fan-out (multiple of 16; hidden: multiple of 64)
     int tc_kind;              // which tensor-core kernel the image was packed for (hb_tc_kernel_kind, fixed at finalize)
+    unsigned char* act_scratch;   // wide nets (hb_sur_tcw.cu): two pre-tiled activation buffers of one chunk
 };
 
 struct HbParticles {
@@ -97,5 +98,14 @@ cudaError_t hb_launch_sur_tcs(const HbParticles& p, size_t n, const HbSurDev& sd
 bool hb_tc2_supported(int n_linear, const int* widths);
 cudaError_t hb_launch_sur_tc2(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials,
                               int* nblocks_out, int sm_count, cudaStream_t s);
-// 0: no tensor-core schedule for this shape, 1: weights resident (hb_sur_tc.cu), 2: weights streamed (hb_sur_tcs.cu)
+// 0: no tensor-core schedule for this shape, 1: weights resident (hb_sur_tc.cu), 2: weights streamed (hb_sur_tcs.cu),
+// 3: wide nets, one launch per layer, activations through global scratch (hb_sur_tcw.cu)
 int hb_tc_kernel_kind(int prec, int n_linear, const int* widths);
+// wide nets (hidden width 513..1024, equal widths; bf16 / f16): hb_sur_tcw.cu
+#define HB_TCW_CHUNK (1 << 20)        // particles per chunk (scratch: 2 buffers x chunk x padded width x 2 B)
+bool hb_tcw_supported(int prec, int n_linear, const int* widths);
+size_t hb_tcw_scratch_bytes(int n_linear, const int* widths);
+size_t hb_tcw_pack_weights(int prec, int n_linear, const int* widths, const float* const* W,
+                           void* dst, long long* off_bytes, int* kpad, int* npad);
+cudaError_t hb_launch_sur_tcw(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials, bool partials_zeroed,
+                              int* nblocks_out, int sm_count, cudaStream_t s);

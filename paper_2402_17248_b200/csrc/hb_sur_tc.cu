@@ -506,7 +506,8 @@ int hb_tc_kernel_kind(int prec, int n_linear, const int* widths) {
     if (use_stream(prec, n_linear, widths)) return 2;
     if (prec == 3) return 0;
     TcPlan pl;
-    return choose_cg(n_linear, widths, pl) ? 1 : 0;
+    if (choose_cg(n_linear, widths, pl)) return 1;
+    return hb_tcw_supported(prec, n_linear, widths) ? 3 : 0;
 }
 
 bool hb_tc_supported(int prec, int n_linear, const int* widths, char* why, size_t why_len) {
@@ -520,9 +521,9 @@ bool hb_tc_supported(int prec, int n_linear, const int* widths, char* why, size_
         return false;
     }
     TcPlan pl;
-    if (!choose_cg(n_linear, widths, pl) && !hb_tcs_supported(prec, n_linear, widths)) {
+    if (!choose_cg(n_linear, widths, pl) && !hb_tcs_supported(prec, n_linear, widths) && !hb_tcw_supported(prec, n_linear, widths)) {
         snprintf(why, why_len, "no tensor-core schedule for this shape: the weights do not fit resident in shared memory "
-                               "and the streamed kernel needs equal hidden widths <= 512");
+                               "and the streamed / layered kernels need equal hidden widths <= 512 / <= 1024");
         return false;
     }
     return true;
@@ -535,6 +536,7 @@ bool hb_tc_supported(int prec, int n_linear, const int* widths, char* why, size_
 size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float* const* W, void* dst,
                           long long* off_bytes, int* kpad, int* npad) {
     if (use_stream(prec, n_linear, widths)) return hb_tcs_pack_weights(prec, n_linear, widths, W, dst, off_bytes, kpad, npad);
+    if (hb_tc_kernel_kind(prec, n_linear, widths) == 3) return hb_tcw_pack_weights(prec, n_linear, widths, W, dst, off_bytes, kpad, npad);
     int ksteps[HB_MAX_LINEAR];
     layer_geometry(n_linear, widths, kpad, npad, ksteps);
     size_t total = 0;

@@ -260,3 +260,43 @@ def test_tf32_unsupported_shapes_fail_loudly(hb):
     z, o = np.zeros(6), np.ones(6)
     with pytest.raises(Exception):
         hb.Lattice.from_description(wl.lattice([wl.surrogate([6, 512, 512, 6], W, b, "tanh", z, o, z, o, prec="tf32")]), device=0)
+
+
+# ------------------------------------------------------------------ wide nets: one launch per layer (hb_sur_tcw.cu)
+@pytest.mark.parametrize("prec", ["bf16", "f16"])
+@pytest.mark.parametrize("H", [768, 1024])
+def test_tcw_bringup_identity_net(hb, prec, H):
+    """identity weights through the layered kernel: pre-tiled scratch, ring stages, output blocks, bulk stores"""
+    x = wl.gaussian_bunch(3000, 3, sigma=np.ones(6))
+    got, _ = gpu_push(hb, wl.lattice([identity_net(H, prec)]), x)
+    eps = 2.0 ** -8 if prec == "bf16" else 2.0 ** -11
+    assert np.all(np.isfinite(got))
+    assert np.max(np.abs(got - x) / np.maximum(np.abs(x), 1e-3)) <= 1.01 * eps
+
+
+@pytest.mark.parametrize("prec", ["bf16", "f16"])
+@pytest.mark.parametrize("act,widths,n", [("prelu", [6, 900, 900, 900, 900, 900, 6], 20_000), ("prelu", [6, 700, 700, 700, 6], 20_000),
+                                          ("tanh", [6, 520, 520, 6], 257), ("relu", [6, 1024, 6], 1),
+                                          ("relu", [6, 600, 600, 6], 40_001)])
+def test_tcw_shapes(hb, prec, act, widths, n):
+    """the paper's own network shapes (6-900^5-6, 6-700^3-6 PReLU) and the edges of the layered kernel"""
+    init = "he" if act in ("relu", "prelu") else "xavier"
+    W, b = wl.make_mlp(widths, init, 61, len(widths))
+    rng = np.random.default_rng(10)
+    a = rng.uniform(0.05, 0.3, len(widths) - 2).astype(np.float32) if act == "prelu" else None
+    full = wl.correlated_bunch(max(n, 8), 45)
+    x = full[:, :n].copy()
+    f64 = full.astype(np.float64)
+    sur = wl.surrogate(widths, W, b, act, f64.mean(axis=1), f64.std(axis=1), rng.normal(size=6),
+                       rng.uniform(0.5, 2.0, 6), prelu_a=a, prec=prec)
+    desc = wl.lattice([sur, wl.monitor()])
+    assert hb.hb_surrogate_kernel(prec, widths) == "tcgen05-layered"
+    ref, _ = oracle.push(desc, x)
+    got, rec = gpu_push(hb, desc, x, moments=True)
+    scale = ref.std(axis=1) if n > 1 else np.abs(sur["out_std"])
+    e = np.max(np.abs(got - ref), axis=1) / scale
+    print("layered shape", widths, act, prec, "max err/std", e.max())
+    assert np.all(np.isfinite(got))
+    assert e.max() <= TOL[prec]
+    own = oracle.moments(np.ascontiguousarray(got))
+    assert np.allclose(rec[0][:6], own[:6], rtol=1e-9, atol=1e-16)

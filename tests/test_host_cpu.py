@@ -105,8 +105,11 @@ def test_surrogate_kernel_dispatch_is_a_host_decision(hb, monkeypatch):
     assert K("bf16", [6, 6]) == "tcgen05-resident"                        # no hidden layer
     assert K("tf32", [6, 256, 256, 256, 6]) == "tcgen05-streamed"
     assert K("tf32", [6, 512, 512, 6]) is None and "TF32" in hb.hb_last_error()
-    assert K("bf16", [6, 900, 900, 900, 900, 900, 6]) is None             # NEXT-1 widths: no schedule yet
-    assert K("bf16", [6, 512, 300, 512, 6]) is None                       # streamed kernel: equal widths only
+    assert K("bf16", [6, 900, 900, 900, 900, 900, 6]) == "tcgen05-layered"   # the paper's own nets: one launch per layer
+    assert K("f16", [6, 700, 700, 700, 6]) == "tcgen05-layered"
+    assert K("tf32", [6, 700, 700, 700, 6]) is None and K("bf16", [6, 1100, 1100, 6]) is None
+    assert K("bf16", [6, 512, 300, 512, 6]) == "tcgen05-layered"          # unequal widths that pad to the same 256-multiple
+    assert K("bf16", [6, 512, 1024, 512, 6]) is None                      # streamed / layered kernels: equal padded widths only
     assert K("bf16", [6, 1025, 6]) is None and K("bf16", [5, 8, 6]) is None
     monkeypatch.setenv("HB_TC_FORCE_STREAM", "1")
     assert K("bf16", [6, 256, 256, 256, 6]) == "tcgen05-streamed"
