@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the hybrid-beamline hot path on B200 (one process per GPU).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3|C4|C2|C5] [--impl hb|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3|C4|C2|C5|P900|P700] [--impl hb|reference]
 
 A step = one hb_push_moments of the whole lattice of the workload over one resident bunch.  Default
 workload = BASELINE.json config 3 ("surrogate particles/s at 1e7; % of tensor peak": N = 1e7,
@@ -111,6 +111,10 @@ def build_workload(name, prec, n):
     elif name == "C5":
         desc, x = wl.config5(prec=prec, n=n or 100_000_000)
         label = "C5 large bunch: N=%d, 9 x surrogate 6-512^4-6 tanh %s + 8 x 10 FODO cells, 17 monitors"
+    elif name in ("P900", "P700"):
+        w, h = (900, 5) if name == "P900" else (700, 3)
+        desc, x = wl.paper_net(w, h, prec=prec, n=n or 10_000_000)
+        label = "%s the paper's own network shape (P:177): N=%%d, one stage 6-%d^%d-6 PReLU %%s, random He weights, monitor after stage" % (name, w, h)
     else:
         raise SystemExit("unknown workload " + name)
     return desc, x, label % (x.shape[1], prec)
@@ -442,7 +446,7 @@ def main():
         per = flops / max(n_sur, 1)
         ach = per * n / (dom_ms * 1e-3) / 1e12
         widest = max(max(e["widths"][1:-1]) for e in desc["elements"] if e["kind"] == "surrogate")
-        kname = "hb_sur_tcs_kernel" if widest > 256 else "hb_sur_tc_kernel"
+        kname = "hb_sur_tcw_kernel" if widest > 512 else ("hb_sur_tcs_kernel" if widest > 256 else "hb_sur_tc_kernel")
         roof = {"bound": "tensor", "achieved": ach, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
                 "frac": ach / pk["bf16_tflops"], "traffic": NCU_TRAFFIC.get((kname, n)), "kernel": kname,
                 "kernel_ms": dom_ms, "peak_source": pk["source"] + " (burst, cuBLAS bf16)",
@@ -454,9 +458,12 @@ def main():
                 "traffic": NCU_TRAFFIC.get(("hb_run_composed_kernel", n)), "kernel": "hb_run_composed_kernel",
                 "kernel_ms": dom_ms, "peak_source": pk["source"]}
 
+    # BASELINE.md holds the paper's number only for its own network shapes at N = 1e7 (P:199, 1 x A100: context)
+    paper_rate = {"P900": 1e7 / 1.12, "P700": 1e7 / 0.494}.get(args.workload) if n == 10_000_000 and world == 1 else None
     line = {
         "metric": METRIC, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": (value / paper_rate) if paper_rate else None,
         "dtype": args.prec if n_sur else "f32", "data": "synthetic (seeded; shapes of the paper's workloads, DESIGN.md)",
         "config": {"workload": label, "l2": "inputs (%d MB) exceed L2 and a 256 MB buffer is written between timed steps" % (24 * n // 1000000),
                    "timing": "CUDA events per step on the launching stream, summed; max over ranks", "parallelism": "particles sharded, no collective"},

@@ -14,6 +14,8 @@
 // Warp roles (16 warps): 0-3 IO, 4-11 epilogue, 12 idle, 13 producer (TMA ring), 14 relay, 15 MMA issuer.
 #include "hb_tc_common.cuh"
 
+#include <algorithm>
+
 namespace {
 
 constexpr int W_THREADS = 512;
@@ -33,9 +35,9 @@ enum : int {
 };
 
 struct TcwPlan {
-    int npad;             // padded hidden width, multiple of 256, <= 1024
+    int npad;             // padded hidden width, multiple of 64, <= 1024
     int ns;               // npad / 64  K slabs of a hidden operand
-    int nb;               // npad / 256 output blocks of a hidden layer
+    int nb;               // ceil(npad / 256) output blocks of a hidden layer: 256 columns each, the last one the rest
     int ring_off, stage_out_off, a0_off, bias_off, bar_off, red_off, total;
 };
 
@@ -110,8 +112,13 @@ hb_sur_tcw_kernel(HbParticles p, size_t n_chunk, const __grid_constant__ HbSurDe
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
-    // bytes of the weight part of a stage, and where the stages of this rank start in the image
-    const uint32_t w_bytes = ly.first ? 128u * 32u : (ly.last ? 1024u : 16384u);
+    // output block nb is 256 columns wide, the last one what is left of npad; this CTA holds half of its weight rows
+    auto blk_w = [&](int nb) -> int { return ly.last ? 16 : min(256, pl.npad - 256 * nb); };
+    // bytes of the weight part of a stage of block nb (full blocks precede the narrow one, so nb * full size = offset)
+    auto w_bytes_of = [&](int nb) -> uint32_t {
+        return ly.last ? 1024u : (uint32_t)(blk_w(nb) / 2) * (ly.first ? 32u : 128u);
+    };
+    const uint32_t w_full = ly.first ? 128u * 32u : (ly.last ? 1024u : 16384u);
     const unsigned char* wimg = reinterpret_cast<const unsigned char*>(sd.wtc) + ly.w_off + (size_t)rank * (size_t)ly.w_rank_bytes;
 
     if (warp == 13) {
@@ -120,15 +127,17 @@ hb_sur_tcw_kernel(HbParticles p, size_t n_chunk, const __grid_constant__ HbSurDe
             uint32_t cnt = 0;
             for (size_t g = cluster_id; g < ngroups; g += nclusters) {
                 const unsigned char* a_tile = ly.first ? nullptr : ly.act_in + ((g * CG + rank) * (size_t)NS) * A_SLAB_BYTES;
-                for (int nb = 0; nb < NB; ++nb)
+                for (int nb = 0; nb < NB; ++nb) {
+                    const uint32_t w_bytes = w_bytes_of(nb);
                     for (int s = 0; s < KS; ++s, ++cnt) {
                         const uint32_t slot = cnt % W_RING, phs = (cnt / W_RING) & 1;
                         mbar_wait<false>(bar(Q_RING_EMPTY + slot), phs ^ 1);
                         const uint32_t dst = sbase + pl.ring_off + slot * W_STAGE_BYTES;
                         mbar_expect_tx(bar(Q_RING_FULL + slot), (ly.first ? 0u : (uint32_t)A_SLAB_BYTES) + w_bytes);
                         if (!ly.first) bulk_g2s(dst, a_tile + (size_t)s * A_SLAB_BYTES, A_SLAB_BYTES, bar(Q_RING_FULL + slot));
-                        bulk_g2s(dst + A_SLAB_BYTES, wimg + ((size_t)nb * KS + s) * w_bytes, w_bytes, bar(Q_RING_FULL + slot));
+                        bulk_g2s(dst + A_SLAB_BYTES, wimg + (size_t)nb * KS * w_full + (size_t)s * w_bytes, w_bytes, bar(Q_RING_FULL + slot));
                     }
+                }
             }
         }
         __syncwarp();
@@ -149,7 +158,6 @@ hb_sur_tcw_kernel(HbParticles p, size_t n_chunk, const __grid_constant__ HbSurDe
         if (rank == 0) {
             const uint32_t fmt = F16 ? 0u : 1u;
             const uint32_t idesc_base = (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)((TILE_M * CG) >> 4) << 24);
-            const uint32_t idesc = idesc_base | ((uint32_t)((ly.last ? 16 : 256) >> 3) << 17);
             const bool issuer = elect_one();
             uint32_t cnt = 0;                        // ring stages consumed
             uint32_t use[2] = {0, 0};                // how often D[b] has been filled so far
@@ -160,6 +168,7 @@ hb_sur_tcw_kernel(HbParticles p, size_t n_chunk, const __grid_constant__ HbSurDe
                 for (int nb = 0; nb < NB; ++nb) {
                     const uint32_t b = (uint32_t)nb & 1u;
                     const uint32_t d_tmem = tmem_base + b * 256u;
+                    const uint32_t idesc = idesc_base | ((uint32_t)(blk_w(nb) >> 3) << 17);
                     // the epilogue must have read the block that filled D[b] before
                     if (!ly.last && use[b] > 0) mbar_wait<true>(bar(Q_D_FREE + b), (use[b] - 1) & 1);
                     ++use[b];
@@ -274,13 +283,14 @@ hb_sur_tcw_kernel(HbParticles p, size_t n_chunk, const __grid_constant__ HbSurDe
                     mbar_wait<true>(bar(Q_D_FULL + b), (ph_d >> b) & 1);
                     ph_d ^= 1u << b;
                     tc_fence_after();
+                    const int nj = blk_w(nb) >> 6;    // 64-column slabs of this output block
                     uint32_t ra[32], rb[32];
                     tmem_ld32(tlane + b * 256u, ra);
-                    for (int j = 0; j < 4; ++j, ++jj) {
+                    for (int j = 0; j < nj; ++j, ++jj) {
                         uint32_t (&cur)[32] = (j & 1) ? rb : ra;
                         uint32_t (&nxt)[32] = (j & 1) ? ra : rb;
                         tmem_ld_wait();
-                        if (j + 1 < 4) tmem_ld32(tlane + b * 256u + 64 * (j + 1), nxt);
+                        if (j + 1 < nj) tmem_ld32(tlane + b * 256u + 64 * (j + 1), nxt);
                         else {                        // every column of D[b] is in registers: hand it back
                             tc_fence_before();
                             __syncwarp();
@@ -323,14 +333,14 @@ bool make_wplan(int prec, int n_linear, const int* widths, TcwPlan& pl) {
     if (n_linear < 2) return false;
     int npad = 0;
     for (int l = 0; l < n_linear - 1; ++l) {
-        const int w = w_round_up(widths[l + 1], 256);
+        const int w = w_round_up(widths[l + 1], 64);
         if (l == 0) npad = w;
         else if (w != npad) return false;                            // equal (padded) hidden widths only
     }
     if (npad > 1024) return false;
     pl.npad = npad;
     pl.ns = npad / 64;
-    pl.nb = npad / 256;
+    pl.nb = (npad + 255) / 256;
     int off = 0;
     pl.ring_off = off;
     off += W_RING * W_STAGE_BYTES;
@@ -350,9 +360,10 @@ bool make_wplan(int prec, int n_linear, const int* widths, TcwPlan& pl) {
 
 // bytes of one rank's block sequence of layer l
 long long w_layer_rank_bytes(const TcwPlan& pl, int n_linear, int l) {
-    if (l == 0) return (long long)pl.nb * 128 * 32;
+    const long long half_rows = pl.npad / 2;                  // this rank's rows over all output blocks
+    if (l == 0) return half_rows * 32;
     if (l == n_linear - 1) return (long long)pl.ns * 1024;
-    return (long long)pl.nb * pl.ns * 16384;
+    return half_rows * 128 * pl.ns;
 }
 
 template <int ACT, bool F16>
@@ -430,14 +441,16 @@ size_t hb_tcw_pack_weights(int prec, int n_linear, const int* widths, const floa
         for (int rank = 0; rank < 2; ++rank) {
             const size_t r0 = (size_t)off_bytes[l] + (size_t)rank * (size_t)rb;
             if (l == 0) {
-                for (int nb = 0; nb < pl.nb; ++nb)
-                    for (int i = 0; i < 128; ++i) {
-                        const int o = nb * 256 + rank * 128 + i;
+                for (int nb = 0; nb < pl.nb; ++nb) {
+                    const int hw = std::min(256, pl.npad - 256 * nb) / 2;     // this rank's rows of the block
+                    for (int i = 0; i < hw; ++i) {
+                        const int o = nb * 256 + rank * hw + i;
                         if (o >= fout) continue;
                         for (int k = 0; k < 12; ++k)
                             put(r0 + (size_t)nb * 4096 + (size_t)(i / 8) * 256 + (size_t)(k / 8) * 128 + (size_t)(i % 8) * 16 + (size_t)(k % 8) * 2,
                                 W[0][(size_t)o * fin + (k % 6)]);
                     }
+                }
             } else if (l == n_linear - 1) {
                 for (int i = 0; i < 8; ++i) {
                     const int o = rank * 8 + i;
@@ -449,11 +462,12 @@ size_t hb_tcw_pack_weights(int prec, int n_linear, const int* widths, const floa
                     }
                 }
             } else {
-                for (int nb = 0; nb < pl.nb; ++nb)
+                for (int nb = 0; nb < pl.nb; ++nb) {
+                    const int hw = std::min(256, pl.npad - 256 * nb) / 2;
                     for (int s = 0; s < pl.ns; ++s) {
-                        const size_t b0 = r0 + ((size_t)nb * pl.ns + s) * 16384;
-                        for (int i = 0; i < 128; ++i) {
-                            const int o = nb * 256 + rank * 128 + i;
+                        const size_t b0 = r0 + (size_t)nb * pl.ns * 16384 + (size_t)s * hw * 128;
+                        for (int i = 0; i < hw; ++i) {
+                            const int o = nb * 256 + rank * hw + i;
                             if (o >= fout) continue;
                             for (int kk = 0; kk < 64; ++kk) {
                                 const int k = s * 64 + kk;
@@ -463,6 +477,7 @@ size_t hb_tcw_pack_weights(int prec, int n_linear, const int* widths, const floa
                             }
                         }
                     }
+                }
             }
         }
     }

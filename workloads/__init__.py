@@ -186,6 +186,18 @@ def config5(prec="bf16", n=100_000_000, stages=9, width=512, particles=True):
     return lattice(el), (gaussian_bunch(n, 5) if particles else None)
 
 
+def paper_net(width, hidden, prec="bf16", n=10_000_000, particles=True):
+    """One stage with the paper's own network shape (5 hidden x 900 for stages 1-3, 3 hidden x 700 for stages
+    4-15, PReLU), He-initialised weights from the seed (the trained weights are not available), COORD_S, N = 1e7 as
+    in the paper's timing; monitor after the stage."""
+    zero = np.zeros(6)
+    widths = [6] + [int(width)] * int(hidden) + [6]
+    W, b = make_mlp(widths, "he", 7, int(width))
+    a = np.full(len(widths) - 2, 0.25, dtype=np.float32)       # PyTorch's default PReLU slope
+    el = [surrogate(widths, W, b, "prelu", zero, NOMINAL_SIGMA, zero, NOMINAL_SIGMA, prelu_a=a, prec=prec), monitor()]
+    return lattice(el), (gaussian_bunch(n, 7) if particles else None)
+
+
 def subsample_indices(n: int, m: int = 1 << 20) -> np.ndarray:
     """Fixed parity subsample: every floor(n/m)-th particle, m particles (all of them if n <= m)."""
     if n <= m:
