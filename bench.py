@@ -332,6 +332,21 @@ def kernel_extras(torch, hb, args, pk, flush, dev):
                                  "frac": tf / pk["bf16_tflops"], "frac_of_sustained": tf / pk["bf16_tflops_sustained"],
                                  "traffic": None, "peak_source": pk["source"]}})
         del x5
+        # (b3) the paper's own network shapes on the layered kernel, one stage at N = 1e7; the paper's timings
+        # (P:199, 1 x A100, PyTorch) are context, not the target
+        for wname, (wd, hd, paper_ms) in (("P900", (900, 5, 1120.0)), ("P700", (700, 3, 494.0))):
+            descp, xp = wl.paper_net(wd, hd, prec="bf16", n=n)
+            flp = wl.flops_per_particle(descp["elements"][0]["widths"])
+            ms, seg = measure(descp, xp, "sur", True, steps=3)
+            k_ms = float(seg[0])
+            tf = flp * n / (k_ms * 1e-3) / 1e12
+            out.append({"kernel": "hb_sur_tcw_kernel<bf16> (%d launches: one per layer and 2^20-particle chunk)" % ((hd + 1) * ((n + (1 << 20) - 1) >> 20)),
+                        "workload": "%s: one stage 6-%d^%d-6 PReLU, N=%d" % (wname, wd, hd, n), "ms": k_ms,
+                        "particle_inferences_per_s": n / (k_ms * 1e-3), "paper_ms_per_stage_a100": paper_ms if n == 10_000_000 else None,
+                        "roofline": {"bound": "tensor", "achieved": tf, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
+                                     "frac": tf / pk["bf16_tflops"], "frac_of_sustained": tf / pk["bf16_tflops_sustained"],
+                                     "traffic": None, "peak_source": pk["source"]}})
+            del xp
         # (c) C4 hybrid lattice (all rows a1-a7 in one push)
         desc4, x4 = wl.config4(prec="bf16", n=n)
         ms, seg = measure(desc4, x4, "c4", True)
