@@ -493,7 +493,10 @@ cudaError_t hb_launch_sur_tcw(const HbParticles& p, size_t n, const HbSurDev& sd
     if (!sd.act_scratch) return cudaErrorInvalidValue;
     const int grid_max = (sm_count / 2) * 2;
     const size_t nchunks = (n + HB_TCW_CHUNK - 1) / HB_TCW_CHUNK;
-    if (partials && nchunks * (size_t)grid_max > (size_t)HB_MOM_MAX_BLOCKS) return cudaErrorNotSupported;
+    // rows of the partial buffer this stage may write: the whole buffer, or (hb_push_host: partials_zeroed) the row
+    // range of one host chunk
+    const size_t max_rows = partials_zeroed ? (size_t)HB_MOM_GRID_MAX : (size_t)HB_MOM_MAX_BLOCKS;
+    if (partials && nchunks * (size_t)grid_max > max_rows) return cudaErrorNotSupported;
     cudaError_t e = cudaSuccess;
     if (partials && !partials_zeroed)
         e = cudaMemsetAsync(partials, 0, (size_t)HB_NMOM * HB_MOM_MAX_BLOCKS * sizeof(double), s);

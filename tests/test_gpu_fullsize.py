@@ -127,3 +127,30 @@ def test_config5_full_size_first_stage_and_run(hb):
     assert np.all(np.isfinite(own))
     # record of the whole bunch vs plain moments of a 5e6-particle prefix: statistical agreement only
     assert np.allclose(np.sqrt(rec[-1][[6, 17, 24]]), np.sqrt(own[[6, 17, 24]]), rtol=5e-2)
+
+
+@pytest.mark.parametrize("name,width,hidden", [("P900", 900, 5), ("P700", 700, 3)])
+def test_paper_shaped_nets_full_size_sampled(hb, name, width, hidden):
+    """NEXT-1 at the paper's N (1e7) in the launch configuration `bench.py --workload P900|P700` times: the
+    layered kernel (10 chunks x (hidden + 1) launches), f16 operands, sampled particles vs the oracle; record vs
+    output; and the same bunch through hb_push_host (chunked host pipeline around the chunked layered stage)"""
+    import torch
+    desc, x = wl.paper_net(width, hidden, prec="f16")
+    n = x.shape[1]
+    assert n == 10_000_000 and hb.hb_surrogate_kernel("f16", desc["elements"][0]["widths"]) == "tcgen05-layered"
+    out, rec = gpu_push_full(hb, desc, x)
+    idx = sample_indices(n, m=3000)
+    idx = np.unique(np.concatenate([idx, np.arange((1 << 20) - 300, (1 << 20) + 300)]))     # a chunk boundary
+    ref, _ = oracle.push(desc, np.ascontiguousarray(x[:, idx]))
+    assert np.all(np.isfinite(out))
+    std = out[:, ::7].astype(np.float64).std(axis=1)
+    err = np.max(np.abs(out[:, idx].astype(np.float64) - ref), axis=1) / std
+    print(name, "full size f16 max err/std on", idx.size, "sampled particles:", err)
+    assert err.max() <= TOL["f16"]
+    check_moments(rec[-1], out)
+    lat = hb.Lattice.from_description(desc, device=0)
+    host = torch.from_numpy(x.copy()).pin_memory()
+    rec_h = lat.push_host(host, chunks=8)
+    lat.close()
+    assert np.array_equal(host.numpy(), out)
+    assert np.allclose(rec_h[-1][:6], rec[-1][:6], rtol=1e-12, atol=1e-18)
