@@ -425,6 +425,9 @@ def main():
     total_ms = float(t.item())
     ms_step = total_ms / args.steps
     assert bool(torch.isfinite(rec).all()), "non-finite moments"
+    if world > 1:       # monitor records of the whole N-rank bunch: 224 B per monitor and rank, outside the timed region
+        merged = hb.allgather_merge_records(rec, n)
+        assert bool(np.isfinite(merged).all()), "non-finite merged records"
 
     # ---- end to end through the C ABI with HOST buffers: hb_push_host (pinned host arrays in, results and moment
     # records back in host memory when the call returns; H2D, kernels, D2H pipelined in chunks inside the library).

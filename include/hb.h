@@ -178,6 +178,17 @@ hb_status hb_moments(const float *x, const float *px, const float *y, const floa
                      void *cuda_stream);
 size_t hb_moments_scratch_bytes(void);
 
+/* Record of the union of two disjoint particle sets from their records (HOST arithmetic, no device needed):
+ * the sharded-monitor step of a distributed bunch (every rank pushes its own particles; a monitor, P:138,
+ * is over all of them).  rec_a / rec_b: HOST, 27 doubles each as hb_push_moments writes them (6 means, then the
+ * 21 centred second moments with 1/N, upper triangle row-major); n_a, n_b: the particle counts behind them.
+ *   mean = (n_a mean_a + n_b mean_b) / n,   C = (n_a C_a + n_b C_b) / n + (n_a n_b / n^2) d d^T,  d = mean_b - mean_a
+ * (the pairwise update of the raw sums of R10, exact up to rounding).  A set with n = 0 contributes nothing (its
+ * record may hold NaN); n_a = n_b = 0 writes NaN.  rec_out: HOST, 27 doubles, may alias rec_a or rec_b.
+ * Errors: NULL pointer -> HB_ERR_INVALID_ARG. */
+hb_status hb_moments_merge(const double *rec_a, unsigned long long n_a, const double *rec_b, unsigned long long n_b,
+                           double *rec_out);
+
 /* Optional per-segment device timing (observability; P:199 gives the paper's manual breakdown).  When on,
  * every push records a CUDA event before the first and after each segment's kernels on the caller's stream.
  * hb_lattice_get_timing synchronises on the last event of the most recent push and writes, for each of the

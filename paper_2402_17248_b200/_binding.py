@@ -21,7 +21,8 @@ EXPORTED_SYMBOLS = [
     "hb_lattice_create", "hb_lattice_add_element", "hb_lattice_add_multipole", "hb_lattice_add_surrogate",
     "hb_lattice_set_run_mode",
     "hb_lattice_finalize", "hb_lattice_num_monitors", "hb_lattice_num_launches", "hb_lattice_ref_bg_out",
-    "hb_push", "hb_push_moments", "hb_push_host", "hb_moments", "hb_moments_scratch_bytes", "hb_lattice_destroy",
+    "hb_push", "hb_push_moments", "hb_push_host", "hb_moments", "hb_moments_scratch_bytes", "hb_moments_merge",
+    "hb_lattice_destroy",
     "hb_lattice_enable_timing", "hb_lattice_get_timing",
     "hb_status_string", "hb_last_error", "hb_version", "hb_surrogate_kernel",
 ]
@@ -83,6 +84,8 @@ def lib():
     L.hb_moments.argtypes = [c_void_p] * 6 + [c_size_t, POINTER(c_double), c_void_p, c_void_p, c_void_p]
     L.hb_moments_scratch_bytes.restype = c_size_t
     L.hb_moments_scratch_bytes.argtypes = []
+    L.hb_moments_merge.argtypes = [POINTER(c_double), ctypes.c_ulonglong, POINTER(c_double), ctypes.c_ulonglong,
+                                   POINTER(c_double)]
     L.hb_lattice_destroy.argtypes = [c_void_p]
     L.hb_lattice_enable_timing.argtypes = [c_void_p, c_int]
     L.hb_lattice_get_timing.argtypes = [c_void_p, POINTER(c_float), c_int, POINTER(c_int)]
@@ -223,6 +226,18 @@ def hb_moments(x, px, y, py, t, pt, n: int, pivot, d_out27: int, d_scratch: int,
     if pivot is not None:
         pv = (c_double * 6)(*[float(v) for v in pivot])
     _check(lib().hb_moments(x, px, y, py, t, pt, n, pv, d_out27, d_scratch, cuda_stream), "hb_moments")
+
+
+def hb_moments_merge(rec_a, n_a: int, rec_b, n_b: int):
+    """Record of the union of two disjoint particle sets (host arithmetic inside libhb.so).  rec_a / rec_b: 27 float64."""
+    import numpy as np
+    a = np.ascontiguousarray(rec_a, dtype=np.float64).reshape(27)
+    b = np.ascontiguousarray(rec_b, dtype=np.float64).reshape(27)
+    out = np.empty(27, dtype=np.float64)
+    pd = POINTER(c_double)
+    _check(lib().hb_moments_merge(a.ctypes.data_as(pd), int(n_a), b.ctypes.data_as(pd), int(n_b),
+                                  out.ctypes.data_as(pd)), "hb_moments_merge")
+    return out
 
 
 def hb_lattice_enable_timing(lat, on: bool = True):
@@ -391,4 +406,44 @@ def moments(coords, pivot=None, out=None):
     if key not in _scratch:
         _scratch[key] = torch.empty(hb_moments_scratch_bytes(), dtype=torch.uint8, device=dev)
     hb_moments(*[r.data_ptr() for r in rows], n, pivot, out.data_ptr(), _scratch[key].data_ptr(), _stream(dev))
+    return out
+
+
+def allgather_merge_records(records, n_local: int, group=None):
+    """Monitor records of a bunch sharded over the ranks of a torch.distributed group (each rank pushes its own
+    particles; no other exchange on the path).  records: [m, 27] float64 (tensor or array) of this rank's shard,
+    n_local its particle count.  All-gathers the m records and counts (224 B per monitor and rank) and merges them
+    in rank order with hb_moments_merge, so every rank returns the same [m, 27] numpy array: the records of the
+    whole bunch."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    rec = torch.as_tensor(records).detach().to("cpu", torch.float64).reshape(-1, 27).contiguous()
+    m = rec.shape[0]
+    if not (dist.is_available() and dist.is_initialized()):
+        return rec.numpy().copy()
+    world = dist.get_world_size(group)
+    backend = dist.get_backend(group)
+    dev = torch.device("cuda", torch.cuda.current_device()) if backend == "nccl" else torch.device("cpu")
+    # counts travel as two 32-bit halves inside the float64 payload (exact for any size_t below 2^64)
+    mine = torch.empty(m * 27 + 2, dtype=torch.float64)
+    mine[:m * 27] = rec.reshape(-1)
+    mine[m * 27] = float(int(n_local) >> 32)
+    mine[m * 27 + 1] = float(int(n_local) & 0xffffffff)
+    mine = mine.to(dev)
+    parts = [torch.empty_like(mine) for _ in range(world)]
+    dist.all_gather(parts, mine, group=group)
+    parts = [q.cpu().numpy() for q in parts]
+    out = np.empty((m, 27), dtype=np.float64)
+    for k in range(m):
+        acc, n_acc = None, 0
+        for q in parts:
+            n_q = (int(q[m * 27]) << 32) | int(q[m * 27 + 1])
+            r_q = q[k * 27:(k + 1) * 27]
+            if acc is None:
+                acc, n_acc = r_q.copy(), n_q
+            else:
+                acc = hb_moments_merge(acc, n_acc, r_q, n_q)
+                n_acc += n_q
+        out[k] = acc
     return out

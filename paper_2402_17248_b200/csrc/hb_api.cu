@@ -1,6 +1,7 @@
 // hb_api.cu -- the C ABI of include/hb.h: lattice construction, reference tracking (R1, R7), fp64
 // composition of conventional runs (R2-R5), weight packing, segment sequencing (row a7).
 // Host code only; kernels live in hb_run.cu / hb_sur_fp32.cu / hb_sur_tc.cu.
+#include <limits>
 #include "../../include/hb.h"
 #include "hb_internal.h"
 
@@ -778,6 +779,31 @@ hb_status hb_push_host(hb_lattice* lat, float* x, float* px, float* y, float* py
     }
     if (prev != lat->device) cudaSetDevice(prev);
     return st;
+}
+
+hb_status hb_moments_merge(const double* rec_a, unsigned long long n_a, const double* rec_b, unsigned long long n_b,
+                           double* rec_out) {
+    if (!rec_a || !rec_b || !rec_out) return fail(HB_ERR_INVALID_ARG, "hb_moments_merge: NULL record");
+    double out[HB_NMOM];
+    if (n_a == 0 && n_b == 0) {
+        for (int i = 0; i < HB_NMOM; ++i) out[i] = std::numeric_limits<double>::quiet_NaN();
+    } else if (n_a == 0 || n_b == 0) {
+        const double* src = n_a ? rec_a : rec_b;
+        for (int i = 0; i < HB_NMOM; ++i) out[i] = src[i];
+    } else {
+        const double na = (double)n_a, nb = (double)n_b, n = na + nb;
+        const double wa = na / n, wb = nb / n;
+        double d[6];
+        for (int i = 0; i < 6; ++i) {
+            d[i] = rec_b[i] - rec_a[i];
+            out[i] = rec_a[i] + wb * d[i];
+        }
+        int k = 6;
+        for (int i = 0; i < 6; ++i)
+            for (int j = i; j < 6; ++j, ++k) out[k] = wa * rec_a[k] + wb * rec_b[k] + wa * wb * d[i] * d[j];
+    }
+    for (int i = 0; i < HB_NMOM; ++i) rec_out[i] = out[i];
+    return HB_OK;
 }
 
 size_t hb_moments_scratch_bytes(void) { return (size_t)HB_MOM_MAX_BLOCKS * HB_NMOM * sizeof(double); }

@@ -277,7 +277,7 @@ def test_tcw_bringup_identity_net(hb, prec, H):
 @pytest.mark.parametrize("prec", ["bf16", "f16"])
 @pytest.mark.parametrize("act,widths,n", [("prelu", [6, 900, 900, 900, 900, 900, 6], 20_000), ("prelu", [6, 700, 700, 700, 6], 20_000),
                                           ("tanh", [6, 520, 520, 6], 257), ("relu", [6, 1024, 6], 1),
-                                          ("relu", [6, 600, 600, 6], 40_001)])
+                                          ("relu", [6, 600, 600, 6], 40_001), ("tanh", [6, 900, 930, 960, 6], 3_000)])
 def test_tcw_shapes(hb, prec, act, widths, n):
     """the paper's own network shapes (6-900^5-6, 6-700^3-6 PReLU) and the edges of the layered kernel"""
     init = "he" if act in ("relu", "prelu") else "xavier"

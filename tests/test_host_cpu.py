@@ -108,8 +108,53 @@ def test_surrogate_kernel_dispatch_is_a_host_decision(hb, monkeypatch):
     assert K("bf16", [6, 900, 900, 900, 900, 900, 6]) == "tcgen05-layered"   # the paper's own nets: one launch per layer
     assert K("f16", [6, 700, 700, 700, 6]) == "tcgen05-layered"
     assert K("tf32", [6, 700, 700, 700, 6]) is None and K("bf16", [6, 1100, 1100, 6]) is None
-    assert K("bf16", [6, 512, 300, 512, 6]) == "tcgen05-layered"          # unequal widths that pad to the same 256-multiple
+    assert K("bf16", [6, 900, 930, 960, 6]) == "tcgen05-layered"          # unequal widths that pad to the same multiple of 64
+    assert K("bf16", [6, 512, 300, 512, 6]) is None
     assert K("bf16", [6, 512, 1024, 512, 6]) is None                      # streamed / layered kernels: equal padded widths only
     assert K("bf16", [6, 1025, 6]) is None and K("bf16", [5, 8, 6]) is None
     monkeypatch.setenv("HB_TC_FORCE_STREAM", "1")
     assert K("bf16", [6, 256, 256, 256, 6]) == "tcgen05-streamed"
+
+
+def test_moments_merge_against_plain_moments(hb):
+    """hb_moments_merge (host arithmetic of the sharded monitor): records of parts -> record of the whole, against
+    numpy's mean / covariance of the concatenation; uneven three-way split, far-off-centre data, empty parts,
+    aliasing, NULL"""
+    rng = np.random.default_rng(5)
+    a = rng.normal(size=(6, 1000)) * np.array([1e-3, 1e-4, 2e-3, 1e-4, 5e-4, 1e-3])[:, None] + 0.25
+    a[1] += 3.0 * a[0]                                  # off-diagonal terms that matter
+
+    def rec(z):
+        m = z.mean(axis=1)
+        c = np.cov(z, bias=True)
+        return np.concatenate([m, c[np.triu_indices(6)]])
+
+    cuts = [0, 17, 640, 1000]
+    acc, n_acc = None, 0
+    for lo, hi in zip(cuts[:-1], cuts[1:]):
+        r = rec(a[:, lo:hi])
+        acc = r if acc is None else hb.hb_moments_merge(acc, n_acc, r, hi - lo)
+        n_acc += hi - lo
+    want = rec(a)
+    assert np.allclose(acc[:6], want[:6], rtol=1e-14)
+    scale = np.sqrt(np.outer(np.diag(np.cov(a, bias=True)), np.diag(np.cov(a, bias=True))))[np.triu_indices(6)]
+    assert np.all(np.abs(acc[6:] - want[6:]) <= 1e-9 * scale)   # 0.25 offset: cancellation costs a few digits
+    nan = np.full(27, np.nan)
+    assert np.array_equal(hb.hb_moments_merge(nan, 0, want, 1000), want)
+    assert np.array_equal(hb.hb_moments_merge(want, 1000, nan, 0), want)
+    assert np.all(np.isnan(hb.hb_moments_merge(nan, 0, nan, 0)))
+    # two single particles: mean = midpoint, C = d d^T / 4
+    p, q = a[:, 0], a[:, 1]
+    z = np.zeros(21)
+    got = hb.hb_moments_merge(np.concatenate([p, z]), 1, np.concatenate([q, z]), 1)
+    d = q - p
+    assert np.allclose(got[:6], 0.5 * (p + q), rtol=1e-15)
+    assert np.allclose(got[6:], (np.outer(d, d) / 4)[np.triu_indices(6)], rtol=1e-12, atol=0)
+    import ctypes
+    assert hb.lib().hb_moments_merge(None, 1, None, 1, None) != 0
+    out = want.copy()
+    pd = ctypes.POINTER(ctypes.c_double)
+    r2 = rec(a[:, :500])
+    exp = hb.hb_moments_merge(out, 1000, r2, 500)
+    assert hb.lib().hb_moments_merge(out.ctypes.data_as(pd), 1000, r2.ctypes.data_as(pd), 500, out.ctypes.data_as(pd)) == 0
+    assert np.array_equal(out, exp)
