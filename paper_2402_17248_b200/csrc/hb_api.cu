@@ -440,10 +440,13 @@ static hb_status build_surrogate(hb_lattice* lat, const SurHost& s, double bg_in
             return fail(HB_ERR_UNSUPPORTED, "tensor-core surrogate: %s", why);
         std::vector<const float*> Wp;
         for (int l = 0; l < s.n_linear; ++l) Wp.push_back(s.W[l].data());
-        const size_t bytes = hb_tc_pack_weights(s.prec, s.n_linear, s.widths.data(), Wp.data(), nullptr,
+        std::vector<const float*> Bp;
+        for (int l = 0; l < s.n_linear; ++l) Bp.push_back(s.b[l].data());
+        const size_t bytes = hb_tc_pack_weights(s.prec, s.n_linear, s.widths.data(), Wp.data(), nullptr, nullptr,
                                                 sd.wtc_off, sd.kpad, sd.npadtc);
         std::vector<unsigned char> img(bytes);
-        hb_tc_pack_weights(s.prec, s.n_linear, s.widths.data(), Wp.data(), img.data(), sd.wtc_off, sd.kpad, sd.npadtc);
+        hb_tc_pack_weights(s.prec, s.n_linear, s.widths.data(), Wp.data(), Bp.data(), img.data(), sd.wtc_off, sd.kpad,
+                           sd.npadtc);
         std::vector<float> b;
         for (int l = 0; l < s.n_linear; ++l) {
             sd.btc_off[l] = (int)b.size();

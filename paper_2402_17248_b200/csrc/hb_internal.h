@@ -85,7 +85,9 @@ cudaError_t hb_launch_sur_tc(const HbParticles& p, size_t n, const HbSurDev& sd,
                              int* nblocks_out, int sm_count, cudaStream_t s);
 // host-side packing for the tensor-core path (hb_sur_tc.cu owns the layout)
 //  returns bytes needed; if dst != nullptr writes the image.  W row-major [out][in] fp32.
-size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float* const* W,
+//  B: biases [out] fp32 per layer (the resident kernel's image carries those of the hidden layers; may be nullptr
+//  when dst is).
+size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float* const* W, const float* const* B,
                           void* dst, long long* off_bytes, int* kpad, int* npad);
 bool hb_tc_supported(int prec, int n_linear, const int* widths, char* why, size_t why_len);
 // streamed-weights variant (hb_sur_tcs.cu): hidden width <= 512, equal hidden widths, weights through an smem ring

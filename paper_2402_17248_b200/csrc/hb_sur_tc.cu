@@ -25,7 +25,8 @@ struct TcPlan {
     int npad[HB_MAX_LINEAR];          // padded fan-out (whole layer, both CTAs of a pair)
     int w_off[HB_MAX_LINEAR];         // smem byte offset of layer l's weights (this CTA's rows)
     int w_slab_bytes[HB_MAX_LINEAR];  // l >= 1: (npad / CG) * 128;  l = 0: (npad / CG) * 32 (whole layer)
-    int bias_off[HB_MAX_LINEAR];      // float offset inside the smem bias block
+    int wb_off[HB_MAX_LINEAR];        // 1 <= l <= L-2: smem byte offset of layer l's bias block (K = 16 operand, this CTA's rows)
+    int wb_bytes[HB_MAX_LINEAR];      //                (npad / CG) * 32
     int a_off, a0_off, stage_off, bias_base, bar_off, red_off, total;
     int d_cols;                       // columns of one accumulator buffer
     int tmem_cols;                    // 2 * d_cols rounded to a power of two >= 32
@@ -90,14 +91,8 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
         tmem_alloc<CG>(smem_u32(tmem_slot), (uint32_t)pl.tmem_cols);
         tmem_relinquish<CG>();
     }
-    {   // biases -> shared (all layers)
-        const int total = pl.bias_off[L - 1] + pl.npad[L - 1];
-        for (int i = tid; i < total; i += THREADS) {
-            int l = 0;
-            while (l + 1 < L && i >= pl.bias_off[l + 1]) ++l;
-            bias_s[i] = sd.btc[sd.btc_off[l] + (i - pl.bias_off[l])];
-        }
-    }
+    // bias of the last layer -> shared (fp32, added by the IO warps); the hidden layers' biases ride in the MMAs
+    for (int i = tid; i < pl.npad[L - 1]; i += THREADS) bias_s[i] = sd.btc[sd.btc_off[L - 1] + i];
     tc_fence_before();
     __syncthreads();
     if (CG == 2) cluster_sync_all();
@@ -117,6 +112,10 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                     const unsigned char* src = wg + sd.wtc_off[l] + (size_t)s * pl.npad[l] * 128 + (size_t)rank * pl.w_slab_bytes[l];
                     bulk_g2s(sbase + pl.w_off[l] + s * pl.w_slab_bytes[l], src, (uint32_t)pl.w_slab_bytes[l], bar(B_W));
                 }
+            for (int l = 1; l + 1 < L; ++l)      // bias blocks of the hidden layers (behind the layer's K slabs)
+                bulk_g2s(sbase + pl.wb_off[l],
+                         wg + sd.wtc_off[l] + (size_t)pl.nslab[l] * pl.npad[l] * 128 + (size_t)rank * pl.wb_bytes[l],
+                         (uint32_t)pl.wb_bytes[l], bar(B_W));
             int stage = 0;
             uint32_t ph = 0;
             for (size_t g = cluster_id; g < ngroups; g += nclusters) {
@@ -149,13 +148,14 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
             uint32_t it = 0;
             // per-layer constants are fetched one layer ahead: anything issued behind a batch of MMAs waits for
             // the tensor pipe's queue, so the loads for layer l+1 go out before the MMAs of layer l
-            struct LayerC { uint32_t idesc; int nsl; uint64_t bd, bd_step; };
+            struct LayerC { uint32_t idesc; int nsl; uint64_t bd, bd_step, wbd; };
             auto layer_consts = [&](int l) {
                 LayerC c;
                 c.idesc = idesc_base | ((uint32_t)(pl.npad[l] >> 3) << 17);
                 c.nsl = pl.nslab[l];
                 c.bd = make_desc(sbase + pl.w_off[l]);
                 c.bd_step = (uint64_t)(pl.w_slab_bytes[l] >> 4);
+                c.wbd = make_desc_l0(sbase + pl.wb_off[l]);
                 return c;
             };
             const LayerC c0 = layer_consts(0);
@@ -188,6 +188,12 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                     const uint64_t bd = cur.bd, bd_step = cur.bd_step;
                     // D[last_buf] still holds the previous tile's outputs until the IO warps have read them
                     if (it > 0 && l == last_buf) mbar_wait<true>(bar(B_OUT_READ), (it - 1) & 1);
+                    // hidden layer: the bias goes in first, as one K = 16 MMA of this tile's layer-0 operand (ones
+                    // in columns 12, 13) with the layer's bias block (b_hi, b_lo in columns 12, 13, zeros elsewhere).
+                    // It depends on nothing the epilogue produces, so it runs in the bubble before slab 0 arrives.
+                    const bool hid = l + 1 < L;
+                    if (hid && issuer)
+                        umma<CG, false>(d_tmem, make_desc_l0(sbase + pl.a0_off + (it & 1) * A0_BYTES), cur.wbd, idesc);
                     // fully unrolled over the (at most MAX_SLABS) K slabs
                     uint32_t ready = 0;               // slab j's barrier already seen complete (peeked)
 #pragma unroll
@@ -204,7 +210,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                                 // four K = 16 steps inside the 64-wide slab: the start address advances by 32 B
                                 const uint64_t ad = a_desc0 + (uint64_t)(j * (A_SLAB_BYTES >> 4));
                                 const uint64_t bj = bd + (uint64_t)j * bd_step;
-                                if (j == 0) umma<CG, false>(d_tmem, ad, bj, idesc);
+                                if (j == 0 && !hid) umma<CG, false>(d_tmem, ad, bj, idesc);
                                 else umma<CG, true>(d_tmem, ad, bj, idesc);
                                 umma<CG, true>(d_tmem, ad + 2, bj + 2, idesc);
                                 umma<CG, true>(d_tmem, ad + 4, bj + 4, idesc);
@@ -226,7 +232,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
         const int row = 32 * wq + lane;          // tile row = TMEM lane = particle within the tile
         const uint32_t a0_row = sbase + pl.a0_off + (uint32_t)(row >> 3) * 256 + (uint32_t)(row & 7) * 16;
         const uint32_t tlane = tmem_base + ((uint32_t)(32 * wq) << 16) + (uint32_t)(last_buf * pl.d_cols);
-        const float* bl = bias_s + pl.bias_off[L - 1];
+        const float* bl = bias_s;
         HbMomAcc acc;
         acc.clear();
         int stage = 0;
@@ -257,10 +263,11 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
             float lo[6];
 #pragma unroll
             for (int j = 0; j < 6; ++j) lo[j] = nin[j] - round16<F16>(nin[j]);
-            // K = 16 operand row: hi0..hi5, lo0..lo5, 0, 0, 0, 0  (two 16-byte chunks, 128 B apart)
+            // K = 16 operand row: hi0..hi5, lo0..lo5, 1, 1, 0, 0  (two 16-byte chunks, 128 B apart); the ones meet
+            // b_hi, b_lo in columns 12, 13 of the weights (layer 0) and of the bias blocks (hidden layers)
             const uint32_t q0[4] = {pack2<F16>(nin[0], nin[1]), pack2<F16>(nin[2], nin[3]), pack2<F16>(nin[4], nin[5]),
                                     pack2<F16>(lo[0], lo[1])};
-            const uint32_t q1[4] = {pack2<F16>(lo[2], lo[3]), pack2<F16>(lo[4], lo[5]), 0u, 0u};
+            const uint32_t q1[4] = {pack2<F16>(lo[2], lo[3]), pack2<F16>(lo[4], lo[5]), pack2<F16>(1.0f, 1.0f), 0u};
             const uint32_t dst = a0_row + buf * A0_BYTES;
             asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(dst), "r"(q0[0]), "r"(q0[1]), "r"(q0[2]), "r"(q0[3]) : "memory");
             asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(dst + 128), "r"(q1[0]), "r"(q1[1]), "r"(q1[2]), "r"(q1[3]) : "memory");
@@ -318,7 +325,6 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
             for (int l = 0; l < L - 1; ++l) {
                 const int b = l & 1;
                 const int nsl = pl.npad[l] >> 6;
-                                const float* bl = bias_s + pl.bias_off[l];   // (from global/L1 instead: 2.63 -> 3.07 ms on C3, measured)
                 const float slope = sd.prelu[l];
                 // this warp's 32-column chunks of the layer: columns 32 * (c * G + grp), c = 0 .. nch-1
                 // (G = 2: one chunk per 64-column slab; G = 1: both chunks of every slab)
@@ -334,7 +340,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                     const int col_a = CW * (c * G + grp), col_b = CW * ((c + 1) * G + grp);
                     tmem_ld_wait();
                     if (c + 1 < nch) tmem_ld<CW>(tlane + (uint32_t)(b * pl.d_cols + col_b), rb);
-                    epi_store<CW, ACT, F16>(ra, bl, col_a, slope, a_row, sw);
+                    epi_store_nb<CW, ACT, F16>(ra, col_a, slope, a_row, sw);
                     if (G == 2 || c + 1 >= nch) {           // chunk a closes its slab
                         fence_proxy_async();
                         tc_fence_before();
@@ -345,7 +351,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                     if (c + 1 < nch) {
                         tmem_ld_wait();
                         if (c + 2 < nch) tmem_ld<CW>(tlane + (uint32_t)(b * pl.d_cols + CW * ((c + 2) * G + grp)), ra);
-                        epi_store<CW, ACT, F16>(rb, bl, col_b, slope, a_row, sw);
+                        epi_store_nb<CW, ACT, F16>(rb, col_b, slope, a_row, sw);
                         fence_proxy_async();
                         tc_fence_before();
                         __syncwarp();
@@ -383,7 +389,7 @@ bool make_plan(int cg, int n_linear, const int* widths, TcPlan& pl) {
     int kpad[HB_MAX_LINEAR], ksteps[HB_MAX_LINEAR];
     layer_geometry(n_linear, widths, kpad, pl.npad, ksteps);
     pl.n_linear = n_linear;
-    int off = 0, boff = 0, maxslab = 1, maxn = 32;
+    int off = 0, maxslab = 1, maxn = 32;
     for (int l = 0; l < n_linear; ++l) {
         pl.ksteps[l] = ksteps[l];
         pl.nslab[l] = l == 0 ? 0 : kpad[l] / 64;
@@ -391,15 +397,18 @@ bool make_plan(int cg, int n_linear, const int* widths, TcPlan& pl) {
         pl.w_slab_bytes[l] = pl.npad[l] / cg * (l == 0 ? 32 : 128);
         pl.w_off[l] = off;
         off += (l == 0 ? 1 : pl.nslab[l]) * pl.w_slab_bytes[l];
+        if (l >= 1 && l + 1 < n_linear) {
+            pl.wb_off[l] = off;
+            pl.wb_bytes[l] = pl.npad[l] / cg * 32;
+            off += pl.wb_bytes[l];
+        }
         off = round_up(off, 1024);
-        pl.bias_off[l] = boff;
-        boff += pl.npad[l];
         if (pl.nslab[l] > maxslab) maxslab = pl.nslab[l];
         if (pl.npad[l] > maxn) maxn = pl.npad[l];
     }
     if (maxn > 256 || maxslab > MAX_SLABS) return false;            // two accumulators must fit the 512 TMEM columns
     pl.w_bytes_total = 0;
-    for (int l = 0; l < n_linear; ++l) pl.w_bytes_total += (l == 0 ? 1 : pl.nslab[l]) * pl.w_slab_bytes[l];
+    for (int l = 0; l < n_linear; ++l) pl.w_bytes_total += (l == 0 ? 1 : pl.nslab[l]) * pl.w_slab_bytes[l] + pl.wb_bytes[l];
     pl.a_off = off;
     off += maxslab * A_SLAB_BYTES;
     pl.a0_off = off;
@@ -407,7 +416,7 @@ bool make_plan(int cg, int n_linear, const int* widths, TcPlan& pl) {
     pl.stage_off = off;
     off += IN_STAGES * STAGE_BYTES;
     pl.bias_base = off;
-    off += round_up(boff * 4, 16);
+    off += round_up(pl.npad[n_linear - 1] * 4, 16);
     pl.bar_off = off;
     off += round_up(8 * B_COUNT + 8, 16);
     pl.red_off = off;
@@ -533,8 +542,9 @@ bool hb_tc_supported(int prec, int n_linear, const int* widths, char* why, size_
 // (8 x 16 B) followed by K chunk 1; W_0 is carried twice (columns 0..5 multiply the hi parts of the inputs,
 // 6..11 the lo parts).  Layers >= 1: per 64-wide K slab, npad rows of 128 bytes (K-major, 128-byte swizzle:
 // the 16-byte chunk c of row r sits at chunk position c ^ (r mod 8)).
-size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float* const* W, void* dst,
-                          long long* off_bytes, int* kpad, int* npad) {
+size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float* const* W, const float* const* B,
+                          void* dst, long long* off_bytes, int* kpad, int* npad) {
+    (void)B;
     if (use_stream(prec, n_linear, widths)) return hb_tcs_pack_weights(prec, n_linear, widths, W, dst, off_bytes, kpad, npad);
     if (hb_tc_kernel_kind(prec, n_linear, widths) == 3) return hb_tcw_pack_weights(prec, n_linear, widths, W, dst, off_bytes, kpad, npad);
     int ksteps[HB_MAX_LINEAR];
@@ -543,11 +553,34 @@ size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float
     for (int l = 0; l < n_linear; ++l) {
         off_bytes[l] = (long long)total;
         total += l == 0 ? (size_t)npad[l] * 32 : (size_t)(kpad[l] / 64) * npad[l] * 128;
+        if (l >= 1 && l + 1 < n_linear) total += (size_t)npad[l] * 32;      // bias block of a hidden layer
         total = (total + 15) / 16 * 16;
     }
     if (!dst) return total;
     std::memset(dst, 0, total);
     unsigned char* base = static_cast<unsigned char*>(dst);
+    auto bits16 = [prec](float w) {
+        unsigned short bits;
+        if (prec == 2) { __half h = __float2half_rn(w); std::memcpy(&bits, &h, 2); }
+        else { __nv_bfloat16 h = __float2bfloat16_rn(w); std::memcpy(&bits, &h, 2); }
+        return bits;
+    };
+    auto back32 = [prec](unsigned short bits) {
+        if (prec == 2) { __half h; std::memcpy(&h, &bits, 2); return __half2float(h); }
+        __nv_bfloat16 h; std::memcpy(&h, &bits, 2); return __bfloat162float(h);
+    };
+    // biases of layers 0 .. L-2 as b_hi, b_lo (value rounded to the operand type, rounded remainder) in K columns
+    // 12, 13 of a K = 16 operand: inside W_0 for layer 0, in a block of its own behind the K slabs for the others
+    for (int l = 0; l + 1 < n_linear; ++l) {
+        const size_t blk = (size_t)off_bytes[l] + (l == 0 ? 0 : (size_t)(kpad[l] / 64) * npad[l] * 128);
+        for (int o = 0; o < widths[l + 1]; ++o) {
+            const unsigned short hi = bits16(B[l][o]);
+            const unsigned short lo = bits16(B[l][o] - back32(hi));
+            const size_t byte = blk + (size_t)(o / 8) * 256 + 128 + (size_t)(o % 8) * 16 + 4 * 2;   // k = 12
+            std::memcpy(base + byte, &hi, 2);
+            std::memcpy(base + byte + 2, &lo, 2);
+        }
+    }
     for (int l = 0; l < n_linear; ++l) {
         const int fin = widths[l], fout = widths[l + 1];
         const int kcols = l == 0 ? 12 : fin;
@@ -562,9 +595,7 @@ size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float
                     byte = (size_t)off_bytes[l] + (size_t)slab * npad[l] * 128 + (size_t)o * 128 +
                            (size_t)((c ^ (o & 7)) << 4) + (size_t)e * 2;
                 }
-                unsigned short bits;
-                if (prec == 2) { __half h = __float2half_rn(w); std::memcpy(&bits, &h, 2); }
-                else { __nv_bfloat16 h = __float2bfloat16_rn(w); std::memcpy(&bits, &h, 2); }
+                const unsigned short bits = bits16(w);
                 std::memcpy(base + byte, &bits, 2);
             }
     }

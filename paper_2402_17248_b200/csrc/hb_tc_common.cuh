@@ -275,6 +275,21 @@ __device__ __forceinline__ void epi_store(const uint32_t (&r)[CW], const float* 
 }
 
 
+// As epi_store without the bias: the accumulator already holds W a + b (the bias went in as an MMA of its own).
+template <int CW, int ACT, bool F16>
+__device__ __forceinline__ void epi_store_nb(const uint32_t (&r)[CW], int c0, float slope, uint32_t a_row, uint32_t sw) {
+    uint32_t q[CW / 2];
+#pragma unroll
+    for (int k = 0; k < CW / 2; ++k)
+        q[k] = act_pack<ACT, F16>(__uint_as_float(r[2 * k]), __uint_as_float(r[2 * k + 1]), slope);
+    const uint32_t slab = a_row + (uint32_t)(c0 >> 6) * A_SLAB_BYTES;
+    const uint32_t ch0 = (uint32_t)((c0 & 63) >> 3);
+#pragma unroll
+    for (int k = 0; k < CW / 8; ++k)
+        asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(slab + (((ch0 + k) ^ sw) << 4)),
+                     "r"(q[4 * k]), "r"(q[4 * k + 1]), "r"(q[4 * k + 2]), "r"(q[4 * k + 3]) : "memory");
+}
+
 // a4: six s-coordinates of one particle -> the K = 16 layer-0 operand row  hi0..hi5, lo0..lo5, 0, 0, 0, 0
 // (hi = value rounded to the operand type, lo = rounded remainder), as two 16-byte chunks.
 template <bool F16>
