@@ -27,7 +27,7 @@ struct TcPlan {
     int w_slab_bytes[HB_MAX_LINEAR];  // l >= 1: (npad / CG) * 128;  l = 0: (npad / CG) * 32 (whole layer)
     int wb_off[HB_MAX_LINEAR];        // 1 <= l <= L-2: smem byte offset of layer l's bias block (K = 16 operand, this CTA's rows)
     int wb_bytes[HB_MAX_LINEAR];      //                (npad / CG) * 32
-    int a_off, a0_off, stage_off, bias_base, bar_off, red_off, total;
+    int a0_off, stage_off, bias_base, bar_off, red_off, total;
     int d_cols;                       // columns of one accumulator buffer
     int tmem_cols;                    // 2 * d_cols rounded to a power of two >= 32
     int w_bytes_total;                // bytes this CTA loads
@@ -141,7 +141,6 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
             const uint32_t fmt = F16 ? 0u : 1u;
             const uint32_t idesc_base = (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)((TILE_M * CG) >> 4) << 24);
             const bool issuer = elect_one();
-            const uint64_t a_desc0 = make_desc(sbase + pl.a_off);
             const uint64_t w0_desc = make_desc_l0(sbase + pl.w_off[0]);
             TR_DECL;
             uint32_t ph_slab = 0;                    // bit j: parity of the next completion of SLAB_FULL[j]
@@ -183,6 +182,9 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                     const LayerC cur = nxt;
                     nxt = layer_consts(l + 1 < L ? l + 1 : 1);
                     const uint32_t d_tmem = tmem_base + (uint32_t)((l & 1) * pl.d_cols);
+                    // the operand of layer l sits in the accumulator buffer of layer l-1 (written there in place by
+                    // the epilogue): slab j = columns [64 j, 64 j + 16) and [64 j + 32, 64 j + 48), 8 per K = 16 step
+                    const uint32_t a_tmem = tmem_base + (uint32_t)(((l - 1) & 1) * pl.d_cols);
                     const uint32_t idesc = cur.idesc;
                     const int nsl = cur.nsl;
                     const uint64_t bd = cur.bd, bd_step = cur.bd_step;
@@ -207,14 +209,15 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                             ready = (j + 1 < nsl) ? mbar_test(bar(B_SLAB_FULL + j + 1), (ph_slab >> (j + 1)) & 1) : 0u;
                             if (j == 0) TR(0, 17);
                             if (issuer) {
-                                // four K = 16 steps inside the 64-wide slab: the start address advances by 32 B
-                                const uint64_t ad = a_desc0 + (uint64_t)(j * (A_SLAB_BYTES >> 4));
+                                // four K = 16 steps inside the 64-wide slab: B advances by 32 B, A by 8 columns
+                                // (second 32-column chunk of the slab: + 32)
+                                const uint32_t ad = a_tmem + (uint32_t)(64 * j);
                                 const uint64_t bj = bd + (uint64_t)j * bd_step;
-                                if (j == 0 && !hid) umma<CG, false>(d_tmem, ad, bj, idesc);
-                                else umma<CG, true>(d_tmem, ad, bj, idesc);
-                                umma<CG, true>(d_tmem, ad + 2, bj + 2, idesc);
-                                umma<CG, true>(d_tmem, ad + 4, bj + 4, idesc);
-                                umma<CG, true>(d_tmem, ad + 6, bj + 6, idesc);
+                                if (j == 0 && !hid) umma_ts<CG, false>(d_tmem, ad, bj, idesc);
+                                else umma_ts<CG, true>(d_tmem, ad, bj, idesc);
+                                umma_ts<CG, true>(d_tmem, ad + 8, bj + 2, idesc);
+                                umma_ts<CG, true>(d_tmem, ad + 32, bj + 4, idesc);
+                                umma_ts<CG, true>(d_tmem, ad + 40, bj + 6, idesc);
                             }
                         }
                     }
@@ -313,9 +316,6 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
         // ===================================================== hidden-layer epilogue warps
         const int wq = warp & 3;
         const int grp = (warp - EPI_WARP0) >> 2;  // column group inside every 64-column slab
-        const int row = 32 * wq + lane;
-        const uint32_t a_row = sbase + pl.a_off + row * 128;
-        const uint32_t sw = (uint32_t)(row & 7);
         const uint32_t tlane = tmem_base + ((uint32_t)(32 * wq) << 16);
         TR_DECL;
         [[maybe_unused]] const int trole = 4 + (warp - EPI_WARP0);
@@ -329,20 +329,20 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                 // this warp's 32-column chunks of the layer: columns 32 * (c * G + grp), c = 0 .. nch-1
                 // (G = 2: one chunk per 64-column slab; G = 1: both chunks of every slab)
                 const int nch = nsl * (2 / G);
-                const uint32_t t0 = tlane + (uint32_t)(b * pl.d_cols + grp * CW);
+                const uint32_t tl = tlane + (uint32_t)(b * pl.d_cols);
                 mbar_wait<true>(bar(B_D_HID + b), (ph_d >> b) & 1);
                 ph_d ^= 1u << b;
                 tc_fence_after();
                 TR(trole, 2);
                 uint32_t ra[CW], rb[CW];
-                tmem_ld<CW>(t0, ra);
+                tmem_ld<CW>(tl + (uint32_t)(grp * CW), ra);
                 for (int c = 0; c < nch; c += 2) {
                     const int col_a = CW * (c * G + grp), col_b = CW * ((c + 1) * G + grp);
                     tmem_ld_wait();
-                    if (c + 1 < nch) tmem_ld<CW>(tlane + (uint32_t)(b * pl.d_cols + col_b), rb);
-                    epi_store_nb<CW, ACT, F16>(ra, col_a, slope, a_row, sw);
+                    if (c + 1 < nch) tmem_ld<CW>(tl + (uint32_t)col_b, rb);
+                    epi_store_tmem<ACT, F16>(ra, tl + (uint32_t)col_a, slope);
                     if (G == 2 || c + 1 >= nch) {           // chunk a closes its slab
-                        fence_proxy_async();
+                        tmem_st_wait();
                         tc_fence_before();
                         __syncwarp();
                         if (lane == 0) mbar_arrive_cluster(bar(B_SLAB_FULL + (col_a >> 6)), 0);
@@ -350,9 +350,9 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                     }
                     if (c + 1 < nch) {
                         tmem_ld_wait();
-                        if (c + 2 < nch) tmem_ld<CW>(tlane + (uint32_t)(b * pl.d_cols + CW * ((c + 2) * G + grp)), ra);
-                        epi_store_nb<CW, ACT, F16>(rb, col_b, slope, a_row, sw);
-                        fence_proxy_async();
+                        if (c + 2 < nch) tmem_ld<CW>(tl + (uint32_t)(CW * ((c + 2) * G + grp)), ra);
+                        epi_store_tmem<ACT, F16>(rb, tl + (uint32_t)col_b, slope);
+                        tmem_st_wait();
                         tc_fence_before();
                         __syncwarp();
                         if (lane == 0) mbar_arrive_cluster(bar(B_SLAB_FULL + (col_b >> 6)), 0);
@@ -409,8 +409,6 @@ bool make_plan(int cg, int n_linear, const int* widths, TcPlan& pl) {
     if (maxn > 256 || maxslab > MAX_SLABS) return false;            // two accumulators must fit the 512 TMEM columns
     pl.w_bytes_total = 0;
     for (int l = 0; l < n_linear; ++l) pl.w_bytes_total += (l == 0 ? 1 : pl.nslab[l]) * pl.w_slab_bytes[l] + pl.wb_bytes[l];
-    pl.a_off = off;
-    off += maxslab * A_SLAB_BYTES;
     pl.a0_off = off;
     off += 2 * A0_BYTES;
     pl.stage_off = off;

@@ -216,6 +216,27 @@ __device__ __forceinline__ void tmem_ld(uint32_t taddr, uint32_t (&r)[CW]) {
     else tmem_ld16(taddr, r);
 }
 
+// D[tmem] (+)= A[tmem] * B[smem]: the A operand is read from tensor memory (lane = row, one 32-bit column = two
+// consecutive K elements, so one K = 16 step is 8 columns); 16-bit kinds only.
+template <int CG, bool ACC>
+__device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc) {
+    if (CG == 1)
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                     "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+                     ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "n"(ACC ? 1 : 0) : "memory");
+    else
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                     "tcgen05.mma.cta_group::2.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+                     ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "n"(ACC ? 1 : 0) : "memory");
+}
+// 16 columns of this thread's TMEM lane <- registers
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+        ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+          "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]) : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 // K-major, no swizzle (layer 0, K = 16): core matrices of 8 rows x 16 bytes; the two K chunks of an 8-row
 // group sit 128 B apart (LBO), 8-row groups 256 B apart (SBO).
 __device__ __forceinline__ uint64_t make_desc_l0(uint32_t saddr) {
@@ -288,6 +309,18 @@ __device__ __forceinline__ void epi_store_nb(const uint32_t (&r)[CW], int c0, fl
     for (int k = 0; k < CW / 8; ++k)
         asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(slab + (((ch0 + k) ^ sw) << 4)),
                      "r"(q[4 * k]), "r"(q[4 * k + 1]), "r"(q[4 * k + 2]), "r"(q[4 * k + 3]) : "memory");
+}
+
+// One hidden-layer epilogue step of one warp with the next operand kept in tensor memory: 32 accumulator columns
+// (bias already inside) -> sigma, round to 16 bit -> 16 packed columns, written over the first half of the very
+// columns they came from (taddr = lane | first column of the chunk).
+template <int ACT, bool F16>
+__device__ __forceinline__ void epi_store_tmem(const uint32_t (&r)[32], uint32_t taddr, float slope) {
+    uint32_t q[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k)
+        q[k] = act_pack<ACT, F16>(__uint_as_float(r[2 * k]), __uint_as_float(r[2 * k + 1]), slope);
+    tmem_st16(taddr, q);
 }
 
 // a4: six s-coordinates of one particle -> the K = 16 layer-0 operand row  hi0..hi5, lo0..lo5, 0, 0, 0, 0
