@@ -25,7 +25,11 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
     double* red = reinterpret_cast<double*>(Ws + KC * OC);
 
     const int tid = threadIdx.x;
-    const int og = tid & 15, pg = tid >> 4;
+    // a warp = 8 particle groups x 4 output groups: per k step its lanes read 8 consecutive float4 of the activation
+    // row and 4 consecutive float4 of the weight row -- one shared-memory wavefront each (16 x 2 took three)
+    constexpr int P = TP / 4, PW = P >= 8 ? 8 : P, OW = 32 / PW;     // particle / output groups per warp
+    const int og = ((tid >> 5) / (P / PW)) * OW + (tid & 31) % OW;
+    const int pg = ((tid >> 5) % (P / PW)) * PW + (tid & 31) / OW;
     HbMomAcc acc;
     if (MOM) acc.clear();
     const size_t ntiles = (n + TP - 1) / TP;
