@@ -113,6 +113,18 @@ hb_status hb_lattice_create(double ref_kinetic_energy_MeV, double rest_energy_Me
  * Errors: finalized lattice -> STATE; non-finite or negative QUAD/SBEND length -> INVALID_ARG. */
 hb_status hb_lattice_add_element(hb_lattice *lat, hb_elem_kind kind, double length_m, double param);
 
+/* Change length and parameter of element `index` (0-based position in the order of the add calls; monitors and
+ * surrogate stages count) -- the elements of a beamline are "programmable at run time", and the paper's
+ * optimisation (Nelder-Mead over lens position and strength, one tracking run per evaluation) changes two or
+ * three of them between pushes.  Allowed before and after hb_lattice_finalize; the element keeps its kind.  On a
+ * finalized lattice only the run that holds the element is rebuilt (fp64 concatenation of its maps on the host, R5);
+ * surrogate weights, records and scratch are untouched.  The call synchronises the lattice's device (the element table
+ * of sequential runs is device-resident), so it orders itself after every push enqueued before it; a CUDA graph
+ * captured earlier keeps the old maps and must be re-captured.
+ * Errors: index out of range, or a monitor / surrogate / multipole element -> INVALID_ARG; values as in
+ * hb_lattice_add_element. */
+hb_status hb_lattice_set_element(hb_lattice *lat, int index, double length_m, double param);
+
 /* Append a thin multipole kick (R5x) of order m (1 dipole, 2 quadrupole, 3 sextupole, ... <= 8) with integrated normal
  * and skew strengths kn, ks [m^-(m-1)]:  px - i py -= (kn + i ks)(x + i y)^(m-1)/(m-1)!.  Non-linear for m > 2: the run
  * that holds it is applied element by element in fp64 registers.  Errors as hb_lattice_add_element. */

@@ -18,7 +18,8 @@ COORDS = {"s": 0, "t": 1}
 RUN_MODES = {"composed": 0, "sequential": 1, "sequential_fp32": 2}
 
 EXPORTED_SYMBOLS = [
-    "hb_lattice_create", "hb_lattice_add_element", "hb_lattice_add_multipole", "hb_lattice_add_surrogate",
+    "hb_lattice_create", "hb_lattice_add_element", "hb_lattice_set_element", "hb_lattice_add_multipole",
+    "hb_lattice_add_surrogate",
     "hb_lattice_set_run_mode",
     "hb_lattice_finalize", "hb_lattice_num_monitors", "hb_lattice_num_launches", "hb_lattice_ref_bg_out",
     "hb_push", "hb_push_moments", "hb_push_host", "hb_moments", "hb_moments_scratch_bytes", "hb_moments_merge",
@@ -72,6 +73,7 @@ def lib():
     L.hb_lattice_create.argtypes = [c_double, c_double, POINTER(c_void_p)]
     L.hb_lattice_add_element.argtypes = [c_void_p, c_int, c_double, c_double]
     L.hb_lattice_add_multipole.argtypes = [c_void_p, c_int, c_double, c_double]
+    L.hb_lattice_set_element.argtypes = [c_void_p, c_int, c_double, c_double]
     L.hb_lattice_add_surrogate.argtypes = [c_void_p, POINTER(_SurrogateDesc)]
     L.hb_lattice_set_run_mode.argtypes = [c_void_p, c_int]
     L.hb_lattice_finalize.argtypes = [c_void_p, c_int]
@@ -139,6 +141,10 @@ def hb_lattice_add_multipole(lat, order: int, kn: float, ks: float = 0.0):
 def hb_lattice_add_element(lat, kind, length_m: float = 0.0, param: float = 0.0):
     k = ELEM_KINDS[kind] if isinstance(kind, str) else int(kind)
     _check(lib().hb_lattice_add_element(lat, k, float(length_m), float(param)), "hb_lattice_add_element")
+
+
+def hb_lattice_set_element(lat, index: int, length_m: float = 0.0, param: float = 0.0):
+    _check(lib().hb_lattice_set_element(lat, int(index), float(length_m), float(param)), "hb_lattice_set_element")
 
 
 def hb_lattice_add_surrogate(lat, widths, W, b, act, in_mean, in_std, out_mean, out_std, coord="s",
@@ -328,6 +334,10 @@ class Lattice:
 
     def add_element(self, kind, length_m=0.0, param=0.0):
         hb_lattice_add_element(self._h, kind, length_m, param)
+
+    def set_element(self, index, length_m=0.0, param=0.0):
+        """re-set length / parameter of element `index` (position in the description's element list)"""
+        hb_lattice_set_element(self._h, index, length_m, param)
 
     def add_surrogate(self, *a, **k):
         hb_lattice_add_surrogate(self._h, *a, **k)

@@ -66,6 +66,8 @@ struct Segment {
     int type;
     HbRunMap map;          // SEG_RUN composed
     int seq_off, seq_cnt;  // SEG_RUN sequential: range in d_seq
+    int e_lo, e_hi;        // SEG_RUN: its elements are lat->elems[e_lo, e_hi)
+    double bg;             // SEG_RUN: (beta gamma) of the reference inside the run
     bool nonlinear;        // SEG_RUN holds a non-linear element: no composed map, always the fp64 sequential kernel
     HbSurDev sd;           // SEG_SUR
     bool tc;               // SEG_SUR: tensor-core kernel
@@ -296,6 +298,54 @@ hb_status hb_lattice_add_element(hb_lattice* lat, hb_elem_kind kind, double L, d
     return HB_OK;
 }
 
+hb_status hb_lattice_set_element(hb_lattice* lat, int index, double L, double param) {
+    if (!lat) return fail(HB_ERR_INVALID_ARG, "lattice is NULL");
+    if (index < 0 || (size_t)index >= lat->elems.size())
+        return fail(HB_ERR_INVALID_ARG, "element index %d out of range (lattice has %zu elements)", index, lat->elems.size());
+    Elem& e = lat->elems[(size_t)index];
+    if (e.kind == HB_ELEM_MONITOR || e.kind == 4 || e.kind == HB_ELEM_MULTIPOLE)
+        return fail(HB_ERR_INVALID_ARG, "element %d is a monitor, surrogate or multipole: only elements added with "
+                                        "hb_lattice_add_element(length, param) can be re-set", index);
+    const bool is_drift = e.kind == HB_ELEM_DRIFT || e.kind == HB_ELEM_DRIFT_EXACT;
+    if (!std::isfinite(L)) return fail(HB_ERR_INVALID_ARG, "length must be finite");
+    if (!is_drift && (!std::isfinite(param) || L < 0.0))
+        return fail(HB_ERR_INVALID_ARG, "quad/plens/sbend need a finite parameter and length >= 0");
+    if (!lat->finalized) {
+        e.L = L;
+        e.param = is_drift ? 0.0 : param;
+        return HB_OK;
+    }
+    // finalized: rebuild the one run that holds the element (its reference energy is fixed by the stages before it)
+    for (Segment& sg : lat->segs) {
+        if (sg.type != SEG_RUN || index < sg.e_lo || index >= sg.e_hi) continue;
+        const Elem old = e;
+        e.L = L;
+        e.param = is_drift ? 0.0 : param;
+        Mat6 M = mat_identity();
+        std::vector<HbSeqElem> seq;
+        for (int k = sg.e_lo; k < sg.e_hi; ++k) {
+            M = mat_mul(elem_matrix(lat->elems[(size_t)k], sg.bg), M);
+            seq.push_back(seq_elem(lat->elems[(size_t)k], sg.bg));
+        }
+        // the element table of sequential runs lives on the device: no push may still be reading it
+        int prev = 0;
+        cudaError_t ce = cudaGetDevice(&prev);
+        if (ce == cudaSuccess) ce = cudaSetDevice(lat->device);
+        if (ce == cudaSuccess) ce = cudaDeviceSynchronize();
+        if (ce == cudaSuccess)
+            ce = cudaMemcpy(lat->d_seq + sg.seq_off, seq.data(), seq.size() * sizeof(HbSeqElem), cudaMemcpyHostToDevice);
+        cudaSetDevice(prev);
+        if (ce != cudaSuccess) {
+            e = old;
+            return fail(HB_ERR_CUDA, "hb_lattice_set_element: %s", cudaGetErrorString(ce));
+        }
+        for (int r = 0; r < 6; ++r)
+            for (int c = 0; c < 6; ++c) sg.map.m[r * 6 + c] = (float)M.m[r][c];
+        return HB_OK;
+    }
+    return fail(HB_ERR_STATE, "element %d belongs to no run", index);
+}
+
 hb_status hb_lattice_add_multipole(hb_lattice* lat, int order, double kn, double ks) {
     if (!lat) return fail(HB_ERR_INVALID_ARG, "lattice is NULL");
     if (lat->finalized) return fail(HB_ERR_STATE, "lattice already finalized");
@@ -520,6 +570,8 @@ hb_status hb_lattice_finalize(hb_lattice* lat, int device) {
             s.type = SEG_RUN;
             s.monitor = -1;
             s.seq_off = (int)seq.size();
+            s.e_lo = (int)i;
+            s.bg = bg;
             Mat6 M = mat_identity();
             while (i < lat->elems.size() && is_conventional(lat->elems[i].kind)) {
                 s.nonlinear = s.nonlinear || is_nonlinear(lat->elems[i].kind);
@@ -528,6 +580,7 @@ hb_status hb_lattice_finalize(hb_lattice* lat, int device) {
                 ++i;
             }
             s.seq_cnt = (int)seq.size() - s.seq_off;
+            s.e_hi = (int)i;
             for (int r = 0; r < 6; ++r)
                 for (int c = 0; c < 6; ++c) s.map.m[r * 6 + c] = (float)M.m[r][c];
             lat->segs.push_back(s);

@@ -511,3 +511,91 @@ def test_lens_optimisation_loop_on_the_gpu(hb):
     for dk in ([0.3, 0.0], [0.0, -0.3]):                   # and it is a (local) minimum of the oracle's objective too
         _, r2 = oracle.push(line(res.x + np.array(dk)), x)
         assert r2[-1][6] + r2[-1][17] >= f_ref * (1 - 1e-6)
+
+
+@pytest.mark.parametrize("run_mode", ["composed", "sequential"])
+def test_set_element_rebuilds_only_its_run(hb, run_mode):
+    """hb_lattice_set_element on a finalized lattice (P:68 'programmable at run time'): elements before and behind a
+    COORD_T surrogate stage with energy gain (so the two runs have different reference momenta) are re-set, and the
+    push must equal the oracle's push of the re-described lattice; the untouched lattice object is reused."""
+    import torch
+    desc, x = wl.config4(prec="fp32", n=30_000)
+    els = desc["elements"]
+    idx = [i for i, e in enumerate(els) if e["kind"] in ("quad", "drift", "sbend")]
+    sur = [i for i, e in enumerate(els) if e["kind"] == "surrogate"]
+    before = [i for i in idx if i < sur[0]] or [i for i in idx if i < sur[1]]
+    behind = [i for i in idx if i > sur[-1]]
+    assert before and behind
+    lat = hb.Lattice.from_description(desc, run_mode=run_mode, device=0)
+    c = hb.to_device(x)
+    lat.push_moments(c)                                   # a push with the original elements first
+    import copy
+    new = copy.deepcopy(desc)
+    for i, scale in ((before[0], 1.3), (behind[0], 0.7), (behind[-1], 1.1)):
+        e = new["elements"][i]
+        e["L"] = e["L"] * scale
+        par = {"quad": "k", "sbend": "theta"}.get(e["kind"])
+        if par:
+            e[par] = e[par] * scale
+        lat.set_element(i, e["L"], e[par] if par else 0.0)
+    c = hb.to_device(x)
+    rec = lat.push_moments(c).cpu().numpy()
+    torch.cuda.synchronize()
+    got = hb.to_host(c)
+    lat.close()
+    ref, ref_rec = oracle.push(new, x)
+    err = np.max(np.abs(got.astype(np.float64) - ref), axis=1) / ref.std(axis=1)
+    print("set_element", run_mode, "max err/std", err)
+    assert err.max() <= 1e-5
+    assert np.allclose(rec[-1][:6], np.asarray(ref_rec)[-1][:6], rtol=1e-4, atol=1e-9)
+    old, _ = oracle.push(desc, x)
+    assert (np.max(np.abs(old - ref), axis=1) / ref.std(axis=1)).max() > 1e-3     # the change was not a no-op
+
+
+def test_stagewise_lens_optimisation_without_rebuilding(hb):
+    """The paper's procedure on one cell: minimise eps_x behind a (synthetic) surrogate stage over the POSITION
+    and STRENGTH of the plasma lens in front of it -- drift(d), lens(k), drift(D - d), stage, monitor.  One lattice is
+    built once (weights packed and uploaded once); every Nelder-Mead evaluation is three hb_lattice_set_element calls
+    and one hb_push_moments.  The optimum is checked with the fp64 oracle."""
+    import torch
+    from scipy.optimize import minimize
+    widths = [6, 64, 64, 6]
+    W, b = wl.make_mlp(widths, "xavier", 5, 0)
+    x = wl.correlated_bunch(60_000, 41)
+    f64 = x.astype(np.float64)
+    sur = wl.surrogate(widths, W, b, "tanh", f64.mean(axis=1), f64.std(axis=1) * 3.0, f64.mean(axis=1), f64.std(axis=1),
+                       prec="fp32")
+    D, LL = 1.2, 0.05
+
+    def line(v):
+        d, k = float(v[0]), float(v[1])
+        return wl.lattice([wl.drift(d), wl.plens(LL, k), wl.drift(D - d), sur, wl.monitor()])
+
+    def eps_x(rec):
+        return float(np.sqrt(max(rec[6] * rec[12] - rec[7] ** 2, 0.0)))
+
+    lat = hb.Lattice.from_description(line([0.6, 1.0]), device=0)
+    c0 = torch.from_numpy(x).cuda()
+    work = torch.empty_like(c0)
+    evals = []
+
+    def objective(v):
+        d = min(max(float(v[0]), 0.0), D)
+        lat.set_element(0, d, 0.0)
+        lat.set_element(1, LL, float(v[1]))
+        lat.set_element(2, D - d, 0.0)
+        work.copy_(c0)
+        rec = lat.push_moments(work).cpu().numpy()[-1]
+        evals.append(1)
+        return eps_x(rec)
+
+    start = np.array([0.6, 1.0])
+    f0 = objective(start)
+    res = minimize(objective, start, method="Nelder-Mead", options={"xatol": 1e-3, "fatol": 1e-13, "maxfev": 150})
+    lat.close()
+    assert len(evals) > 20 and res.fun <= f0
+    v = np.array([min(max(res.x[0], 0.0), D), res.x[1]])
+    _, ref_rec = oracle.push(line(v), x)
+    f_ref = eps_x(np.asarray(ref_rec)[-1])
+    print("stagewise optimisation:", len(evals), "evaluations, eps_x", f0, "->", res.fun, "oracle at optimum", f_ref)
+    assert abs(res.fun - f_ref) <= 1e-3 * f_ref

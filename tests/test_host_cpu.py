@@ -158,3 +158,20 @@ def test_moments_merge_against_plain_moments(hb):
     exp = hb.hb_moments_merge(out, 1000, r2, 500)
     assert hb.lib().hb_moments_merge(out.ctypes.data_as(pd), 1000, r2.ctypes.data_as(pd), 500, out.ctypes.data_as(pd)) == 0
     assert np.array_equal(out, exp)
+
+
+def test_set_element_host_validation(hb):
+    """hb_lattice_set_element before finalize is pure host logic: index and value checks, kinds that cannot be re-set"""
+    lat = hb.hb_lattice_create(1000.0, wl.ELECTRON_MEV)
+    hb.hb_lattice_add_element(lat, "drift", 1.0)
+    hb.hb_lattice_add_element(lat, "quad", 0.3, 2.0)
+    hb.hb_lattice_add_element(lat, "monitor")
+    hb.hb_lattice_add_multipole(lat, 3, 0.5, 0.0)
+    hb.hb_lattice_set_element(lat, 0, -0.5)              # negative drift length is allowed (as in add_element)
+    hb.hb_lattice_set_element(lat, 1, 0.2, -3.0)
+    for args in ((4, 1.0, 0.0), (-1, 1.0, 0.0), (2, 1.0, 0.0), (3, 1.0, 0.0), (1, -0.1, 1.0), (1, 0.1, float("nan")),
+                 (0, float("inf"), 0.0)):
+        with pytest.raises(hb.HbError) as e:
+            hb.hb_lattice_set_element(lat, *args)
+        assert e.value.status == 1                       # HB_ERR_INVALID_ARG
+    hb.hb_lattice_destroy(lat)
