@@ -8,12 +8,20 @@
 //   warps 0-3   IO warps      : a4 prologue (s->t R6 in deviation form, normalise R8, hi/lo split, layer-0
 //                               operand) of tile i+1, then a6 epilogue of tile i (tcgen05.ld of the 6 outputs,
 //                               de-normalise R8, reference update R7, t->s R6, coalesced store, fp64 moments R10).
-//   warps 4..   4G hidden-layer epilogue warps: tcgen05.ld of the accumulator, + bias (fp32), sigma (Eq. 1/2,
-//                               tanh), round to 16 bit, write the next A operand in the 128-byte-swizzled
-//                               K-major layout the MMA reads.  Hidden activations never leave the SM.
-// Pipeline (v2).  The accumulator is double-buffered in TMEM (layer l writes D[l & 1]) and the next A operand
-// is handed to the MMA issuer per 64-column K slab: the MMAs of layer l+1 start as soon as the epilogue of
-// layer l has produced slab 0 and then run back to back while the epilogue finishes the other slabs, so the
+//   warps 4..   4G hidden-layer epilogue warps: tcgen05.ld of 32 accumulator columns (bias already inside, see
+//                               below), sigma (Eq. 1/2, tanh), round to 16 bit, tcgen05.st of the 16 packed columns
+//                               over the first half of the columns just read.  Hidden activations never leave
+//                               tensor memory (they never touch HBM).
+// Bias.  The layer-0 operand row is  hi0..5, lo0..5, 1, 1, 0, 0;  W_0 carries b_hi, b_lo (bias rounded to the
+// operand type + rounded remainder) in K columns 12, 13.  Every hidden layer gets one extra K = 16 MMA of that same
+// operand tile against a bias block (b_hi, b_lo in columns 12, 13, zeros elsewhere) with accumulate = 0, issued
+// before the layer's first K slab is awaited.
+// Operand.  Layer l >= 1 reads A from tensor memory (tcgen05.mma [d], [a], b-desc): K step kappa of slab j is the
+// 8 columns at 64 j + 32 (kappa / 2) + 8 (kappa mod 2) of D[(l-1) & 1]; shared memory only feeds B.
+// Pipeline.  The accumulator is double-buffered in TMEM (layer l writes D[l & 1]) and the next operand is handed
+// to the MMA issuer per 64-column K slab: the MMAs of layer l+1 start as soon as the epilogue of layer l has
+// converted slab 0 and then run back to back while the epilogue finishes the other slabs; layer 0 of the next
+// tile is issued directly behind the last layer of the current one.
 #include "hb_tc_common.cuh"
 
 namespace {
