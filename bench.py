@@ -241,6 +241,7 @@ def run_reference(args, rank, world):
 
 def kernel_extras(torch, hb, args, pk, flush, dev):
     """per-kernel measurements at N = 1e7 beside the headline step"""
+    p16 = args.prec if args.prec in ("f16", "bf16") else "f16"      # 16-bit operand type of the tensor-core extras
     out = []
     n = args.n or 10_000_000
     reps = 10
@@ -332,14 +333,14 @@ def kernel_extras(torch, hb, args, pk, flush, dev):
                                  "frac": ach / fma_peak, "traffic": None}})
         del x3
         # (b2) one C5 stage (6-512^4-6 tanh, weights streamed from L2) at N = 1e7
-        desc5, _ = wl.config5(prec="bf16", particles=False)
+        desc5, _ = wl.config5(prec=p16, particles=False)
         d5 = wl.lattice(desc5["elements"][:2])
         x5 = wl.gaussian_bunch(n, 5)
         fl5 = wl.flops_per_particle(d5["elements"][0]["widths"])
         ms, seg = measure(d5, x5, "sur", True, steps=5)
         k_ms = float(seg[0])
         tf = fl5 * n / (k_ms * 1e-3) / 1e12
-        out.append({"kernel": "hb_sur_tcs_kernel<bf16> (streamed weights)", "workload": "one C5 stage 6-512^4-6 tanh, N=%d" % n, "ms": k_ms,
+        out.append({"kernel": "hb_sur_tcs_kernel<%s> (streamed weights)" % p16, "workload": "one C5 stage 6-512^4-6 tanh, N=%d" % n, "ms": k_ms,
                     "particle_inferences_per_s": n / (k_ms * 1e-3),
                     "roofline": {"bound": "tensor", "achieved": tf, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
                                  "frac": tf / pk["bf16_tflops"], "frac_of_sustained": tf / pk["bf16_tflops_sustained"],
@@ -348,12 +349,12 @@ def kernel_extras(torch, hb, args, pk, flush, dev):
         # (b3) the paper's own network shapes on the layered kernel, one stage at N = 1e7; the paper's timings
         # (P:199, 1 x A100, PyTorch) are context, not the target
         for wname, (wd, hd, paper_ms) in (("P900", (900, 5, 1120.0)), ("P700", (700, 3, 494.0))):
-            descp, xp = wl.paper_net(wd, hd, prec="bf16", n=n)
+            descp, xp = wl.paper_net(wd, hd, prec=p16, n=n)
             flp = wl.flops_per_particle(descp["elements"][0]["widths"])
             ms, seg = measure(descp, xp, "sur", True, steps=3)
             k_ms = float(seg[0])
             tf = flp * n / (k_ms * 1e-3) / 1e12
-            out.append({"kernel": "hb_sur_tcw_kernel<bf16> (%d launches: one per layer and 2^20-particle chunk)" % ((hd + 1) * ((n + (1 << 20) - 1) >> 20)),
+            out.append({"kernel": "hb_sur_tcw_kernel<%s> (%d launches: one per layer and 2^20-particle chunk)" % (p16, (hd + 1) * ((n + (1 << 20) - 1) >> 20)),
                         "workload": "%s: one stage 6-%d^%d-6 PReLU, N=%d" % (wname, wd, hd, n), "ms": k_ms,
                         "particle_inferences_per_s": n / (k_ms * 1e-3), "paper_ms_per_stage_a100": paper_ms if n == 10_000_000 else None,
                         "roofline": {"bound": "tensor", "achieved": tf, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
@@ -361,7 +362,7 @@ def kernel_extras(torch, hb, args, pk, flush, dev):
                                      "traffic": None, "peak_source": pk["source"]}})
             del xp
         # (c) C4 hybrid lattice (all rows a1-a7 in one push)
-        desc4, x4 = wl.config4(prec="bf16", n=n)
+        desc4, x4 = wl.config4(prec=p16, n=n)
         ms, seg = measure(desc4, x4, "c4", True)
         fl4 = wl.flops_per_particle([6, 128, 128, 128, 6])
         kinds = segment_kinds(desc4)
