@@ -502,8 +502,10 @@ TcShape choose_shape(int n_linear, const int* widths, TcPlan& pl) {
     const char* force = getenv("HB_TC_FORCE_CG");
     const char* occ2 = getenv("HB_TC_OCC2");
     const bool allow_occ2 = !(occ2 && occ2[0] == '0') && !force;
-    if (allow_occ2 && make_plan(2, n_linear, widths, pl) && (size_t)pl.total + 2048 <= SMEM_LIMIT / 2 && pl.tmem_cols <= 256)
-        return {2, 1, 2};
+    // single CTAs where the whole net fits one (local hand-over barriers: C4 1.45 -> 1.40 ms), else CTA pairs
+    for (int cg = 1; cg <= 2 && allow_occ2; ++cg)
+        if (make_plan(cg, n_linear, widths, pl) && (size_t)pl.total + 2048 <= SMEM_LIMIT / 2 && pl.tmem_cols <= 256)
+            return {cg, 1, 2};
     const int cg = choose_cg(n_linear, widths, pl);
     return {cg, 2, 1};
 }
