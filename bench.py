@@ -439,9 +439,13 @@ def main():
     total_ms = float(t.item())
     ms_step = total_ms / args.steps
     assert bool(torch.isfinite(rec).all()), "non-finite moments"
+    merged_ok = None
     if world > 1:       # monitor records of the whole N-rank bunch: 224 B per monitor and rank, outside the timed region
-        merged = hb.allgather_merge_records(rec, n)
-        assert bool(np.isfinite(merged).all()), "non-finite merged records"
+        try:
+            merged = hb.allgather_merge_records(rec, n)
+            merged_ok = bool(np.isfinite(merged).all())
+        except Exception as ex:                     # reported, never fatal to the timing line
+            merged_ok = "failed: %s" % (ex,)
 
     # ---- end to end through the C ABI with HOST buffers: hb_push_host (pinned host arrays in, results and moment
     # records back in host memory when the call returns; H2D, kernels, D2H pipelined in chunks inside the library).
@@ -507,6 +511,7 @@ def main():
                 "d2h_bytes_per_step": int(host.numel() * 4 + rec_bytes), "ms_per_step": e2e_ms,
                 "api": "hb_push_host(chunks=%d): pinned host arrays, synchronous, host clock" % e2e_chunks},
         "gpu_launches": int(args.steps * lat.num_launches(True)),
+        "records_merged_over_ranks": merged_ok,
         "roofline": roof,
     }
     gpu_head = work[:, :1 << 22].cpu().numpy() if (rank == 0 and world == 1 and not args.no_cpu_baseline) else None
