@@ -2,16 +2,19 @@
 //
 // One block owns a tile of TP particles.  Activations live in shared memory as [feature][particle]
 // (two ping-pong buffers); the transposed weights W^T [k][n] (packed, zero-padded to 64 outputs, by
-// hb_api.cu) are streamed through a [32][64] shared slab (the next slab is fetched into registers while
-// the current one is multiplied).  Each thread owns a 4-particle x 4-output register tile.  Partial sums of each 32-wide K chunk are formed separately and then added (shorter
-// rounding chains), bias is added last in fp32, tanh is tanhf.
+// hb_api.cu) are streamed through two [16][64] shared slabs filled by cp.async (slab c + 1 lands while
+// slab c is multiplied: one barrier per slab).  Each thread owns a 4-particle x 4-output register tile; the
+// operands of k step k + 1 are loaded before the 16 FFMA of step k.  The kernel is bound by the shared-memory
+// data path, so the lane -> (particle group, output group) map is the one for which ncu counts two wavefronts
+// per LDS.128 for both operands (profiles/r1_fp32.md).  Partial sums of each 32-wide K span are formed
+// separately and then added (shorter rounding chains), bias is added last in fp32, tanh is tanhf.
 // Prologue (s->t R6, normalise R8) and epilogue (de-normalise R8, reference R7, t->s R6, moments R10)
 // are fused: hidden activations never touch HBM (data preparation is 1-2 % of the push).
 #include "hb_device.cuh"
 
 #include <cstdlib>
 
-#define KC 32
+#define KC 16
 #define OC 64
 
 template <int TP, int ACT, bool MOM>
@@ -21,17 +24,23 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
     extern __shared__ __align__(16) float smem[];
     float* actA = smem;                          // [hmax][TP]
     float* actB = actA + (size_t)hmax * TP;      // [hmax][TP]
-    float* Ws = actB + (size_t)hmax * TP;        // [KC][OC]
-    double* red = reinterpret_cast<double*>(Ws + KC * OC);
+    float* Ws = actB + (size_t)hmax * TP;        // [2][KC][OC]
+    double* red = reinterpret_cast<double*>(Ws + 2 * KC * OC);
+    const uint32_t ws_addr = (uint32_t)__cvta_generic_to_shared(Ws);
 
     const int tid = threadIdx.x;
-    // a warp = 8 particle groups x 4 output groups: per k step its lanes read 8 consecutive float4 of the activation
-    // row and 4 consecutive float4 of the weight row -- one shared-memory wavefront each (16 x 2 took three)
+    // a warp = 8 particle groups x 4 output groups.  Lane bits (4,3,0) pick the particle group and bits (2,1) the
+    // output group: both LDS.128 of a k step then cost two shared-memory wavefronts (with output group = lane % 4
+    // the weight load took four: ncu, L1 Wavefronts Shared per instruction)
     constexpr int P = TP / 4, PW = P >= 8 ? 8 : P, OW = 32 / PW;     // particle / output groups per warp
-    const int og = ((tid >> 5) / (P / PW)) * OW + (tid & 31) % OW;
-    const int pg = ((tid >> 5) % (P / PW)) * PW + (tid & 31) / OW;
+    const int lane = tid & 31;
+    const int ol = PW == 8 ? ((lane >> 1) & 3) : lane % OW;
+    const int pl = PW == 8 ? ((lane & 1) | ((lane >> 3) << 1)) : lane / OW;
+    const int og = ((tid >> 5) / (P / PW)) * OW + ol;
+    const int pg = ((tid >> 5) % (P / PW)) * PW + pl;
     HbMomAcc acc;
     if (MOM) acc.clear();
+    int c = 0;                                   // running K-chunk counter (selects the weight-slab buffer)
     const size_t ntiles = (n + TP - 1) / TP;
 
     for (size_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
@@ -53,55 +62,74 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
             const bool last = (l == sd.n_linear - 1);
             const float slope = sd.prelu[l];
             for (int o0 = 0; o0 < npad; o0 += OC) {
-                float tot[4][4];
+                float tot[4][4], part[4][4];
 #pragma unroll
                 for (int a = 0; a < 4; ++a)
 #pragma unroll
-                    for (int b = 0; b < 4; ++b) tot[a][b] = 0.0f;
-                // weight slab of the next K chunk travels global -> registers while this chunk is being multiplied
-                constexpr int PER = (KC * (OC / 4) + NT - 1) / NT;      // float4 per thread and slab
-                float4 pre[PER];
-                auto fetch = [&](int k0) {
-                    const int kk = min(KC, K - k0);
+                    for (int b = 0; b < 4; ++b) { tot[a][b] = 0.0f; part[a][b] = 0.0f; }
+                // weight slab of K chunk c: global -> shared by cp.async into buffer c & 1 while chunk c - 1 is being
+                // multiplied; every thread moves PER 16-byte pieces (rows past K are not fetched and not read)
+                constexpr int PER = KC * (OC / 4) / NT;
+                static_assert(PER * NT == KC * (OC / 4), "slab pieces must divide over the threads");
+                const float* wsrc = Wt + (size_t)(tid >> 4) * npad + o0 + 4 * (tid & 15);
+                const size_t ustep = (size_t)(NT / 16) * npad;
+                auto fetch = [&](int k0, int buf) {
+                    const float* s0 = wsrc + (size_t)k0 * npad;
+                    const uint32_t d0 = ws_addr + (uint32_t)(buf * KC * OC * 4 + tid * 16);
 #pragma unroll
-                    for (int u = 0; u < PER; ++u) {
-                        const int idx = tid + u * NT;
-                        const int k = idx / (OC / 4), c4 = idx % (OC / 4);
-                        pre[u] = k < kk ? __ldg(reinterpret_cast<const float4*>(Wt + (size_t)(k0 + k) * npad + o0) + c4)
-                                        : make_float4(0.f, 0.f, 0.f, 0.f);
-                    }
+                    for (int u = 0; u < PER; ++u)
+                        if (k0 + (tid >> 4) + u * (NT / 16) < K)
+                            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d0 + u * NT * 16),
+                                         "l"(s0 + u * ustep) : "memory");
+                    asm volatile("cp.async.commit_group;" ::: "memory");
                 };
-                fetch(0);
-                for (int k0 = 0; k0 < K; k0 += KC) {
+                fetch(0, c & 1);          // c runs on over output blocks and layers: buffer c & 1 was last read in
+                                          // chunk c - 2, which every warp has left (barrier of chunk c - 1)
+                for (int k0 = 0; k0 < K; k0 += KC, ++c) {
                     const int kk = min(KC, K - k0);
-                    __syncthreads();          // previous slab consumed; layer input complete
+                    asm volatile("cp.async.wait_all;" ::: "memory");
+                    __syncthreads();          // slab c visible; slab c - 1 consumed by every warp; layer input complete
+                    if (k0 + KC < K) fetch(k0 + KC, (c + 1) & 1);
+                    const float* __restrict__ ap = in + (size_t)k0 * TP + 4 * pg;
+                    const float* __restrict__ wp = Ws + (c & 1) * (KC * OC) + 4 * og;
+                    if (kk == KC) {
+                        // operands of step k + 1 are loaded before the 16 FFMA of step k (the shared-memory latency
+                        // was exposed with three warps per scheduler: profiles/r1_fp32.md)
+                        float4 av = *reinterpret_cast<const float4*>(ap), wv = *reinterpret_cast<const float4*>(wp);
 #pragma unroll
-                    for (int u = 0; u < PER; ++u) {
-                        const int idx = tid + u * NT;
-                        if (idx < KC * (OC / 4)) reinterpret_cast<float4*>(Ws)[idx] = pre[u];
+                        for (int k = 0; k < KC; ++k) {
+                            float4 an = av, wn = wv;
+                            if (k + 1 < KC) {
+                                an = *reinterpret_cast<const float4*>(ap + (k + 1) * TP);
+                                wn = *reinterpret_cast<const float4*>(wp + (k + 1) * OC);
+                            }
+                            const float a4[4] = {av.x, av.y, av.z, av.w};
+                            const float w4[4] = {wv.x, wv.y, wv.z, wv.w};
+#pragma unroll
+                            for (int a = 0; a < 4; ++a)
+#pragma unroll
+                                for (int b = 0; b < 4; ++b) part[a][b] = fmaf(a4[a], w4[b], part[a][b]);
+                            av = an; wv = wn;
+                        }
+                    } else {
+                        for (int k = 0; k < kk; ++k) {
+                            const float4 av = *reinterpret_cast<const float4*>(ap + k * TP);
+                            const float4 wv = *reinterpret_cast<const float4*>(wp + k * OC);
+                            const float a4[4] = {av.x, av.y, av.z, av.w};
+                            const float w4[4] = {wv.x, wv.y, wv.z, wv.w};
+#pragma unroll
+                            for (int a = 0; a < 4; ++a)
+#pragma unroll
+                                for (int b = 0; b < 4; ++b) part[a][b] = fmaf(a4[a], w4[b], part[a][b]);
+                        }
                     }
-                    __syncthreads();
-                    if (k0 + KC < K) fetch(k0 + KC);
-                    float part[4][4];
-#pragma unroll
-                    for (int a = 0; a < 4; ++a)
-#pragma unroll
-                        for (int b = 0; b < 4; ++b) part[a][b] = 0.0f;
-#pragma unroll 8
-                    for (int k = 0; k < kk; ++k) {
-                        const float4 av = *reinterpret_cast<const float4*>(in + (size_t)(k0 + k) * TP + 4 * pg);
-                        const float4 wv = *reinterpret_cast<const float4*>(Ws + k * OC + 4 * og);
-                        const float a4[4] = {av.x, av.y, av.z, av.w};
-                        const float w4[4] = {wv.x, wv.y, wv.z, wv.w};
+                    // partial sums of each 32-wide K span are formed separately and then added (shorter rounding chains)
+                    if (((k0 / KC) & (32 / KC - 1)) == 32 / KC - 1 || k0 + KC >= K) {
 #pragma unroll
                         for (int a = 0; a < 4; ++a)
 #pragma unroll
-                            for (int b = 0; b < 4; ++b) part[a][b] = fmaf(a4[a], w4[b], part[a][b]);
+                            for (int b = 0; b < 4; ++b) { tot[a][b] += part[a][b]; part[a][b] = 0.0f; }
                     }
-#pragma unroll
-                    for (int a = 0; a < 4; ++a)
-#pragma unroll
-                        for (int b = 0; b < 4; ++b) tot[a][b] += part[a][b];
                 }
                 const float4 bv = __ldg(reinterpret_cast<const float4*>(bias + o0) + og);
                 const float b4[4] = {bv.x, bv.y, bv.z, bv.w};
@@ -143,7 +171,7 @@ template <int TP, bool MOM>
 static cudaError_t launch_tp(const HbParticles& p, size_t n, const HbSurDev& sd, int hmax, double* partials,
                              int grid, cudaStream_t s) {
     constexpr int NT = (TP / 4) * 16;
-    const size_t smem = ((size_t)2 * hmax * TP + KC * OC) * sizeof(float) + (NT / 32) * HB_NMOM * sizeof(double);
+    const size_t smem = ((size_t)2 * hmax * TP + 2 * KC * OC) * sizeof(float) + (NT / 32) * HB_NMOM * sizeof(double);
 #define HB_LAUNCH_ACT(A)                                                                                         \
     {                                                                                                            \
         cudaError_t e = cudaFuncSetAttribute(hb_sur_fp32_kernel<TP, A, MOM>,                                     \
@@ -170,7 +198,7 @@ cudaError_t hb_launch_sur_fp32(const HbParticles& p, size_t n, const HbSurDev& s
     const char* force = getenv("HB_FP32_TP");
     int tp = hmax <= 128 ? 64 : (hmax <= 768 ? 32 : 16);
     if (force) tp = atoi(force) == 64 && hmax <= 384 ? 64 : (atoi(force) == 16 ? 16 : (hmax <= 768 ? 32 : 16));
-    const size_t smem_blk = ((size_t)2 * hmax * tp + KC * OC) * sizeof(float) + 1024;
+    const size_t smem_blk = ((size_t)2 * hmax * tp + 2 * KC * OC) * sizeof(float) + 1024;
     int per_sm = (int)((227 * 1024) / smem_blk);
     if (per_sm < 1) per_sm = 1;
     if (per_sm > 4) per_sm = 4;
