@@ -61,6 +61,39 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
             const float* __restrict__ bias = sd.b32 + sd.b32_off[l];
             const bool last = (l == sd.n_linear - 1);
             const float slope = sd.prelu[l];
+            if (last && sd.widths[l + 1] <= 8) {
+                // Narrow output layer (6 of the 64 padded outputs are real): thread = (particle, quarter of K),
+                // six dot products over its K quarter, partial sums through the free activation buffer.  The
+                // weight row is the same address for a whole warp (one broadcast load from L1).
+                constexpr int NQ = NT / TP;                      // = 4
+                const int nout = sd.widths[l + 1];
+                const int pl_ = tid % TP, kq = tid / TP;
+                const int KQ = (K + NQ - 1) / NQ;
+                const int kb = kq * KQ, ke = min(K, kb + KQ);
+                float d[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+                __syncthreads();                                 // layer input complete
+                for (int k = kb; k < ke; ++k) {
+                    const float a = in[(size_t)k * TP + pl_];
+                    const float4 w0 = __ldg(reinterpret_cast<const float4*>(Wt + (size_t)k * npad));
+                    const float4 w1 = __ldg(reinterpret_cast<const float4*>(Wt + (size_t)k * npad) + 1);
+                    d[0] = fmaf(a, w0.x, d[0]); d[1] = fmaf(a, w0.y, d[1]);
+                    d[2] = fmaf(a, w0.z, d[2]); d[3] = fmaf(a, w0.w, d[3]);
+                    d[4] = fmaf(a, w1.x, d[4]); d[5] = fmaf(a, w1.y, d[5]);
+                    d[6] = fmaf(a, w1.z, d[6]); d[7] = fmaf(a, w1.w, d[7]);
+                }
+#pragma unroll
+                for (int j = 0; j < 8; ++j) out[(size_t)(8 + j * NQ + kq) * TP + pl_] = d[j];
+                __syncthreads();
+                if (tid < TP) {
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        float z = 0.0f;
+#pragma unroll
+                        for (int q = 0; q < NQ; ++q) z += out[(size_t)(8 + j * NQ + q) * TP + tid];
+                        if (j < nout) out[(size_t)j * TP + tid] = z + __ldg(bias + j);
+                    }
+                }
+            } else
             for (int o0 = 0; o0 < npad; o0 += OC) {
                 float tot[4][4], part[4][4];
 #pragma unroll
