@@ -17,22 +17,25 @@
 #define KC 16
 #define OC 64
 
-template <int TP, int ACT, bool MOM>
-__global__ void __launch_bounds__((TP / 4) * 16, TP == 64 ? 1 : 3)
+// R = 1: 4 x 4 register tile, OCB = 64-wide output blocks; R = 2: 8 x 8 register tile (two float4 per operand and
+// k step: half the shared-memory wavefronts per FFMA), OCB = 256-wide output blocks, one 256-thread block of 64
+// particles per SM (two warps per scheduler at ~240 registers).
+template <int TP, int ACT, bool MOM, int R, int OCB>
+__global__ void __launch_bounds__((TP / (4 * R)) * (OCB / (4 * R)), (TP == 64 || R == 2) ? 1 : 3)
 hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, int hmax, double* __restrict__ partials) {
-    constexpr int NT = (TP / 4) * 16;
+    constexpr int NT = (TP / (4 * R)) * (OCB / (4 * R));
     extern __shared__ __align__(16) float smem[];
     float* actA = smem;                          // [hmax][TP]
     float* actB = actA + (size_t)hmax * TP;      // [hmax][TP]
-    float* Ws = actB + (size_t)hmax * TP;        // [2][KC][OC]
-    double* red = reinterpret_cast<double*>(Ws + 2 * KC * OC);
+    float* Ws = actB + (size_t)hmax * TP;        // [2][KC][OCB]
+    double* red = reinterpret_cast<double*>(Ws + 2 * KC * OCB);
     const uint32_t ws_addr = (uint32_t)__cvta_generic_to_shared(Ws);
 
     const int tid = threadIdx.x;
     // a warp = 8 particle groups x 4 output groups.  Lane bits (4,3,0) pick the particle group and bits (2,1) the
     // output group: both LDS.128 of a k step then cost two shared-memory wavefronts (with output group = lane % 4
     // the weight load took four: ncu, L1 Wavefronts Shared per instruction)
-    constexpr int P = TP / 4, PW = P >= 8 ? 8 : P, OW = 32 / PW;     // particle / output groups per warp
+    constexpr int P = TP / (4 * R), PW = P >= 8 ? 8 : P, OW = 32 / PW;     // particle / output groups per warp
     const int lane = tid & 31;
     const int ol = PW == 8 ? ((lane >> 1) & 3) : lane % OW;
     const int pl = PW == 8 ? ((lane & 1) | ((lane >> 3) << 1)) : lane / OW;
@@ -94,27 +97,52 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
                     }
                 }
             } else
-            for (int o0 = 0; o0 < npad; o0 += OC) {
-                float tot[4][4], part[4][4];
+            for (int o0 = 0; o0 < npad; o0 += OCB) {
+                float tot[4 * R][4 * R], part[4 * R][4 * R];
 #pragma unroll
-                for (int a = 0; a < 4; ++a)
+                for (int a = 0; a < 4 * R; ++a)
 #pragma unroll
-                    for (int b = 0; b < 4; ++b) { tot[a][b] = 0.0f; part[a][b] = 0.0f; }
+                    for (int b = 0; b < 4 * R; ++b) { tot[a][b] = 0.0f; part[a][b] = 0.0f; }
                 // weight slab of K chunk c: global -> shared by cp.async into buffer c & 1 while chunk c - 1 is being
                 // multiplied; every thread moves PER 16-byte pieces (rows past K are not fetched and not read)
-                constexpr int PER = KC * (OC / 4) / NT;
-                static_assert(PER * NT == KC * (OC / 4), "slab pieces must divide over the threads");
-                const float* wsrc = Wt + (size_t)(tid >> 4) * npad + o0 + 4 * (tid & 15);
-                const size_t ustep = (size_t)(NT / 16) * npad;
+                constexpr int RP = OCB / 4;                              // 16-byte pieces per slab row
+                constexpr int PER = KC * RP / NT;
+                static_assert(PER * NT == KC * RP && NT % RP == 0, "slab pieces must divide over the threads");
+                const float* wsrc = Wt + (size_t)(tid / RP) * npad + o0 + 4 * (tid % RP);
+                const size_t ustep = (size_t)(NT / RP) * npad;
                 auto fetch = [&](int k0, int buf) {
                     const float* s0 = wsrc + (size_t)k0 * npad;
-                    const uint32_t d0 = ws_addr + (uint32_t)(buf * KC * OC * 4 + tid * 16);
+                    const uint32_t d0 = ws_addr + (uint32_t)(buf * KC * OCB * 4 + tid * 16);
 #pragma unroll
                     for (int u = 0; u < PER; ++u)
-                        if (k0 + (tid >> 4) + u * (NT / 16) < K)
+                        if (k0 + tid / RP + u * (NT / RP) < K)
                             asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d0 + u * NT * 16),
                                          "l"(s0 + u * ustep) : "memory");
                     asm volatile("cp.async.commit_group;" ::: "memory");
+                };
+                // one k step: R float4 of the activation row, R float4 of the weight row, (4R)^2 FFMA
+                auto lda = [&](const float* ap, int k, float4 (&av)[R]) {
+#pragma unroll
+                    for (int r = 0; r < R; ++r) av[r] = *reinterpret_cast<const float4*>(ap + k * TP + r * (TP / R));
+                };
+                auto ldw = [&](const float* wp, int k, float4 (&wv)[R]) {
+#pragma unroll
+                    for (int r = 0; r < R; ++r) wv[r] = *reinterpret_cast<const float4*>(wp + k * OCB + r * (OCB / R));
+                };
+                auto mac = [&](const float4 (&av)[R], const float4 (&wv)[R]) {
+#pragma unroll
+                    for (int ra = 0; ra < R; ++ra) {
+                        const float a4[4] = {av[ra].x, av[ra].y, av[ra].z, av[ra].w};
+#pragma unroll
+                        for (int rb = 0; rb < R; ++rb) {
+                            const float w4[4] = {wv[rb].x, wv[rb].y, wv[rb].z, wv[rb].w};
+#pragma unroll
+                            for (int a = 0; a < 4; ++a)
+#pragma unroll
+                                for (int b = 0; b < 4; ++b)
+                                    part[4 * ra + a][4 * rb + b] = fmaf(a4[a], w4[b], part[4 * ra + a][4 * rb + b]);
+                        }
+                    }
                 };
                 fetch(0, c & 1);          // c runs on over output blocks and layers: buffer c & 1 was last read in
                                           // chunk c - 2, which every warp has left (barrier of chunk c - 1)
@@ -124,58 +152,55 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
                     __syncthreads();          // slab c visible; slab c - 1 consumed by every warp; layer input complete
                     if (k0 + KC < K) fetch(k0 + KC, (c + 1) & 1);
                     const float* __restrict__ ap = in + (size_t)k0 * TP + 4 * pg;
-                    const float* __restrict__ wp = Ws + (c & 1) * (KC * OC) + 4 * og;
+                    const float* __restrict__ wp = Ws + (c & 1) * (KC * OCB) + 4 * og;
                     if (kk == KC) {
-                        // operands of step k + 1 are loaded before the 16 FFMA of step k (the shared-memory latency
+                        // operands of step k + 1 are loaded before the FFMAs of step k (the shared-memory latency
                         // was exposed with three warps per scheduler: profiles/r1_fp32.md)
-                        float4 av = *reinterpret_cast<const float4*>(ap), wv = *reinterpret_cast<const float4*>(wp);
+                        float4 av[R], wv[R];
+                        lda(ap, 0, av); ldw(wp, 0, wv);
 #pragma unroll
                         for (int k = 0; k < KC; ++k) {
-                            float4 an = av, wn = wv;
+                            float4 an[R], wn[R];
+                            if (k + 1 < KC) { lda(ap, k + 1, an); ldw(wp, k + 1, wn); }
+                            mac(av, wv);
                             if (k + 1 < KC) {
-                                an = *reinterpret_cast<const float4*>(ap + (k + 1) * TP);
-                                wn = *reinterpret_cast<const float4*>(wp + (k + 1) * OC);
+#pragma unroll
+                                for (int r = 0; r < R; ++r) { av[r] = an[r]; wv[r] = wn[r]; }
                             }
-                            const float a4[4] = {av.x, av.y, av.z, av.w};
-                            const float w4[4] = {wv.x, wv.y, wv.z, wv.w};
-#pragma unroll
-                            for (int a = 0; a < 4; ++a)
-#pragma unroll
-                                for (int b = 0; b < 4; ++b) part[a][b] = fmaf(a4[a], w4[b], part[a][b]);
-                            av = an; wv = wn;
                         }
                     } else {
                         for (int k = 0; k < kk; ++k) {
-                            const float4 av = *reinterpret_cast<const float4*>(ap + k * TP);
-                            const float4 wv = *reinterpret_cast<const float4*>(wp + k * OC);
-                            const float a4[4] = {av.x, av.y, av.z, av.w};
-                            const float w4[4] = {wv.x, wv.y, wv.z, wv.w};
-#pragma unroll
-                            for (int a = 0; a < 4; ++a)
-#pragma unroll
-                                for (int b = 0; b < 4; ++b) part[a][b] = fmaf(a4[a], w4[b], part[a][b]);
+                            float4 av[R], wv[R];
+                            lda(ap, k, av); ldw(wp, k, wv);
+                            mac(av, wv);
                         }
                     }
                     // partial sums of each 32-wide K span are formed separately and then added (shorter rounding chains)
                     if (((k0 / KC) & (32 / KC - 1)) == 32 / KC - 1 || k0 + KC >= K) {
 #pragma unroll
-                        for (int a = 0; a < 4; ++a)
+                        for (int a = 0; a < 4 * R; ++a)
 #pragma unroll
-                            for (int b = 0; b < 4; ++b) { tot[a][b] += part[a][b]; part[a][b] = 0.0f; }
+                            for (int b = 0; b < 4 * R; ++b) { tot[a][b] += part[a][b]; part[a][b] = 0.0f; }
                     }
                 }
-                const float4 bv = __ldg(reinterpret_cast<const float4*>(bias + o0) + og);
-                const float b4[4] = {bv.x, bv.y, bv.z, bv.w};
 #pragma unroll
-                for (int b = 0; b < 4; ++b) {
-                    float r[4];
+                for (int rb = 0; rb < R; ++rb) {
+                    const float4 bv = __ldg(reinterpret_cast<const float4*>(bias + o0 + rb * (OCB / R)) + og);
+                    const float b4[4] = {bv.x, bv.y, bv.z, bv.w};
 #pragma unroll
-                    for (int a = 0; a < 4; ++a) {
-                        const float z = tot[a][b] + b4[b];
-                        r[a] = last ? z : hb_activate<ACT, false>(z, slope);
+                    for (int b = 0; b < 4; ++b) {
+#pragma unroll
+                        for (int ra = 0; ra < R; ++ra) {
+                            float r[4];
+#pragma unroll
+                            for (int a = 0; a < 4; ++a) {
+                                const float z = tot[4 * ra + a][4 * rb + b] + b4[b];
+                                r[a] = last ? z : hb_activate<ACT, false>(z, slope);
+                            }
+                            *reinterpret_cast<float4*>(out + (size_t)(o0 + rb * (OCB / R) + 4 * og + b) * TP +
+                                                       ra * (TP / R) + 4 * pg) = make_float4(r[0], r[1], r[2], r[3]);
+                        }
                     }
-                    *reinterpret_cast<float4*>(out + (size_t)(o0 + 4 * og + b) * TP + 4 * pg) =
-                        make_float4(r[0], r[1], r[2], r[3]);
                 }
             }
             float* tmp = in; in = out; out = tmp;
@@ -200,17 +225,17 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
     }
 }
 
-template <int TP, bool MOM>
+template <int TP, bool MOM, int R, int OCB>
 static cudaError_t launch_tp(const HbParticles& p, size_t n, const HbSurDev& sd, int hmax, double* partials,
                              int grid, cudaStream_t s) {
-    constexpr int NT = (TP / 4) * 16;
-    const size_t smem = ((size_t)2 * hmax * TP + 2 * KC * OC) * sizeof(float) + (NT / 32) * HB_NMOM * sizeof(double);
+    constexpr int NT = (TP / (4 * R)) * (OCB / (4 * R));
+    const size_t smem = ((size_t)2 * hmax * TP + 2 * KC * OCB) * sizeof(float) + (NT / 32) * HB_NMOM * sizeof(double);
 #define HB_LAUNCH_ACT(A)                                                                                         \
     {                                                                                                            \
-        cudaError_t e = cudaFuncSetAttribute(hb_sur_fp32_kernel<TP, A, MOM>,                                     \
+        cudaError_t e = cudaFuncSetAttribute(hb_sur_fp32_kernel<TP, A, MOM, R, OCB>,                             \
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);            \
         if (e != cudaSuccess) return e;                                                                          \
-        hb_sur_fp32_kernel<TP, A, MOM><<<grid, NT, smem, s>>>(p, n, sd, hmax, partials);                         \
+        hb_sur_fp32_kernel<TP, A, MOM, R, OCB><<<grid, NT, smem, s>>>(p, n, sd, hmax, partials);                 \
     }
     switch (sd.act) {
     case 0: HB_LAUNCH_ACT(0) break;
@@ -226,9 +251,28 @@ cudaError_t hb_launch_sur_fp32(const HbParticles& p, size_t n, const HbSurDev& s
                                int* nblocks_out, int sm_count, cudaStream_t s) {
     int hmax = 64;
     for (int l = 0; l < sd.n_linear; ++l) hmax = hmax > sd.npad32[l] ? hmax : sd.npad32[l];
-    // tile size: two activation buffers of hmax x TP floats beside the weight slab; several blocks per SM when they
-    // fit (independent blocks hide each other's barriers and slab loads): hmax 256 -> TP 32, 72 KB, 3 blocks/SM
+    // 8 x 8 register tiles (R = 2): 64 particles and 256 threads per block, one block per SM; needs every layer that
+    // runs through the blocked loop padded to a multiple of 256 outputs and 2 x hmax x 64 floats + two slabs <= 227 KB
+    constexpr int WOCB = 256;
+    bool wide = hmax > 128 && hmax <= 384;
+    for (int l = 0; l < sd.n_linear; ++l) {
+        const bool narrow_last = (l == sd.n_linear - 1) && sd.widths[l + 1] <= 8;
+        if (!narrow_last && sd.npad32[l] % WOCB != 0) wide = false;
+    }
     const char* force = getenv("HB_FP32_TP");
+    if (force && atoi(force) != 0 && atoi(force) != 128) wide = false;      // testing: force the 4 x 4 shapes
+    const bool mom = partials != nullptr;
+    if (wide) {
+        const size_t ntiles = (n + 63) / 64;
+        size_t g = (size_t)sm_count;
+        if (g > ntiles) g = ntiles;
+        if (g < 1) g = 1;
+        if (nblocks_out) *nblocks_out = (int)g;
+        return mom ? launch_tp<64, true, 2, WOCB>(p, n, sd, hmax, partials, (int)g, s)
+                   : launch_tp<64, false, 2, WOCB>(p, n, sd, hmax, partials, (int)g, s);
+    }
+    // 4 x 4 tiles: two activation buffers of hmax x TP floats beside the weight slabs; several blocks per SM when they
+    // fit (independent blocks hide each other's barriers and slab loads): hmax 256 -> TP 32, 72 KB, 3 blocks/SM
     int tp = hmax <= 128 ? 64 : (hmax <= 768 ? 32 : 16);
     if (force) tp = atoi(force) == 64 && hmax <= 384 ? 64 : (atoi(force) == 16 ? 16 : (hmax <= 768 ? 32 : 16));
     const size_t smem_blk = ((size_t)2 * hmax * tp + 2 * KC * OC) * sizeof(float) + 1024;
@@ -241,8 +285,7 @@ cudaError_t hb_launch_sur_fp32(const HbParticles& p, size_t n, const HbSurDev& s
     if (g < 1) g = 1;
     const int grid = (int)g;
     if (nblocks_out) *nblocks_out = grid;
-    const bool mom = partials != nullptr;
-    if (tp == 64) return mom ? launch_tp<64, true>(p, n, sd, hmax, partials, grid, s) : launch_tp<64, false>(p, n, sd, hmax, partials, grid, s);
-    if (tp == 32) return mom ? launch_tp<32, true>(p, n, sd, hmax, partials, grid, s) : launch_tp<32, false>(p, n, sd, hmax, partials, grid, s);
-    return mom ? launch_tp<16, true>(p, n, sd, hmax, partials, grid, s) : launch_tp<16, false>(p, n, sd, hmax, partials, grid, s);
+    if (tp == 64) return mom ? launch_tp<64, true, 1, OC>(p, n, sd, hmax, partials, grid, s) : launch_tp<64, false, 1, OC>(p, n, sd, hmax, partials, grid, s);
+    if (tp == 32) return mom ? launch_tp<32, true, 1, OC>(p, n, sd, hmax, partials, grid, s) : launch_tp<32, false, 1, OC>(p, n, sd, hmax, partials, grid, s);
+    return mom ? launch_tp<16, true, 1, OC>(p, n, sd, hmax, partials, grid, s) : launch_tp<16, false, 1, OC>(p, n, sd, hmax, partials, grid, s);
 }
