@@ -483,11 +483,25 @@ def main():
         ach = per * n / (dom_ms * 1e-3) / 1e12
         widest = max(max(e["widths"][1:-1]) for e in desc["elements"] if e["kind"] == "surrogate")
         kname = "hb_sur_tcw_kernel" if widest > 512 else ("hb_sur_tcs_kernel" if widest > 256 else "hb_sur_tc_kernel")
-        roof = {"bound": "tensor", "achieved": ach, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
-                "frac": ach / pk["bf16_tflops"], "traffic": NCU_TRAFFIC.get((kname, n)), "kernel": kname,
-                "kernel_ms": dom_ms, "peak_source": pk["source"] + " (burst, cuBLAS bf16; f16 and bf16 share tcgen05.mma.kind::f16 and its peak)",
-                "frac_of_sustained": ach / pk["bf16_tflops_sustained"],
-                "algorithmic_flop_per_particle": per}
+        if args.prec == "fp32":
+            # FFMA path on the CUDA cores: peak derived in DESIGN.md 6.3 (148 SMs x 128 lanes x 1.965 GHz)
+            fma_peak = 148 * 128 * 1.965e9 / 1e12
+            ach = 0.5 * per * n / (dom_ms * 1e-3) / 1e12
+            roof = {"bound": "alu", "achieved": ach, "peak": fma_peak, "unit": "TFMA/s (fp32)", "frac": ach / fma_peak,
+                    "traffic": None, "kernel": "hb_sur_fp32_kernel", "kernel_ms": dom_ms,
+                    "peak_source": "derived: 148 SMs x 128 fp32 lanes x 1.965 GHz (DESIGN.md 6.3)",
+                    "algorithmic_fma_per_particle": 0.5 * per}
+        elif args.prec == "tf32":
+            roof = {"bound": "tensor", "achieved": ach, "peak": 0.5 * pk["bf16_tflops"], "unit": "TFLOP/s",
+                    "frac": ach / (0.5 * pk["bf16_tflops"]), "traffic": None, "kernel": "hb_sur_tcs_kernel",
+                    "kernel_ms": dom_ms, "peak_source": pk["source"] + " bf16 x 0.5 (nominal tf32 : bf16 ratio)",
+                    "algorithmic_flop_per_particle": per}
+        else:
+            roof = {"bound": "tensor", "achieved": ach, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
+                    "frac": ach / pk["bf16_tflops"], "traffic": NCU_TRAFFIC.get((kname, n)), "kernel": kname,
+                    "kernel_ms": dom_ms, "peak_source": pk["source"] + " (burst, cuBLAS bf16; f16 and bf16 share tcgen05.mma.kind::f16 and its peak)",
+                    "frac_of_sustained": ach / pk["bf16_tflops_sustained"],
+                    "algorithmic_flop_per_particle": per}
     else:
         ach = 48.0 * n / (dom_ms * 1e-3) / 1e9
         roof = {"bound": "hbm", "achieved": ach, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": ach / pk["hbm_gbs"],
