@@ -2,9 +2,9 @@
 //
 // One block owns a tile of TP particles.  Activations live in shared memory as [feature][particle]
 // (two ping-pong buffers); the transposed weights W^T [k][n] (packed, zero-padded to 64 outputs, by
-// hb_api.cu) are streamed through two [16][64] shared slabs filled by cp.async (slab c + 1 lands while
-// slab c is multiplied: one barrier per slab).  Each thread owns a 4-particle x 4-output register tile; the
-// operands of k step k + 1 are loaded before the 16 FFMA of step k.  The kernel is bound by the shared-memory
+// hb_api.cu) are streamed through two [KCH][OCB] shared slabs filled by cp.async (slab c + 1 lands while
+// slab c is multiplied: one barrier per slab).  Each thread owns a 4 x 4 or 8 x 8 (particles x outputs) register
+// tile; the operands of k step k + 1 are loaded before the FFMAs of step k.  The kernel is bound by the shared-memory
 // data path, so the lane -> (particle group, output group) map is the one for which ncu counts two wavefronts
 // per LDS.128 for both operands (profiles/r1_fp32.md).  Partial sums of each 32-wide K span are formed
 // separately and then added (shorter rounding chains), bias is added last in fp32, tanh is tanhf.
@@ -18,17 +18,17 @@
 #define OC 64
 
 // R = 1: 4 x 4 register tile, OCB = 64-wide output blocks; R = 2: 8 x 8 register tile (two float4 per operand and
-// k step: half the shared-memory wavefronts per FFMA), OCB = 256-wide output blocks, one 256-thread block of 64
-// particles per SM (two warps per scheduler at ~240 registers).
-template <int TP, int ACT, bool MOM, int R, int OCB>
-__global__ void __launch_bounds__((TP / (4 * R)) * (OCB / (4 * R)), (TP == 64 || R == 2) ? 1 : 3)
+// k step: half the shared-memory wavefronts per FFMA) with OCB = 256 (one 256-thread block of 64 particles per SM, two
+// warps per scheduler at ~240 registers) or OCB = 128 (two 128-thread blocks per SM).  KCH = rows per weight slab.
+template <int TP, int ACT, bool MOM, int R, int OCB, int KCH>
+__global__ void __launch_bounds__((TP / (4 * R)) * (OCB / (4 * R)), R == 2 ? (OCB == 128 ? 2 : 1) : (TP == 64 ? 1 : 3))
 hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, int hmax, double* __restrict__ partials) {
     constexpr int NT = (TP / (4 * R)) * (OCB / (4 * R));
     extern __shared__ __align__(16) float smem[];
     float* actA = smem;                          // [hmax][TP]
     float* actB = actA + (size_t)hmax * TP;      // [hmax][TP]
-    float* Ws = actB + (size_t)hmax * TP;        // [2][KC][OCB]
-    double* red = reinterpret_cast<double*>(Ws + 2 * KC * OCB);
+    float* Ws = actB + (size_t)hmax * TP;        // [2][KCH][OCB]
+    double* red = reinterpret_cast<double*>(Ws + 2 * KCH * OCB);
     const uint32_t ws_addr = (uint32_t)__cvta_generic_to_shared(Ws);
 
     const int tid = threadIdx.x;
@@ -106,13 +106,13 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
                 // weight slab of K chunk c: global -> shared by cp.async into buffer c & 1 while chunk c - 1 is being
                 // multiplied; every thread moves PER 16-byte pieces (rows past K are not fetched and not read)
                 constexpr int RP = OCB / 4;                              // 16-byte pieces per slab row
-                constexpr int PER = KC * RP / NT;
-                static_assert(PER * NT == KC * RP && NT % RP == 0, "slab pieces must divide over the threads");
+                constexpr int PER = KCH * RP / NT;
+                static_assert(PER * NT == KCH * RP && NT % RP == 0 && KCH % 16 == 0 && 32 % KCH == 0, "slab pieces must divide over the threads");
                 const float* wsrc = Wt + (size_t)(tid / RP) * npad + o0 + 4 * (tid % RP);
                 const size_t ustep = (size_t)(NT / RP) * npad;
                 auto fetch = [&](int k0, int buf) {
                     const float* s0 = wsrc + (size_t)k0 * npad;
-                    const uint32_t d0 = ws_addr + (uint32_t)(buf * KC * OCB * 4 + tid * 16);
+                    const uint32_t d0 = ws_addr + (uint32_t)(buf * KCH * OCB * 4 + tid * 16);
 #pragma unroll
                     for (int u = 0; u < PER; ++u)
                         if (k0 + tid / RP + u * (NT / RP) < K)
@@ -146,26 +146,31 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
                 };
                 fetch(0, c & 1);          // c runs on over output blocks and layers: buffer c & 1 was last read in
                                           // chunk c - 2, which every warp has left (barrier of chunk c - 1)
-                for (int k0 = 0; k0 < K; k0 += KC, ++c) {
-                    const int kk = min(KC, K - k0);
+                for (int k0 = 0; k0 < K; k0 += KCH, ++c) {
+                    const int kk = min(KCH, K - k0);
                     asm volatile("cp.async.wait_all;" ::: "memory");
                     __syncthreads();          // slab c visible; slab c - 1 consumed by every warp; layer input complete
-                    if (k0 + KC < K) fetch(k0 + KC, (c + 1) & 1);
+                    if (k0 + KCH < K) fetch(k0 + KCH, (c + 1) & 1);
                     const float* __restrict__ ap = in + (size_t)k0 * TP + 4 * pg;
-                    const float* __restrict__ wp = Ws + (c & 1) * (KC * OCB) + 4 * og;
-                    if (kk == KC) {
+                    const float* __restrict__ wp = Ws + (c & 1) * (KCH * OCB) + 4 * og;
+                    if (kk == KCH) {
                         // operands of step k + 1 are loaded before the FFMAs of step k (the shared-memory latency
-                        // was exposed with three warps per scheduler: profiles/r1_fp32.md)
-                        float4 av[R], wv[R];
-                        lda(ap, 0, av); ldw(wp, 0, wv);
+                        // was exposed with three warps per scheduler: profiles/r1_fp32.md); 16 steps per unrolled body
+#pragma unroll 1
+                        for (int h = 0; h < KCH / 16; ++h) {
+                            const float* aph = ap + h * 16 * TP;
+                            const float* wph = wp + h * 16 * OCB;
+                            float4 av[R], wv[R];
+                            lda(aph, 0, av); ldw(wph, 0, wv);
 #pragma unroll
-                        for (int k = 0; k < KC; ++k) {
-                            float4 an[R], wn[R];
-                            if (k + 1 < KC) { lda(ap, k + 1, an); ldw(wp, k + 1, wn); }
-                            mac(av, wv);
-                            if (k + 1 < KC) {
+                            for (int k = 0; k < 16; ++k) {
+                                float4 an[R], wn[R];
+                                if (k + 1 < 16) { lda(aph, k + 1, an); ldw(wph, k + 1, wn); }
+                                mac(av, wv);
+                                if (k + 1 < 16) {
 #pragma unroll
-                                for (int r = 0; r < R; ++r) { av[r] = an[r]; wv[r] = wn[r]; }
+                                    for (int r = 0; r < R; ++r) { av[r] = an[r]; wv[r] = wn[r]; }
+                                }
                             }
                         }
                     } else {
@@ -176,7 +181,7 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
                         }
                     }
                     // partial sums of each 32-wide K span are formed separately and then added (shorter rounding chains)
-                    if (((k0 / KC) & (32 / KC - 1)) == 32 / KC - 1 || k0 + KC >= K) {
+                    if (((k0 / KCH) & (32 / KCH - 1)) == 32 / KCH - 1 || k0 + KCH >= K) {
 #pragma unroll
                         for (int a = 0; a < 4 * R; ++a)
 #pragma unroll
@@ -225,17 +230,17 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
     }
 }
 
-template <int TP, bool MOM, int R, int OCB>
+template <int TP, bool MOM, int R, int OCB, int KCH>
 static cudaError_t launch_tp(const HbParticles& p, size_t n, const HbSurDev& sd, int hmax, double* partials,
                              int grid, cudaStream_t s) {
     constexpr int NT = (TP / (4 * R)) * (OCB / (4 * R));
-    const size_t smem = ((size_t)2 * hmax * TP + 2 * KC * OCB) * sizeof(float) + (NT / 32) * HB_NMOM * sizeof(double);
+    const size_t smem = ((size_t)2 * hmax * TP + 2 * KCH * OCB) * sizeof(float) + (NT / 32) * HB_NMOM * sizeof(double);
 #define HB_LAUNCH_ACT(A)                                                                                         \
     {                                                                                                            \
-        cudaError_t e = cudaFuncSetAttribute(hb_sur_fp32_kernel<TP, A, MOM, R, OCB>,                             \
+        cudaError_t e = cudaFuncSetAttribute(hb_sur_fp32_kernel<TP, A, MOM, R, OCB, KCH>,                        \
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);            \
         if (e != cudaSuccess) return e;                                                                          \
-        hb_sur_fp32_kernel<TP, A, MOM, R, OCB><<<grid, NT, smem, s>>>(p, n, sd, hmax, partials);                 \
+        hb_sur_fp32_kernel<TP, A, MOM, R, OCB, KCH><<<grid, NT, smem, s>>>(p, n, sd, hmax, partials);            \
     }
     switch (sd.act) {
     case 0: HB_LAUNCH_ACT(0) break;
@@ -251,25 +256,32 @@ cudaError_t hb_launch_sur_fp32(const HbParticles& p, size_t n, const HbSurDev& s
                                int* nblocks_out, int sm_count, cudaStream_t s) {
     int hmax = 64;
     for (int l = 0; l < sd.n_linear; ++l) hmax = hmax > sd.npad32[l] ? hmax : sd.npad32[l];
-    // 8 x 8 register tiles (R = 2): 64 particles and 256 threads per block, one block per SM; needs every layer that
-    // runs through the blocked loop padded to a multiple of 256 outputs and 2 x hmax x 64 floats + two slabs <= 227 KB
-    constexpr int WOCB = 256;
-    bool wide = hmax > 128 && hmax <= 384;
-    for (int l = 0; l < sd.n_linear; ++l) {
-        const bool narrow_last = (l == sd.n_linear - 1) && sd.widths[l + 1] <= 8;
-        if (!narrow_last && sd.npad32[l] % WOCB != 0) wide = false;
-    }
+    // 8 x 8 register tiles (R = 2), 64 particles per block.  128 < hmax <= 256: 256-wide output blocks, 256 threads,
+    // 32-row weight slabs, one block per SM (192 KB).  hmax = 128: 128-wide output blocks, 128 threads, two blocks per
+    // SM (80 KB each).  Every layer that runs through the blocked loop must be padded to a multiple of the block width.
     const char* force = getenv("HB_FP32_TP");
-    if (force && atoi(force) != 0 && atoi(force) != 128) wide = false;      // testing: force the 4 x 4 shapes
+    const bool classic = force && atoi(force) != 0 && atoi(force) != 128;   // testing: force the 4 x 4 shapes
+    auto blocked_multiple_of = [&](int m) {
+        for (int l = 0; l < sd.n_linear; ++l) {
+            const bool narrow_last = (l == sd.n_linear - 1) && sd.widths[l + 1] <= 8;
+            if (!narrow_last && sd.npad32[l] % m != 0) return false;
+        }
+        return true;
+    };
     const bool mom = partials != nullptr;
-    if (wide) {
+    const bool wide256 = !classic && hmax == 256 && blocked_multiple_of(256);
+    const bool wide128 = !classic && hmax == 128 && blocked_multiple_of(128);
+    if (wide256 || wide128) {
         const size_t ntiles = (n + 63) / 64;
-        size_t g = (size_t)sm_count;
+        size_t g = (size_t)sm_count * (wide128 ? 2 : 1);
         if (g > ntiles) g = ntiles;
         if (g < 1) g = 1;
         if (nblocks_out) *nblocks_out = (int)g;
-        return mom ? launch_tp<64, true, 2, WOCB>(p, n, sd, hmax, partials, (int)g, s)
-                   : launch_tp<64, false, 2, WOCB>(p, n, sd, hmax, partials, (int)g, s);
+        if (wide256)
+            return mom ? launch_tp<64, true, 2, 256, 32>(p, n, sd, hmax, partials, (int)g, s)
+                       : launch_tp<64, false, 2, 256, 32>(p, n, sd, hmax, partials, (int)g, s);
+        return mom ? launch_tp<64, true, 2, 128, 16>(p, n, sd, hmax, partials, (int)g, s)
+                   : launch_tp<64, false, 2, 128, 16>(p, n, sd, hmax, partials, (int)g, s);
     }
     // 4 x 4 tiles: two activation buffers of hmax x TP floats beside the weight slabs; several blocks per SM when they
     // fit (independent blocks hide each other's barriers and slab loads): hmax 256 -> TP 32, 72 KB, 3 blocks/SM
@@ -285,7 +297,7 @@ cudaError_t hb_launch_sur_fp32(const HbParticles& p, size_t n, const HbSurDev& s
     if (g < 1) g = 1;
     const int grid = (int)g;
     if (nblocks_out) *nblocks_out = grid;
-    if (tp == 64) return mom ? launch_tp<64, true, 1, OC>(p, n, sd, hmax, partials, grid, s) : launch_tp<64, false, 1, OC>(p, n, sd, hmax, partials, grid, s);
-    if (tp == 32) return mom ? launch_tp<32, true, 1, OC>(p, n, sd, hmax, partials, grid, s) : launch_tp<32, false, 1, OC>(p, n, sd, hmax, partials, grid, s);
-    return mom ? launch_tp<16, true, 1, OC>(p, n, sd, hmax, partials, grid, s) : launch_tp<16, false, 1, OC>(p, n, sd, hmax, partials, grid, s);
+    if (tp == 64) return mom ? launch_tp<64, true, 1, OC, KC>(p, n, sd, hmax, partials, grid, s) : launch_tp<64, false, 1, OC, KC>(p, n, sd, hmax, partials, grid, s);
+    if (tp == 32) return mom ? launch_tp<32, true, 1, OC, KC>(p, n, sd, hmax, partials, grid, s) : launch_tp<32, false, 1, OC, KC>(p, n, sd, hmax, partials, grid, s);
+    return mom ? launch_tp<16, true, 1, OC, KC>(p, n, sd, hmax, partials, grid, s) : launch_tp<16, false, 1, OC, KC>(p, n, sd, hmax, partials, grid, s);
 }

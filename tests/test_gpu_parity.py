@@ -170,7 +170,7 @@ def test_config1_fp32_per_segment(hb):
 
 @pytest.mark.parametrize("act", ["identity", "relu", "prelu", "tanh"])
 @pytest.mark.parametrize("widths", [[6, 6], [6, 7, 6], [6, 64, 64, 6], [6, 100, 37, 6], [6, 256, 256, 256, 6],
-                                    [6, 200, 256, 6], [6, 320, 192, 6]])
+                                    [6, 200, 256, 6], [6, 320, 192, 6], [6, 128, 128, 6]])
 def test_fp32_surrogate_shapes(hb, act, widths):
     n = 3001
     W, b = wl.make_mlp(widths, "he" if act in ("relu", "prelu") else "xavier", 77, len(widths))
