@@ -187,6 +187,29 @@ def test_fp32_surrogate_shapes(hb, act, widths):
     moments_close(rec[0], ref_rec[0], 1e-4)
 
 
+@pytest.mark.parametrize("widths", [[6, 256, 256, 6], [6, 128, 128, 128, 6]])
+def test_fp32_register_tile_shapes_agree(hb, widths, monkeypatch):
+    """The 8x8-register-tile shapes (256- / 128-wide output blocks) and the 4x4 shape (forced with HB_FP32_TP, read by
+    the library at launch) are two schedules of the same sums: both within the fp32 bound of the oracle, and the
+    hidden-layer summation order is the same, so they differ only through the output layer's K split."""
+    n = 64 * 37 + 5
+    W, b = wl.make_mlp(widths, "xavier", 91, len(widths))
+    rng = np.random.default_rng(8)
+    sur = wl.surrogate(widths, W, b, "tanh", rng.normal(size=6) * 1e-4, wl.NOMINAL_SIGMA, rng.normal(size=6),
+                       rng.uniform(0.5, 2.0, 6))
+    desc = wl.lattice([sur, wl.monitor()])
+    x = wl.gaussian_bunch(n, 32)
+    ref, ref_rec = oracle.push(desc, x)
+    got8, rec8 = gpu_push(hb, desc, x)
+    monkeypatch.setenv("HB_FP32_TP", "32")
+    got4, rec4 = gpu_push(hb, desc, x)
+    monkeypatch.delenv("HB_FP32_TP")
+    assert rel_err(got8, ref).max() <= 1e-5 and rel_err(got4, ref).max() <= 1e-5
+    assert rel_err(got8, got4.astype(np.float64)).max() <= 2e-6
+    moments_close(rec8[0], ref_rec[0], 1e-4)
+    moments_close(rec4[0], ref_rec[0], 1e-4)
+
+
 def test_fp32_identity_initialised_net(hb):
     H = 64
     A0 = np.zeros((H, 6), np.float32); A0[:6] = np.eye(6)
