@@ -55,9 +55,10 @@ def check_moments(rec_last, out):
     assert np.all(np.abs(rec_last[6:] - own[6:]) <= 1e-9 * scale)
 
 
-@pytest.mark.parametrize("prec", ["bf16", "f16"])
+@pytest.mark.parametrize("prec", ["bf16", "f16", "fp32"])
 def test_config3_full_size_sampled(hb, prec):
-    """C3, N = 1e7, the bench's headline launch: sampled particles vs the oracle, record vs the output."""
+    """C3, N = 1e7, the bench's headline launch (and BJ's second run of C3 on the FFMA path, in the 8x8-register-tile
+    shape the bench times): sampled particles vs the oracle, record vs the output."""
     desc, x = wl.config3(prec=prec)
     n = x.shape[1]
     assert n == 10_000_000
