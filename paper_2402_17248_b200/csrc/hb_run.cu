@@ -257,16 +257,22 @@ hb_moments_finalize_kernel(const double* __restrict__ partials, int nblocks, siz
                            const __grid_constant__ HbPivot pv, double* __restrict__ out) {
     __shared__ double S[HB_NMOM];
     const int j = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // launched with programmatic stream serialization: the block may become resident while the producing kernel is
+    // still draining; its partials are complete and visible once this returns
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     double v = 0.0;
-    for (int k0 = lane; k0 < nblocks; k0 += 32 * 8) {
-        double t[8];
+    // FIN_BATCH loads in flight per lane: one launch's partials (<= 592 blocks) are one batch; same summation order
+    // as a plain ascending loop over this lane's blocks
+    constexpr int FIN_BATCH = 20;
+    for (int k0 = lane; k0 < nblocks; k0 += 32 * FIN_BATCH) {
+        double t[FIN_BATCH];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
+        for (int u = 0; u < FIN_BATCH; ++u) {
             const int k = k0 + 32 * u;
             t[u] = k < nblocks ? __ldcg(partials + (size_t)j * HB_MOM_MAX_BLOCKS + k) : 0.0;
         }
 #pragma unroll
-        for (int u = 0; u < 8; ++u) v += t[u];
+        for (int u = 0; u < FIN_BATCH; ++u) v += t[u];
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -338,6 +344,16 @@ cudaError_t hb_launch_moments_finalize(const double* partials, int nblocks, size
                                        double* d_out27, cudaStream_t s) {
     HbPivot pv;
     for (int j = 0; j < 6; ++j) pv.p[j] = pivot6_host ? pivot6_host[j] : 0.0;
-    hb_moments_finalize_kernel<<<1, FIN_THREADS, 0, s>>>(partials, nblocks, n, pv, d_out27);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(1);
+    cfg.blockDim = dim3(FIN_THREADS);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, hb_moments_finalize_kernel, partials, nblocks, n, pv, d_out27);
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
