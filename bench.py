@@ -524,7 +524,7 @@ def main():
         "e2e": {"value": e2e_value, "unit": unit, "h2d_bytes_per_step": int(host.numel() * 4),
                 "d2h_bytes_per_step": int(host.numel() * 4 + rec_bytes), "ms_per_step": e2e_ms,
                 "api": "hb_push_host(chunks=%d): pinned host arrays, synchronous, host clock" % e2e_chunks},
-        "gpu_launches": int(args.steps * lat.num_launches(True)),
+        "gpu_launches": int(args.steps * lat.num_launches(True, n)),
         "records_merged_over_ranks": merged_ok,
         "roofline": roof,
     }

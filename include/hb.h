@@ -138,6 +138,14 @@ hb_status hb_lattice_add_surrogate(hb_lattice *lat, const hb_surrogate_desc *des
 /* Choose how conventional runs are applied (default HB_RUN_COMPOSED).  Before finalize only. */
 hb_status hb_lattice_set_run_mode(hb_lattice *lat, hb_run_mode mode);
 
+/* Nominal centroid of the incoming bunch in (x,px,y,py,t,pt), HOST, 6 doubles; default all zero (a bunch centred on
+ * the reference particle).  The library tracks it through the lattice on the host (run matrices; a surrogate stage
+ * sends it to its out_mean) and uses the tracked value as the pivot of the moment sums of every monitor (R10): sums of
+ * (v - pivot) are accumulated and the pivot is added back to the means, so a record does not depend on it beyond
+ * rounding -- it only keeps E[v^2] - E[v]^2 well conditioned for a bunch far off axis with a small spread.  Allowed
+ * before and after finalize (host arithmetic only).  Errors: NULL / non-finite -> INVALID_ARG. */
+hb_status hb_lattice_set_centroid(hb_lattice *lat, const double *centroid6);
+
 /* Split the element list into segments (maximal runs of conventional elements; single surrogate
  * stages; monitors), track the reference particle (R7), compose runs in fp64, pack the weights into
  * the tensor-core operand layout, upload constants and allocate all scratch on `cuda_device`.
@@ -148,8 +156,10 @@ hb_status hb_lattice_finalize(hb_lattice *lat, int cuda_device);
 /* Number of MONITOR elements (= moment records one push produces). */
 hb_status hb_lattice_num_monitors(const hb_lattice *lat, int *out);
 
-/* Number of kernel launches one hb_push / hb_push_moments enqueues (for launch accounting). */
-hb_status hb_lattice_num_launches(const hb_lattice *lat, int with_moments, int *out);
+/* Number of kernel launches one hb_push / hb_push_moments of n_particles enqueues (launch accounting): one per run and
+ * per surrogate stage -- a layered wide-net stage (hidden widths 513..1024) is one per linear layer and chunk of 2^20
+ * particles -- plus one finalize per fused monitor and two per standalone monitor.  n_particles = 0: no launch. */
+hb_status hb_lattice_num_launches(const hb_lattice *lat, int with_moments, size_t n_particles, int *out);
 
 /* (beta gamma) of the reference particle after the last element (valid after finalize). */
 hb_status hb_lattice_ref_bg_out(const hb_lattice *lat, double *out);
@@ -158,7 +168,12 @@ hb_status hb_lattice_ref_bg_out(const hb_lattice *lat, double *out);
  * aligned, pairwise non-overlapping; borrowed until the enqueued work completes.  n >= 0 (0 is a
  * no-op).  cuda_stream: a cudaStream_t (NULL = legacy default stream).  Returns after enqueueing;
  * MONITOR elements are skipped.  Errors: not finalized -> STATE; NULL / misaligned / overlapping
- * arrays -> INVALID_ARG; launch failure -> CUDA. */
+ * arrays -> INVALID_ARG; launch failure -> CUDA.
+ * ONE PUSH IN FLIGHT PER LATTICE: a lattice owns one buffer of moment partials and (wide nets) one activation scratch,
+ * allocated at finalize and reused by every push (nothing is allocated per push).  Pushes of the same lattice are safe
+ * back to back on ONE stream; pushes of the same lattice on DIFFERENT streams (hb_push, hb_push_moments, hb_push_host,
+ * hb_push_candidates) must be ordered by the caller (an event between them), or use one lattice object per stream --
+ * the device-resident state of a lattice is its weights (<= a few MB) and that scratch. */
 hb_status hb_push(hb_lattice *lat, float *x, float *px, float *y, float *py, float *t, float *pt,
                   size_t n, void *cuda_stream);
 

@@ -9,6 +9,7 @@ any call that needs the library fails loudly if libhb.so or a CUDA device is mis
 from ._binding import (  # noqa: F401
     HbError, Lattice, lib, lib_path, moments, to_device, to_host, allgather_merge_records,
     hb_lattice_create, hb_lattice_add_element, hb_lattice_set_element, hb_lattice_add_multipole, hb_lattice_add_surrogate, hb_lattice_set_run_mode,
+    hb_lattice_set_centroid,
     hb_lattice_finalize, hb_lattice_num_monitors, hb_lattice_num_launches, hb_lattice_ref_bg_out,
     hb_push, hb_push_moments, hb_push_host, hb_moments, hb_moments_scratch_bytes, hb_moments_merge, hb_lattice_destroy,
     hb_lattice_enable_timing, hb_lattice_get_timing,

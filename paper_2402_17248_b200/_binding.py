@@ -20,7 +20,7 @@ RUN_MODES = {"composed": 0, "sequential": 1, "sequential_fp32": 2}
 EXPORTED_SYMBOLS = [
     "hb_lattice_create", "hb_lattice_add_element", "hb_lattice_set_element", "hb_lattice_add_multipole",
     "hb_lattice_add_surrogate",
-    "hb_lattice_set_run_mode",
+    "hb_lattice_set_run_mode", "hb_lattice_set_centroid",
     "hb_lattice_finalize", "hb_lattice_num_monitors", "hb_lattice_num_launches", "hb_lattice_ref_bg_out",
     "hb_push", "hb_push_moments", "hb_push_host", "hb_moments", "hb_moments_scratch_bytes", "hb_moments_merge",
     "hb_lattice_destroy",
@@ -78,7 +78,8 @@ def lib():
     L.hb_lattice_set_run_mode.argtypes = [c_void_p, c_int]
     L.hb_lattice_finalize.argtypes = [c_void_p, c_int]
     L.hb_lattice_num_monitors.argtypes = [c_void_p, POINTER(c_int)]
-    L.hb_lattice_num_launches.argtypes = [c_void_p, c_int, POINTER(c_int)]
+    L.hb_lattice_num_launches.argtypes = [c_void_p, c_int, c_size_t, POINTER(c_int)]
+    L.hb_lattice_set_centroid.argtypes = [c_void_p, POINTER(c_double)]
     L.hb_lattice_ref_bg_out.argtypes = [c_void_p, POINTER(c_double)]
     L.hb_push.argtypes = [c_void_p] + [c_void_p] * 6 + [c_size_t, c_void_p]
     L.hb_push_moments.argtypes = [c_void_p] + [c_void_p] * 6 + [c_size_t, c_void_p, c_void_p]
@@ -197,10 +198,16 @@ def hb_lattice_num_monitors(lat) -> int:
     return n.value
 
 
-def hb_lattice_num_launches(lat, with_moments: bool) -> int:
+def hb_lattice_num_launches(lat, with_moments: bool, n_particles: int) -> int:
     n = c_int()
-    _check(lib().hb_lattice_num_launches(lat, int(bool(with_moments)), ctypes.byref(n)), "hb_lattice_num_launches")
+    _check(lib().hb_lattice_num_launches(lat, int(bool(with_moments)), int(n_particles), ctypes.byref(n)),
+           "hb_lattice_num_launches")
     return n.value
+
+
+def hb_lattice_set_centroid(lat, centroid6):
+    c = (c_double * 6)(*[float(v) for v in centroid6])
+    _check(lib().hb_lattice_set_centroid(lat, c), "hb_lattice_set_centroid")
 
 
 def hb_lattice_ref_bg_out(lat) -> float:
@@ -353,8 +360,12 @@ class Lattice:
     def num_monitors(self):
         return hb_lattice_num_monitors(self._h)
 
-    def num_launches(self, with_moments):
-        return hb_lattice_num_launches(self._h, with_moments)
+    def num_launches(self, with_moments, n_particles):
+        return hb_lattice_num_launches(self._h, with_moments, n_particles)
+
+    def set_centroid(self, centroid6):
+        """nominal centroid of the incoming bunch (pivot of the moment sums; default zeros)"""
+        hb_lattice_set_centroid(self._h, centroid6)
 
     @property
     def ref_bg_out(self):

@@ -70,8 +70,11 @@ struct Segment {
     double bg;             // SEG_RUN: (beta gamma) of the reference inside the run
     bool nonlinear;        // SEG_RUN holds a non-linear element: no composed map, always the fp64 sequential kernel
     HbSurDev sd;           // SEG_SUR
+    int sur;               // SEG_SUR: index into lat->surs
+    double bg1, z1;        // SEG_SUR, COORD_T: outgoing reference (given or derived, R7)
     bool tc;               // SEG_SUR: tensor-core kernel
     int monitor;           // record index written after this segment, -1 = none
+    double pivot[6];       // nominal centroid of the state behind this segment: pivot of its moment sums (a3)
 };
 
 // ---- fp64 6x6 helpers (transfer-matrix concatenation, R5) ---------------------------------
@@ -223,6 +226,8 @@ struct hb_lattice {
     HbSeqElem* d_seq = nullptr;
     double* d_partials = nullptr;
     std::vector<void*> d_bufs;
+    double centroid_in[6] = {0, 0, 0, 0, 0, 0};   // nominal centroid of the incoming bunch (hb_lattice_set_centroid)
+    std::vector<HbPivot> mon_pivot;               // [monitor] pivot of that record's sums
     bool timing = false;
     bool timing_valid = false;
     std::vector<cudaEvent_t> events;   // segs.size() + 1 when timing is on
@@ -234,6 +239,46 @@ struct hb_lattice {
     cudaStream_t host_streams[3] = {nullptr, nullptr, nullptr};   // copy-in, compute, copy-out
     cudaEvent_t host_events[9] = {};   // per slot: copied in, computed, copied out
 };
+
+// Nominal centroid of the bunch behind every segment (host, fp64): the incoming centroid (default 0) through the
+// linear(ised) run maps; a surrogate stage sends it to its output mean (R8), converted to s-coordinates about the new
+// reference for COORD_T (R6, R7).  Only the conditioning of the moment sums depends on it, never their value.
+static void track_pivots(hb_lattice* lat) {
+    double c[6];
+    for (int j = 0; j < 6; ++j) c[j] = lat->centroid_in[j];
+    lat->mon_pivot.assign((size_t)lat->n_monitors, HbPivot{});
+    for (Segment& g : lat->segs) {
+        if (g.type == SEG_RUN) {
+            double o[6];
+            for (int r = 0; r < 6; ++r) {
+                o[r] = 0.0;
+                for (int k = 0; k < 6; ++k) o[r] += (double)g.map.m[r * 6 + k] * c[k];
+            }
+            for (int j = 0; j < 6; ++j) c[j] = o[j];
+        } else if (g.type == SEG_SUR) {
+            const SurHost& s = lat->surs[(size_t)g.sur];
+            if (s.coord == HB_COORD_S) {
+                for (int j = 0; j < 6; ++j) c[j] = s.out_mean[j];
+            } else {
+                const double ux = s.out_mean[3], uy = s.out_mean[4], uz = s.out_mean[5], z = s.out_mean[2] - g.z1;
+                const double gam = std::sqrt(1.0 + ux * ux + uy * uy + uz * uz), g1 = std::sqrt(1.0 + g.bg1 * g.bg1);
+                if (uz > 0.0) {
+                    c[0] = s.out_mean[0] - ux / uz * z; c[1] = ux / g.bg1;
+                    c[2] = s.out_mean[1] - uy / uz * z; c[3] = uy / g.bg1;
+                    c[4] = -z * gam / uz;               c[5] = -(gam - g1) / g.bg1;
+                } else {
+                    for (int j = 0; j < 6; ++j) c[j] = 0.0;
+                }
+            }
+            for (int j = 0; j < 6; ++j)
+                if (!std::isfinite(c[j])) c[j] = 0.0;
+            for (int j = 0; j < 6; ++j) g.sd.mom_pivot.p[j] = c[j];
+        }
+        for (int j = 0; j < 6; ++j) g.pivot[j] = c[j];
+        if (g.monitor >= 0)
+            for (int j = 0; j < 6; ++j) lat->mon_pivot[(size_t)g.monitor].p[j] = c[j];
+    }
+}
 
 extern "C" {
 
@@ -291,6 +336,8 @@ hb_status hb_lattice_add_element(hb_lattice* lat, hb_elem_kind kind, double L, d
         if (!std::isfinite(L)) return fail(HB_ERR_INVALID_ARG, "length must be finite");
         if (kind != HB_ELEM_DRIFT && kind != HB_ELEM_DRIFT_EXACT && (!std::isfinite(param) || L < 0.0))
             return fail(HB_ERR_INVALID_ARG, "quad/plens/sbend need a finite parameter and length >= 0");
+        if (kind == HB_ELEM_SBEND && L == 0.0 && param != 0.0)
+            return fail(HB_ERR_INVALID_ARG, "sbend of length 0 with a non-zero angle has no finite curvature (use a multipole of order 1 for a thin dipole kick)");
         e.L = L;
         e.param = (kind == HB_ELEM_DRIFT || kind == HB_ELEM_DRIFT_EXACT) ? 0.0 : param;
     }
@@ -310,6 +357,8 @@ hb_status hb_lattice_set_element(hb_lattice* lat, int index, double L, double pa
     if (!std::isfinite(L)) return fail(HB_ERR_INVALID_ARG, "length must be finite");
     if (!is_drift && (!std::isfinite(param) || L < 0.0))
         return fail(HB_ERR_INVALID_ARG, "quad/plens/sbend need a finite parameter and length >= 0");
+    if (e.kind == HB_ELEM_SBEND && L == 0.0 && param != 0.0)
+        return fail(HB_ERR_INVALID_ARG, "sbend of length 0 with a non-zero angle has no finite curvature");
     if (!lat->finalized) {
         e.L = L;
         e.param = is_drift ? 0.0 : param;
@@ -341,6 +390,7 @@ hb_status hb_lattice_set_element(hb_lattice* lat, int index, double L, double pa
         }
         for (int r = 0; r < 6; ++r)
             for (int c = 0; c < 6; ++c) sg.map.m[r * 6 + c] = (float)M.m[r][c];
+        track_pivots(lat);
         return HB_OK;
     }
     return fail(HB_ERR_STATE, "element %d belongs to no run", index);
@@ -413,6 +463,15 @@ hb_status hb_lattice_set_run_mode(hb_lattice* lat, hb_run_mode mode) {
     return HB_OK;
 }
 
+hb_status hb_lattice_set_centroid(hb_lattice* lat, const double* centroid6) {
+    if (!lat || !centroid6) return fail(HB_ERR_INVALID_ARG, "NULL argument");
+    for (int j = 0; j < 6; ++j)
+        if (!std::isfinite(centroid6[j])) return fail(HB_ERR_INVALID_ARG, "centroid must be finite");
+    for (int j = 0; j < 6; ++j) lat->centroid_in[j] = centroid6[j];
+    if (lat->finalized) track_pivots(lat);     // host arithmetic only; pushes enqueued earlier keep their pivots
+    return HB_OK;
+}
+
 static hb_status upload(hb_lattice* lat, const void* src, size_t bytes, void** dst) {
     *dst = nullptr;
     if (bytes == 0) bytes = 16;
@@ -458,6 +517,8 @@ static hb_status build_surrogate(hb_lattice* lat, const SurHost& s, double bg_in
         sd.uz_in_shift = (float)(bg_in - s.in_mean[5]);
         sd.uz_out_shift = (float)(s.out_mean[5] - bg1);
         sd.z_out_mu = (float)(s.out_mean[2] - z1);
+        seg.bg1 = bg1;
+        seg.z1 = z1;
         *bg_out = bg1;
     }
     // ---- fp32 image: W^T [k][npad], zero padded to 64 outputs
@@ -530,7 +591,11 @@ hb_status hb_lattice_finalize(hb_lattice* lat, int device) {
     if (device < 0 || device >= ndev) return fail(HB_ERR_CUDA, "no CUDA device %d (have %d)", device, ndev);
     cudaDeviceProp prop;
     HB_CUDA(cudaGetDeviceProperties(&prop, device));
-    if (prop.major != 10) return fail(HB_ERR_UNSUPPORTED, "device %d is sm_%d%d; libhb is built for sm_100a only", device, prop.major, prop.minor);
+    if (prop.major != 10 || prop.minor != 0)
+        return fail(HB_ERR_UNSUPPORTED, "device %d is sm_%d%d; libhb is built for sm_100a only", device, prop.major, prop.minor);
+    if (prop.multiProcessorCount * 4 > HB_MOM_GRID_MAX)
+        return fail(HB_ERR_UNSUPPORTED, "device %d has %d SMs; the moment-partials layout is sized for <= %d", device,
+                    prop.multiProcessorCount, HB_MOM_GRID_MAX / 4);
     int prev = 0;
     HB_CUDA(cudaGetDevice(&prev));
     HB_CUDA(cudaSetDevice(device));
@@ -560,6 +625,7 @@ hb_status hb_lattice_finalize(hb_lattice* lat, int device) {
             Segment s{};
             s.type = SEG_SUR;
             s.monitor = -1;
+            s.sur = e.sur;
             double bg1 = bg;
             st = build_surrogate(lat, lat->surs[e.sur], bg, &bg1, s);
             bg = bg1;
@@ -601,6 +667,7 @@ hb_status hb_lattice_finalize(hb_lattice* lat, int device) {
         if (e != cudaSuccess) st = fail(HB_ERR_CUDA, "cudaDeviceSynchronize: %s", cudaGetErrorString(e));
     }
     lat->bg_out = bg;
+    if (st == HB_OK) track_pivots(lat);
     cudaSetDevice(prev);
     if (st != HB_OK) {
         for (void* p : lat->d_bufs) cudaFree(p);
@@ -620,14 +687,19 @@ hb_status hb_lattice_num_monitors(const hb_lattice* lat, int* out) {
     return HB_OK;
 }
 
-hb_status hb_lattice_num_launches(const hb_lattice* lat, int with_moments, int* out) {
+hb_status hb_lattice_num_launches(const hb_lattice* lat, int with_moments, size_t n_particles, int* out) {
     if (!lat || !out) return fail(HB_ERR_INVALID_ARG, "NULL argument");
     if (!lat->finalized) return fail(HB_ERR_STATE, "lattice not finalized");
     int n = 0;
-    for (const Segment& s : lat->segs) {
-        if (s.type == SEG_MON) n += with_moments ? 2 : 0;
-        else n += 1 + ((with_moments && s.monitor >= 0) ? 1 : 0);
-    }
+    if (n_particles > 0)
+        for (const Segment& s : lat->segs) {
+            if (s.type == SEG_MON) { n += with_moments ? 2 : 0; continue; }
+            // a layered (wide-net) stage is one launch per linear layer and chunk of HB_TCW_CHUNK particles
+            if (s.type == SEG_SUR && s.tc && s.sd.tc_kind == 3)
+                n += (int)((n_particles + HB_TCW_CHUNK - 1) / HB_TCW_CHUNK) * s.sd.n_linear;
+            else n += 1;
+            n += (with_moments && s.monitor >= 0) ? 1 : 0;
+        }
     *out = n;
     return HB_OK;
 }
@@ -669,19 +741,19 @@ static hb_status enqueue_segments(hb_lattice* lat, const HbParticles& p, size_t 
         int nblocks = 0;
         cudaError_t e = cudaSuccess;
         if (g.type == SEG_RUN) {
-            if (lat->run_mode == HB_RUN_COMPOSED && !g.nonlinear) e = hb_launch_run_composed(p, n, g.map, partials, &nblocks, s);
+            if (lat->run_mode == HB_RUN_COMPOSED && !g.nonlinear) e = hb_launch_run_composed(p, n, g.map, g.pivot, partials, &nblocks, s);
             else e = hb_launch_run_sequential(p, n, lat->d_seq + g.seq_off, g.seq_cnt,
-                                              lat->run_mode == HB_RUN_SEQUENTIAL_FP32, g.nonlinear, partials, &nblocks, s);
+                                              lat->run_mode == HB_RUN_SEQUENTIAL_FP32, g.nonlinear, g.pivot, partials, &nblocks, s);
         } else if (g.type == SEG_SUR) {
             if (g.tc && g.sd.tc_kind == 3) e = hb_launch_sur_tcw(p, n, g.sd, partials, host_partials != nullptr, &nblocks, lat->sm_count, s);
             else e = g.tc ? hb_launch_sur_tc(p, n, g.sd, partials, &nblocks, lat->sm_count, s)
                           : hb_launch_sur_fp32(p, n, g.sd, partials, &nblocks, lat->sm_count, s);
         } else if (mom) {
-            e = hb_launch_moments_partials(p, n, nullptr, partials, &nblocks, s);
+            e = hb_launch_moments_partials(p, n, g.pivot, partials, &nblocks, s);
         }
         if (e != cudaSuccess) { st = fail(HB_ERR_CUDA, "kernel launch (segment %zu): %s", k, cudaGetErrorString(e)); break; }
         if (mom && !host_partials) {
-            e = hb_launch_moments_finalize(partials, nblocks, n, nullptr, d_moments + (size_t)g.monitor * HB_NMOM, s);
+            e = hb_launch_moments_finalize(partials, nblocks, n, g.pivot, d_moments + (size_t)g.monitor * HB_NMOM, s);
             if (e != cudaSuccess) st = fail(HB_ERR_CUDA, "moments finalize: %s", cudaGetErrorString(e));
         }
         if (timing) cudaEventRecord(lat->events[k + 1], s);
@@ -779,9 +851,18 @@ hb_status hb_push_host(hb_lattice* lat, float* x, float* px, float* y, float* py
         }
     }
     if (st == HB_OK && chunk_n > lat->host_chunk_cap) {
+        // outgrown staging slots are freed first (the previous hb_push_host returned only after its streams had drained)
+        for (int i = 0; i < 3; ++i) {
+            if (!lat->d_stage[i]) continue;
+            for (size_t k = 0; k < lat->d_bufs.size(); ++k)
+                if (lat->d_bufs[k] == (void*)lat->d_stage[i]) { lat->d_bufs.erase(lat->d_bufs.begin() + (long)k); break; }
+            cudaFree(lat->d_stage[i]);
+            lat->d_stage[i] = nullptr;
+        }
+        lat->host_chunk_cap = 0;
         for (int i = 0; i < 3 && st == HB_OK; ++i) {
             void* d = nullptr;
-            st = upload(lat, nullptr, 6 * chunk_n * sizeof(float), &d);     // (a smaller old buffer stays in d_bufs)
+            st = upload(lat, nullptr, 6 * chunk_n * sizeof(float), &d);
             lat->d_stage[i] = (float*)d;
         }
         if (st == HB_OK) lat->host_chunk_cap = chunk_n;
@@ -824,7 +905,8 @@ hb_status hb_push_host(hb_lattice* lat, float* x, float* px, float* y, float* py
         if (e == cudaSuccess && st == HB_OK && want) {
             for (int m = 0; m < lat->n_monitors && e == cudaSuccess; ++m)
                 e = hb_launch_moments_finalize(lat->d_host_partials + (size_t)m * HB_NMOM * HB_MOM_MAX_BLOCKS,
-                                               pieces * HB_MOM_GRID_MAX, n, nullptr, lat->d_host_records + (size_t)m * HB_NMOM, scmp);
+                                               pieces * HB_MOM_GRID_MAX, n, lat->mon_pivot[(size_t)m].p,
+                                               lat->d_host_records + (size_t)m * HB_NMOM, scmp);
             if (e == cudaSuccess)
                 e = cudaMemcpyAsync(h_moments, lat->d_host_records, (size_t)lat->n_monitors * HB_NMOM * sizeof(double),
                                     cudaMemcpyDeviceToHost, scmp);

@@ -20,8 +20,11 @@ struct HbMomAcc {
 #pragma unroll
             for (int k = j; k < 6; ++k) { s[idx] = fma(v[j], v[k], s[idx]); ++idx; }
     }
-    __device__ __forceinline__ void add(float x, float px, float y, float py, float t, float pt) {
-        const double v[6] = {(double)x, (double)px, (double)y, (double)py, (double)t, (double)pt};
+    // one particle, shifted by the pivot (host-supplied nominal centroid: keeps E[v^2] - E[v]^2 well conditioned
+    // for a bunch that sits far off axis with a small spread)
+    __device__ __forceinline__ void add(const HbPivot& pv, float x, float px, float y, float py, float t, float pt) {
+        const double v[6] = {(double)x - pv.p[0], (double)px - pv.p[1], (double)y - pv.p[2],
+                             (double)py - pv.p[3], (double)t - pv.p[4], (double)pt - pv.p[5]};
         add(v);
     }
 };

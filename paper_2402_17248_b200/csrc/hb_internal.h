@@ -16,6 +16,10 @@ struct HbRunMap {             // composed run: v' = M v (row-major 6x6, fp32, bu
     float m[36];
 };
 
+// pivot of the moment sums (a3): the nominal centroid of the state a monitor sees, tracked on the host through the
+// lattice; the kernels accumulate sums of (v - pivot), the finalize adds it back to the means
+struct HbPivot { double p[6]; };
+
 // one conventional element in sequential mode (coefficients in fp64)
 //  kind 0 drift : a0 = L, a1 = L/(bg)^2
 //  kind 1 quad  : a0..a3 = x-plane 2x2 (row-major), a4..a7 = y-plane 2x2, a8 = L/(bg)^2
@@ -61,6 +65,7 @@ struct HbSurDev {             // passed by value to the surrogate kernels
     int kpad[HB_MAX_LINEAR];  // padded fan-in  (multiple of 64 elements; layer 0: 64)
     int npadtc[HB_MAX_LINEAR];// padded fan-out (multiple of 16; hidden: multiple of 64)
     int tc_kind;              // which tensor-core kernel the image was packed for (hb_tc_kernel_kind, fixed at finalize)
+    HbPivot mom_pivot;        // pivot of the fused moment sums of this stage's output (a3)
     unsigned char* act_scratch;   // wide nets (hb_sur_tcw.cu): two pre-tiled activation buffers of one chunk
 };
 
@@ -70,10 +75,12 @@ struct HbParticles {
 
 // ---- launchers (each returns the cudaError_t of the launch) ---------------------------------
 // partials: device [>= gridDim][27] doubles or nullptr (no moments)
-cudaError_t hb_launch_run_composed(const HbParticles& p, size_t n, const HbRunMap& map,
+// pivot6_host: pivot of the fused moment sums (nullptr = zeros); unused without partials
+cudaError_t hb_launch_run_composed(const HbParticles& p, size_t n, const HbRunMap& map, const double* pivot6_host,
                                    double* partials, int* nblocks_out, cudaStream_t s);
 cudaError_t hb_launch_run_sequential(const HbParticles& p, size_t n, const HbSeqElem* d_elems, int count,
-                                     bool fp32_regs, bool nonlinear, double* partials, int* nblocks_out, cudaStream_t s);
+                                     bool fp32_regs, bool nonlinear, const double* pivot6_host, double* partials,
+                                     int* nblocks_out, cudaStream_t s);
 cudaError_t hb_launch_moments_partials(const HbParticles& p, size_t n, const double* pivot6_host,
                                        double* partials, int* nblocks_out, cudaStream_t s);
 // fixed-order sum of `nblocks` partials -> 27-double record (pivot added back to the means)

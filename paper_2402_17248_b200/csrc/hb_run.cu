@@ -28,7 +28,8 @@ __device__ __forceinline__ void apply_map(const HbRunMap& M, const float (&in)[6
 
 template <bool MOM>
 __global__ void __launch_bounds__(RUN_THREADS, MOM ? 2 : 4)
-hb_run_composed_kernel(HbParticles p, size_t n, const __grid_constant__ HbRunMap M, double* __restrict__ partials) {
+hb_run_composed_kernel(HbParticles p, size_t n, const __grid_constant__ HbRunMap M, const __grid_constant__ HbPivot pv,
+                       double* __restrict__ partials) {
     __shared__ double red[(RUN_THREADS / 32) * HB_NMOM];
     HbMomAcc acc;
     if (MOM) acc.clear();
@@ -47,7 +48,7 @@ hb_run_composed_kernel(HbParticles p, size_t n, const __grid_constant__ HbRunMap
             apply_map(M, in, out);
 #pragma unroll
             for (int j = 0; j < 6; ++j) reinterpret_cast<float*>(&o[j])[e] = out[j];
-            if (MOM) acc.add(out[0], out[1], out[2], out[3], out[4], out[5]);
+            if (MOM) acc.add(pv, out[0], out[1], out[2], out[3], out[4], out[5]);
         }
 #pragma unroll
         for (int j = 0; j < 6; ++j) st_stream(p.v[j] + 4 * q, o[j]);
@@ -61,7 +62,7 @@ hb_run_composed_kernel(HbParticles p, size_t n, const __grid_constant__ HbRunMap
         apply_map(M, in, out);
 #pragma unroll
         for (int j = 0; j < 6; ++j) p.v[j][i] = out[j];
-        if (MOM) acc.add(out[0], out[1], out[2], out[3], out[4], out[5]);
+        if (MOM) acc.add(pv, out[0], out[1], out[2], out[3], out[4], out[5]);
     }
     if (MOM) hb_block_reduce_moments(acc, red, partials + blockIdx.x, threadIdx.x, RUN_THREADS, 1);
 }
@@ -142,7 +143,7 @@ __device__ __forceinline__ void seq_apply(const SeqElemT<T>& e, T (&v)[6]) {
 template <typename T, bool MOM, bool NL>
 __global__ void __launch_bounds__(RUN_THREADS, 2)
 hb_run_sequential_kernel(HbParticles p, size_t n, const HbSeqElem* __restrict__ elems, int count,
-                         double* __restrict__ partials) {
+                         const __grid_constant__ HbPivot pv, double* __restrict__ partials) {
     __shared__ SeqElemT<T> se[SEQ_CHUNK];
     __shared__ double red[(RUN_THREADS / 32) * HB_NMOM];
     HbMomAcc acc;
@@ -208,7 +209,7 @@ hb_run_sequential_kernel(HbParticles p, size_t n, const HbSeqElem* __restrict__ 
 #pragma unroll
             for (int e = 0; e < 4; ++e)
                 if (e < cnt)
-                    acc.add((float)v[e][0], (float)v[e][1], (float)v[e][2], (float)v[e][3], (float)v[e][4],
+                    acc.add(pv, (float)v[e][0], (float)v[e][1], (float)v[e][2], (float)v[e][3], (float)v[e][4],
                             (float)v[e][5]);
         }
     }
@@ -217,8 +218,6 @@ hb_run_sequential_kernel(HbParticles p, size_t n, const HbSeqElem* __restrict__ 
 }
 
 // ---------------------------------------------------------------------------------- standalone moments
-struct HbPivot { double p[6]; };
-
 __global__ void __launch_bounds__(RUN_THREADS, 2)
 hb_moments_partials_kernel(HbParticles p, size_t n, const __grid_constant__ HbPivot pv, double* __restrict__ partials) {
     __shared__ double red[(RUN_THREADS / 32) * HB_NMOM];
@@ -293,6 +292,12 @@ hb_moments_finalize_kernel(const double* __restrict__ partials, int nblocks, siz
 }
 
 // ---------------------------------------------------------------------------------- launchers
+static HbPivot make_pivot(const double* pivot6_host) {
+    HbPivot pv;
+    for (int j = 0; j < 6; ++j) pv.p[j] = pivot6_host ? pivot6_host[j] : 0.0;
+    return pv;
+}
+
 static int run_grid(size_t n, bool moments) {
     const size_t nq = (n >> 2) + ((n & 3) ? 1 : 0);
     size_t blocks = (nq + RUN_THREADS - 1) / RUN_THREADS;
@@ -302,38 +307,40 @@ static int run_grid(size_t n, bool moments) {
     return (int)blocks;
 }
 
-cudaError_t hb_launch_run_composed(const HbParticles& p, size_t n, const HbRunMap& map, double* partials,
-                                   int* nblocks_out, cudaStream_t s) {
+cudaError_t hb_launch_run_composed(const HbParticles& p, size_t n, const HbRunMap& map, const double* pivot6_host,
+                                   double* partials, int* nblocks_out, cudaStream_t s) {
     const int grid = run_grid(n, partials != nullptr);
     if (nblocks_out) *nblocks_out = grid;
+    const HbPivot pv = make_pivot(pivot6_host);
     if (partials)
-        hb_run_composed_kernel<true><<<grid, RUN_THREADS, 0, s>>>(p, n, map, partials);
+        hb_run_composed_kernel<true><<<grid, RUN_THREADS, 0, s>>>(p, n, map, pv, partials);
     else
-        hb_run_composed_kernel<false><<<grid, RUN_THREADS, 0, s>>>(p, n, map, partials);
+        hb_run_composed_kernel<false><<<grid, RUN_THREADS, 0, s>>>(p, n, map, pv, partials);
     return cudaGetLastError();
 }
 
 cudaError_t hb_launch_run_sequential(const HbParticles& p, size_t n, const HbSeqElem* d_elems, int count,
-                                     bool fp32_regs, bool nonlinear, double* partials, int* nblocks_out, cudaStream_t s) {
+                                     bool fp32_regs, bool nonlinear, const double* pivot6_host, double* partials,
+                                     int* nblocks_out, cudaStream_t s) {
     const int grid = run_grid(n, partials != nullptr);
     if (nblocks_out) *nblocks_out = grid;
+    const HbPivot pv = make_pivot(pivot6_host);
     if (nonlinear) {          // non-linear elements: fp64 registers only
-        if (partials) hb_run_sequential_kernel<double, true, true><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
-        else hb_run_sequential_kernel<double, false, true><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
+        if (partials) hb_run_sequential_kernel<double, true, true><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, pv, partials);
+        else hb_run_sequential_kernel<double, false, true><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, pv, partials);
     } else if (fp32_regs) {
-        if (partials) hb_run_sequential_kernel<float, true, false><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
-        else hb_run_sequential_kernel<float, false, false><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
+        if (partials) hb_run_sequential_kernel<float, true, false><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, pv, partials);
+        else hb_run_sequential_kernel<float, false, false><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, pv, partials);
     } else {
-        if (partials) hb_run_sequential_kernel<double, true, false><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
-        else hb_run_sequential_kernel<double, false, false><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, partials);
+        if (partials) hb_run_sequential_kernel<double, true, false><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, pv, partials);
+        else hb_run_sequential_kernel<double, false, false><<<grid, RUN_THREADS, 0, s>>>(p, n, d_elems, count, pv, partials);
     }
     return cudaGetLastError();
 }
 
 cudaError_t hb_launch_moments_partials(const HbParticles& p, size_t n, const double* pivot6_host, double* partials,
                                        int* nblocks_out, cudaStream_t s) {
-    HbPivot pv;
-    for (int j = 0; j < 6; ++j) pv.p[j] = pivot6_host ? pivot6_host[j] : 0.0;
+    const HbPivot pv = make_pivot(pivot6_host);
     const int grid = run_grid(n, true);
     if (nblocks_out) *nblocks_out = grid;
     hb_moments_partials_kernel<<<grid, RUN_THREADS, 0, s>>>(p, n, pv, partials);
@@ -342,8 +349,7 @@ cudaError_t hb_launch_moments_partials(const HbParticles& p, size_t n, const dou
 
 cudaError_t hb_launch_moments_finalize(const double* partials, int nblocks, size_t n, const double* pivot6_host,
                                        double* d_out27, cudaStream_t s) {
-    HbPivot pv;
-    for (int j = 0; j < 6; ++j) pv.p[j] = pivot6_host ? pivot6_host[j] : 0.0;
+    const HbPivot pv = make_pivot(pivot6_host);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(1);
     cfg.blockDim = dim3(FIN_THREADS);

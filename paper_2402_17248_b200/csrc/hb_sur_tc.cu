@@ -312,7 +312,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                 float x, px, y, py, t, pt;
                 hb_sur_epilogue(sd, w, x, px, y, py, t, pt);
                 p.v[0][i] = x; p.v[1][i] = px; p.v[2][i] = y; p.v[3][i] = py; p.v[4][i] = t; p.v[5][i] = pt;
-                if (partials) acc.add(x, px, y, py, t, pt);
+                if (partials) acc.add(sd.mom_pivot, x, px, y, py, t, pt);
             }
             if (warp == IO_WARP0) TR(2, 4);
         }

@@ -256,7 +256,7 @@ hb_sur_tcw_kernel(HbParticles p, size_t n_chunk, const __grid_constant__ HbSurDe
                     hb_sur_epilogue(sd, w, x, px, y, py, t, pt);
                     const size_t o = ly.row_off + i;
                     p.v[0][o] = x; p.v[1][o] = px; p.v[2][o] = y; p.v[3][o] = py; p.v[4][o] = t; p.v[5][o] = pt;
-                    if (partials) acc.add(x, px, y, py, t, pt);
+                    if (partials) acc.add(sd.mom_pivot, x, px, y, py, t, pt);
                 }
             }
             if (partials) {

@@ -14,7 +14,7 @@ import workloads as wl
 
 pytestmark = pytest.mark.gpu
 
-TOL = {"f16": 2e-2, "bf16": 1.5e-1, "fp32": 1e-5}
+TOL = {"f16": 2e-2, "bf16": 1.2e-1, "fp32": 1e-5}      # bf16: regression bound at the measured level (test_gpu_tc.py)
 
 
 @pytest.fixture(scope="module")
@@ -66,7 +66,7 @@ def test_config3_full_size_sampled(hb, prec):
     idx = sample_indices(n)
     ref, _ = oracle.push(desc, np.ascontiguousarray(x[:, idx]))
     assert np.all(np.isfinite(out))
-    std = out.astype(np.float64).std(axis=1)
+    std = ref.std(axis=1)                      # G14: std of the oracle's output coordinate (over the sample)
     err = np.max(np.abs(out[:, idx].astype(np.float64) - ref), axis=1) / std
     print("C3 full size", prec, "max err/std on", idx.size, "sampled particles:", err)
     assert err.max() <= TOL[prec]
@@ -79,7 +79,7 @@ def test_config2_full_size_sampled(hb):
     out, rec = gpu_push_full(hb, desc, x)
     idx = sample_indices(x.shape[1])
     ref, _ = oracle.push(desc, np.ascontiguousarray(x[:, idx]))
-    std = out.astype(np.float64).std(axis=1)
+    std = ref.std(axis=1)
     err = np.max(np.abs(out[:, idx].astype(np.float64) - ref), axis=1) / std
     print("C2 lattice N=1e7 max err/std:", err)
     assert err.max() <= 1e-6
@@ -93,10 +93,12 @@ def test_config4_full_size_sampled(hb):
     idx = sample_indices(x.shape[1])
     ref, _ = oracle.push(desc, np.ascontiguousarray(x[:, idx]))
     assert np.all(np.isfinite(out))
-    std = out.astype(np.float64).std(axis=1)
+    std = ref.std(axis=1)
     err = np.max(np.abs(out[:, idx].astype(np.float64) - ref), axis=1) / std
     print("C4 full size f16 free-running max err/std:", err)
-    assert err.max() <= 5e-2          # two 16-bit stages in a row (per-stage bound 2e-2: test_gpu_tc.py)
+    # two 16-bit stages in a row compound: reported, and held to the measured level (the per-stage contract, 2e-2 with
+    # every stage fed from the oracle, is test_config4_full_size_every_stage_oracle_fed below)
+    assert err.max() <= 5e-2
     assert rec.shape[0] == 4
     check_moments(rec[-1], out)
 
@@ -113,7 +115,7 @@ def test_config5_full_size_first_stage_and_run(hb):
     out, rec = gpu_push_full(hb, first, x)
     idx = sample_indices(n)
     ref, _ = oracle.push(first, np.ascontiguousarray(x[:, idx]))
-    std = out[:, ::97].astype(np.float64).std(axis=1)
+    std = ref.std(axis=1)
     err = np.max(np.abs(out[:, idx].astype(np.float64) - ref), axis=1) / std
     print("C5 N=1e8 stage 1 + run, f16, max err/std:", err)
     assert err.max() <= TOL["f16"]
@@ -144,7 +146,7 @@ def test_paper_shaped_nets_full_size_sampled(hb, name, width, hidden):
     idx = np.unique(np.concatenate([idx, np.arange((1 << 20) - 300, (1 << 20) + 300)]))     # a chunk boundary
     ref, _ = oracle.push(desc, np.ascontiguousarray(x[:, idx]))
     assert np.all(np.isfinite(out))
-    std = out[:, ::7].astype(np.float64).std(axis=1)
+    std = ref.std(axis=1)
     err = np.max(np.abs(out[:, idx].astype(np.float64) - ref), axis=1) / std
     print(name, "full size f16 max err/std on", idx.size, "sampled particles:", err)
     assert err.max() <= TOL["f16"]
@@ -155,3 +157,55 @@ def test_paper_shaped_nets_full_size_sampled(hb, name, width, hidden):
     lat.close()
     assert np.array_equal(host.numpy(), out)
     assert np.allclose(rec_h[-1][:6], rec[-1][:6], rtol=1e-12, atol=1e-18)
+
+
+# ------------------------------------------------------------------ every stage fed from the oracle, at full size
+def full_size_oracle_fed(hb, desc, x, idx):
+    """The whole bunch stays on the device and goes through the lattice piece by piece (tests/test_gpu_stagefed.py
+    stage_lattices: every surrogate stage on its own, with the reference energy it has in the lattice).  The oracle
+    carries the sampled particles `idx` in fp64; before every surrogate stage its state, rounded to fp32, is written
+    over those particles of the device bunch, so the stage is oracle-fed on the sample while it runs in the launch
+    configuration of the full size.  Returns per-stage max |gpu - oracle| / std(oracle output) over the sample."""
+    import torch
+    from test_gpu_stagefed import stage_lattices
+    c = hb.to_device(x)
+    tidx = torch.from_numpy(idx).cuda()
+    state = np.ascontiguousarray(x[:, idx].astype(np.float64))
+    errs = []
+    for sub, is_sur in stage_lattices(desc):
+        lat = hb.Lattice.from_description(sub, device=0)
+        if is_sur:
+            fed = state.astype(np.float32)
+            tf = torch.from_numpy(fed).cuda()
+            for j in range(6):
+                c[j].index_copy_(0, tidx, tf[j])
+            ref, _ = oracle.push(sub, fed)
+            lat.push(c)
+            got = torch.stack([c[j].index_select(0, tidx) for j in range(6)]).cpu().numpy().astype(np.float64)
+            assert np.all(np.isfinite(got))
+            errs.append(np.max(np.abs(got - ref), axis=1) / ref.std(axis=1))
+        else:
+            lat.push(c)
+        torch.cuda.synchronize()
+        lat.close()
+        state, _ = oracle.push(sub, state)
+    del c
+    torch.cuda.empty_cache()
+    return np.array(errs)
+
+
+def test_config4_full_size_every_stage_oracle_fed(hb):
+    """C4, N = 1e7, f16: both COORD_T stages at 2e-2 (stage 2: 8 GeV incoming reference)"""
+    desc, x = wl.config4(prec="f16")
+    e = full_size_oracle_fed(hb, desc, x, sample_indices(x.shape[1]))
+    print("C4 N=1e7 oracle-fed per-stage max err/std (f16):", e.max(axis=1))
+    assert e.shape[0] == 2 and e.max() <= TOL["f16"]
+
+
+def test_config5_full_size_every_stage_oracle_fed(hb):
+    """C5 as specified (N = 1e8, 9 stages 6-512^4-6 tanh + 8 transport sections), f16: every stage at 2e-2"""
+    desc, x = wl.config5(prec="f16")
+    assert x.shape[1] == 100_000_000
+    e = full_size_oracle_fed(hb, desc, x, sample_indices(x.shape[1], m=4000))
+    print("C5 N=1e8 oracle-fed per-stage max err/std (f16):", e.max(axis=1))
+    assert e.shape[0] == 9 and e.max() <= TOL["f16"]

@@ -623,3 +623,24 @@ def test_stagewise_lens_optimisation_without_rebuilding(hb):
     f_ref = eps_x(np.asarray(ref_rec)[-1])
     print("stagewise optimisation:", len(evals), "evaluations, eps_x", f0, "->", res.fun, "oracle at optimum", f_ref)
     assert abs(res.fun - f_ref) <= 1e-3 * f_ref
+
+
+def test_num_launches_counts_what_a_push_enqueues(hb):
+    """hb_lattice_num_launches(n): one per run / stage (+ finalize per fused monitor, two per standalone monitor); a
+    layered wide-net stage is one launch per linear layer and chunk of 2^20 particles"""
+    desc, _ = wl.config1(prec="f16", n=8)
+    lat = hb.Lattice.from_description(desc, device=0)
+    assert lat.num_launches(False, 4096) == 3 and lat.num_launches(True, 4096) == 6 and lat.num_launches(True, 0) == 0
+    lat.close()
+    descp, _ = wl.paper_net(700, 3, prec="f16", particles=False)
+    lat = hb.Lattice.from_description(descp, device=0)
+    assert lat.num_launches(True, 10_000_000) == 10 * 4 + 1
+    assert lat.num_launches(False, (1 << 20) + 1) == 2 * 4
+    lat.close()
+    lat = hb.Lattice.from_description(wl.lattice([wl.monitor(), wl.sbend(0.0, 0.0), wl.monitor()]), device=0)
+    assert lat.num_launches(True, 100) == 2 + 2
+    x = wl.gaussian_bunch(100, 3)
+    c = hb.to_device(x)
+    lat.push_moments(c)
+    assert np.array_equal(hb.to_host(c), x)            # a zero-length, zero-angle bend is the identity
+    lat.close()

@@ -1,0 +1,229 @@
+"""Per-stage parity with every stage fed from the oracle (-m gpu), the reference update of R7 derived by the library
+itself, and the pivot of the fused moment sums.
+
+SURVEY 8(c) A-bf16: "for multi-stage configs errors compound through later random nets: the per-stage contract is
+checked by feeding stage k of the GPU with the oracle's (fp32-rounded) stage k-1 state".  `stage_lattices` cuts a
+lattice description at its surrogate stages into sub-lattices, each with the reference energy the oracle's tracker has
+at that point (R7: C4's second stage sees an 8 GeV reference, not 1 GeV); `oracle_fed` walks them: the oracle carries
+its own fp64 state, every surrogate stage of the GPU gets that state rounded to fp32, and the stage's output is compared
+with the oracle's output of the very same fp32 input -- max |gpu - oracle| / std(oracle output coordinate) (G14).
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+# BASELINE.json north_star: fp32 surrogate 1e-5, 16-bit tensor-core path 2e-2 (x std of the oracle's output coordinate).
+# Plain bf16 operands (8 significand bits) are outside 2e-2 on these random nets; the value below is the
+# largest per-stage error on record for them (C3 at N = 1e7: 1.1e-1), kept as a regression bound, and
+# test_plain_bf16_does_not_meet_the_north_star_bound states the miss against 2e-2 itself.
+TOL = {"fp32": 1e-5, "f16": 2e-2, "tf32": 2e-2, "bf16x3": 2e-2}
+BF16_MEASURED = 1.2e-1
+
+
+@pytest.fixture(scope="module")
+def hb():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2402_17248_b200 as hb
+    hb.lib()
+    return hb
+
+
+def stage_lattices(desc):
+    """[(sub-lattice description, is_surrogate_stage)] in lattice order: every surrogate on its own, the elements
+    between two surrogates together; kinetic energy of each piece = the oracle tracker's reference at its entrance."""
+    tr = oracle.Tracker(desc)
+    rest = desc["rest_MeV"]
+    pieces, cur = [], []
+
+    def kin():
+        return (math.sqrt(1.0 + tr.bg * tr.bg) - 1.0) * rest
+
+    cur_kin = kin()
+    for el in desc["elements"]:
+        if el["kind"] == "surrogate":
+            if cur:
+                pieces.append((wl.lattice(cur, cur_kin, rest), False))
+                cur = []
+            pieces.append((wl.lattice([el], kin(), rest), True))
+            if el["coord"] == "t":
+                tr.bg, _ = oracle.surrogate_reference_out(el, tr.bg)
+            cur_kin = kin()
+        else:
+            cur.append(el)
+    if cur:
+        pieces.append((wl.lattice(cur, cur_kin, rest), False))
+    return pieces
+
+
+def oracle_fed(hb, desc, x, prec=None):
+    """per-stage max err/std, one row per surrogate stage; the oracle's chain is free running in fp64"""
+    state = np.ascontiguousarray(x.astype(np.float64))
+    errs = []
+    for sub, is_sur in stage_lattices(desc):
+        if not is_sur:
+            state, _ = oracle.push(sub, state)
+            continue
+        fed = state.astype(np.float32)                       # the oracle's stage k-1 state, rounded to fp32
+        ref, _ = oracle.push(sub, fed)
+        lat = hb.Lattice.from_description(sub, device=0, prec=prec)
+        c = hb.to_device(fed)
+        lat.push(c)
+        got = hb.to_host(c).astype(np.float64)
+        lat.close()
+        assert np.all(np.isfinite(got))
+        errs.append(np.max(np.abs(got - ref), axis=1) / ref.std(axis=1))
+        state, _ = oracle.push(sub, state)                   # the oracle continues from its own unrounded state
+    return np.array(errs)
+
+
+@pytest.mark.parametrize("prec", ["fp32", "f16", "bf16"])
+def test_config4_every_stage_oracle_fed(hb, prec):
+    """C4: both COORD_T stages; stage 2 has the 8 GeV incoming reference (other bg0, uz_in_shift than stage 1)"""
+    desc, x = wl.config4(prec=prec, n=50_000, stages=2)
+    e = oracle_fed(hb, desc, x)
+    print("C4 oracle-fed per-stage max err/std (%s):" % prec, e.max(axis=1))
+    assert e.shape[0] == 2
+    assert e.max() <= (BF16_MEASURED if prec == "bf16" else TOL[prec])
+
+
+@pytest.mark.parametrize("prec", ["f16", "bf16"])
+def test_config5_every_stage_oracle_fed(hb, prec):
+    """C5's nine 6-512^4-6 tanh stages (streamed-weights kernel) and the eight transport sections between them"""
+    desc, x = wl.config5(prec=prec, n=50_000)
+    e = oracle_fed(hb, desc, x)
+    print("C5 oracle-fed per-stage max err/std (%s):" % prec, e.max(axis=1))
+    assert e.shape[0] == 9
+    assert e.max() <= (BF16_MEASURED if prec == "bf16" else TOL[prec])
+
+
+@pytest.mark.xfail(strict=True, reason="plain bf16 operands: 8 significand bits give 4e-2..1.1e-1 x std on the random "
+                   "synthetic nets, outside BASELINE.json's 2e-2 (DESIGN.md 6.5); HB_PREC_F16 / HB_PREC_BF16X3 meet it")
+def test_plain_bf16_does_not_meet_the_north_star_bound(hb):
+    desc, x = wl.config3(prec="bf16", n=200_000)
+    ref, _ = oracle.push(desc, x)
+    lat = hb.Lattice.from_description(desc, device=0)
+    c = hb.to_device(x)
+    lat.push(c)
+    got = hb.to_host(c).astype(np.float64)
+    lat.close()
+    e = np.max(np.abs(got - ref), axis=1) / ref.std(axis=1)
+    print("C3 plain bf16 max err/std:", e)
+    assert e.max() <= 2e-2
+
+
+@pytest.mark.parametrize("prec", ["fp32", "f16"])
+def test_reference_update_derived_by_the_library(hb, prec):
+    """R7 with ref_bg_out = ref_z_out = NaN: the library evaluates the net on the reference input in fp64 on the host
+    at finalize (csrc/hb_api.cu mlp_host); the oracle does the same with its own code.  Two stages, so that the second
+    one's incoming reference is itself a derived one."""
+    desc, x = wl.config4(prec=prec, n=30_000, stages=2)
+    for el in desc["elements"]:
+        if el["kind"] == "surrogate":
+            el["ref_bg_out"] = float("nan")
+            el["ref_z_out"] = float("nan")
+    # the oracle's derived references
+    tr = oracle.Tracker(desc)
+    bgs = []
+    for el in desc["elements"]:
+        if el["kind"] == "surrogate":
+            tr.bg, z1 = oracle.surrogate_reference_out(el, tr.bg)
+            bgs.append((tr.bg, z1))
+    assert all(np.isfinite(b) and b > 0 and np.isfinite(z) for b, z in bgs)
+    # not the nominal +7 GeV values: the random net moves the reference somewhere else
+    nominal = wl.config4(prec=prec, n=8, stages=2)[0]["elements"][0]["ref_bg_out"]
+    assert abs(bgs[0][0] - nominal) > 1e-3
+    lat = hb.Lattice.from_description(desc, device=0)
+    assert abs(lat.ref_bg_out / bgs[-1][0] - 1.0) <= 1e-12
+    lat.close()
+    e = oracle_fed(hb, desc, x)
+    print("C4 derived reference, oracle-fed per-stage max err/std (%s):" % prec, e.max(axis=1))
+    assert e.max() <= TOL[prec]
+    # whole lattice with monitors: the downstream transport uses the derived (beta gamma), records agree
+    ref, ref_rec = oracle.push(desc, x)
+    lat = hb.Lattice.from_description(desc, device=0)
+    c = hb.to_device(x)
+    rec = lat.push_moments(c).cpu().numpy()
+    got = hb.to_host(c).astype(np.float64)
+    lat.close()
+    efree = np.max(np.abs(got - ref), axis=1) / ref.std(axis=1)
+    print("  free running, whole lattice:", efree)
+    assert efree.max() <= (1e-4 if prec == "fp32" else 5e-2)      # two stages compound (reported; per-stage above)
+    sd = np.sqrt(ref_rec[:, [6, 12, 17, 21, 24, 26]])
+    assert np.max(np.abs(rec[:, :6] - ref_rec[:, :6]) / sd) <= (1e-4 if prec == "fp32" else 2e-2)
+
+
+# ------------------------------------------------------------------ a3: pivot of the fused moment sums
+def _affine_stage(out_mean, out_std, prec="fp32"):
+    """COORD_S surrogate that maps the normalised input straight to the output: w = v^ * out_std + out_mean"""
+    A = np.eye(6, dtype=np.float32)
+    return wl.surrogate([6, 6], [A], [np.zeros(6, np.float32)], "identity", np.zeros(6), wl.NOMINAL_SIGMA,
+                        out_mean, out_std, prec=prec)
+
+
+@pytest.mark.parametrize("ratio", [1e4, 1e6])
+def test_fused_moments_of_a_bunch_far_off_axis(hb, ratio):
+    """|mean| / sigma = 1e4 and 1e6 behind a surrogate stage and the run that follows it: raw fp64 sums would lose
+    2 log10(ratio) digits in E[v^2] - E[v]^2 (1e-4 relative at 1e6); with the tracked pivot (out_mean through the run
+    matrix) the record equals the two-pass fp64 moments of the kernel's own fp32 output to ~1e-10"""
+    n = 200_003
+    out_std = np.full(6, 1e-3)
+    out_mean = out_std * ratio * np.array([1.0, -0.7, 0.5, 0.9, -1.0, 0.3])
+    desc = wl.lattice([_affine_stage(out_mean, out_std), wl.monitor(), wl.drift(0.5), wl.quad(0.1, 1.2), wl.monitor()])
+    x = wl.gaussian_bunch(n, 23)
+    states = []
+    lat = hb.Lattice.from_description(desc, device=0)
+    c = hb.to_device(x)
+    # state behind the stage: push the stage alone on a copy
+    lat1 = hb.Lattice.from_description(wl.lattice(desc["elements"][:2]), device=0)
+    c1 = hb.to_device(x)
+    rec1 = lat1.push_moments(c1).cpu().numpy()
+    states.append(hb.to_host(c1).astype(np.float64))
+    lat1.close()
+    rec = lat.push_moments(c).cpu().numpy()
+    states.append(hb.to_host(c).astype(np.float64))
+    lat.close()
+    assert np.array_equal(rec[0], rec1[0])
+    for k in range(2):
+        own = oracle.moments(np.ascontiguousarray(states[k]))      # two-pass fp64 (R10) of the GPU's own output
+        sd = np.sqrt(own[[6, 12, 17, 21, 24, 26]])
+        assert np.all(sd > 0)
+        assert np.max(np.abs(rec[k][:6] - own[:6]) / sd) <= 1e-9
+        scale = np.sqrt(np.outer(sd * sd, sd * sd))[np.triu_indices(6)]
+        err = np.max(np.abs(rec[k][6:] - own[6:]) / scale)
+        print("ratio %g record %d: max second-moment error / (sigma_j sigma_k) = %.3g" % (ratio, k, err))
+        assert err <= 1e-4 * 1e-3          # three orders inside the 1e-4 moment bound of the north star
+
+
+def test_set_centroid_is_the_pivot_of_an_off_axis_input(hb):
+    """an incoming bunch that sits far off axis: hb_lattice_set_centroid gives the pivot of the first monitors; the
+    records do not depend on it beyond rounding, and with it they hold the 1e-10 level"""
+    n = 100_001
+    x = wl.gaussian_bunch(n, 29)
+    shift = wl.NOMINAL_SIGMA * 3e5 * np.array([1, -1, 0.5, 0.25, -0.5, 1])
+    xs = (x.astype(np.float64) + shift[:, None]).astype(np.float32)
+    desc = wl.lattice([wl.monitor()] + wl.fodo_cell(1.2) + [wl.monitor()])
+    recs = []
+    for cen in (None, shift):
+        lat = hb.Lattice.from_description(desc, device=0)
+        if cen is not None:
+            lat.set_centroid(cen)
+        c = hb.to_device(xs)
+        recs.append(lat.push_moments(c).cpu().numpy())
+        out = hb.to_host(c).astype(np.float64)
+        lat.close()
+    own = [oracle.moments(np.ascontiguousarray(xs.astype(np.float64))), oracle.moments(np.ascontiguousarray(out))]
+    for k in range(2):
+        sd = np.sqrt(own[k][[6, 12, 17, 21, 24, 26]])
+        scale = np.sqrt(np.outer(sd * sd, sd * sd))[np.triu_indices(6)]
+        e_raw = np.max(np.abs(recs[0][k][6:] - own[k][6:]) / scale)
+        e_piv = np.max(np.abs(recs[1][k][6:] - own[k][6:]) / scale)
+        print("record %d: raw sums %.3g, pivoted %.3g" % (k, e_raw, e_piv))
+        assert e_piv <= 1e-9
+        assert np.max(np.abs(recs[1][k][:6] - own[k][:6]) / sd) <= 1e-9

@@ -1,8 +1,10 @@
 """Tensor-core surrogate (tcgen05) vs the fp64 oracle, through the C ABI (-m gpu).
 
-BASELINE.json asks <= 2e-2 x std(output coordinate) for the 16-bit path.  DESIGN.md ("16-bit accuracy")
-records what is measured: HB_PREC_F16 meets it; plain bf16 operands do not on the random synthetic nets
-(8 mantissa bits), so bf16 is held to the measured level and reported, not massaged.
+BASELINE.json asks <= 2e-2 x std(oracle's output coordinate) for the 16-bit path.  DESIGN.md 6.5 records what is
+measured: HB_PREC_F16 (and tf32) meet it; plain bf16 operands (8 significand bits) do not on the random synthetic nets.
+Plain bf16 is therefore NOT a conforming mode: its entries below are regression bounds at the largest error on record
+(1.1e-1, C3 at N = 1e7), and tests/test_gpu_stagefed.py::test_plain_bf16_does_not_meet_the_north_star_bound states the
+miss against 2e-2 itself (strict xfail).
 """
 import os
 
@@ -14,7 +16,7 @@ import workloads as wl
 
 pytestmark = pytest.mark.gpu
 
-TOL = {"f16": 2e-2, "bf16": 1.5e-1}
+TOL = {"f16": 2e-2, "bf16": 1.2e-1}
 
 
 @pytest.fixture(scope="module")
@@ -78,8 +80,9 @@ def test_tc_tiles_and_tails(hb, n, force_cg, monkeypatch):
     ref, ref_rec = oracle.push(desc, x)
     got, rec = gpu_push(hb, desc, x, moments=True)
     assert np.all(np.isfinite(got))
-    scale = wl.NOMINAL_SIGMA[:, None] * 0.3           # output std of this net is ~0.3 sigma_nominal or larger
-    assert np.max(np.abs(got - ref) / scale) <= 2e-2
+    # G14: std of the oracle's output coordinate -- over 5000 particles of the same generator (n itself may be 1)
+    big, _ = oracle.push(desc, wl.gaussian_bunch(5000, 17))
+    assert np.max(np.abs(got - ref) / big.std(axis=1)[:, None]) <= 2e-2
     own = oracle.moments(np.ascontiguousarray(got))
     assert np.allclose(rec[0][:6], own[:6], rtol=1e-9, atol=1e-16)
     if n > 1:
@@ -135,6 +138,7 @@ def test_config4_tensor_core_per_stage(hb, prec):
     e = rel_err(got, ref)
     print("C4 free-running 2 stages", prec, "err/std:", e)
     assert np.all(np.isfinite(got))
+    # (every stage fed from the oracle, incl. stage 2 with its 8 GeV reference: tests/test_gpu_stagefed.py)
 
 
 # ------------------------------------------------------------------ streamed-weights kernel (hb_sur_tcs.cu)
@@ -245,7 +249,9 @@ def test_tf32_shapes(hb, act, widths, n):
     desc = wl.lattice([sur, wl.monitor()])
     ref, _ = oracle.push(desc, x)
     got, rec = gpu_push(hb, desc, x, moments=True)
-    scale = np.maximum(ref.std(axis=1), np.abs(sur["out_std"]) * 0.2) if n > 1 else np.abs(sur["out_std"])
+    # G14: std of the oracle's output coordinate (over 5000 particles of the same generator when n is tiny)
+    big, _ = oracle.push(desc, wl.correlated_bunch(5000, 44))
+    scale = ref.std(axis=1) if n >= 1000 else big.std(axis=1)
     e = np.max(np.abs(got - ref), axis=1) / scale
     print("tf32 shape", widths, act, "max err/std", e.max())
     assert np.all(np.isfinite(got))
@@ -293,7 +299,8 @@ def test_tcw_shapes(hb, prec, act, widths, n):
     assert hb.hb_surrogate_kernel(prec, widths) == "tcgen05-layered"
     ref, _ = oracle.push(desc, x)
     got, rec = gpu_push(hb, desc, x, moments=True)
-    scale = ref.std(axis=1) if n > 1 else np.abs(sur["out_std"])
+    big, _ = oracle.push(desc, wl.correlated_bunch(2000, 45)) if n < 1000 else (ref, None)
+    scale = big.std(axis=1)                            # G14 (over 2000 particles of the same bunch when n is tiny)
     e = np.max(np.abs(got - ref), axis=1) / scale
     print("layered shape", widths, act, prec, "max err/std", e.max())
     assert np.all(np.isfinite(got))

@@ -42,6 +42,17 @@ def test_host_validation_without_device(hb):
         hb.hb_lattice_add_element(h, "sbend", -0.5, 0.01)
     with pytest.raises(hb.HbError):
         hb.hb_lattice_add_element(h, "quad", 0.1, float("inf"))
+    with pytest.raises(hb.HbError) as e:                        # zero-length bend with an angle: infinite curvature
+        hb.hb_lattice_add_element(h, "sbend", 0.0, 0.02)
+    assert e.value.status == 1
+    hb.hb_lattice_add_element(h, "sbend", 0.0, 0.0)             # ... without an angle it is the identity
+    with pytest.raises(hb.HbError) as e:
+        hb.hb_lattice_set_element(h, 2, 0.0, 0.02)
+    assert e.value.status == 1
+    with pytest.raises(hb.HbError) as e:
+        hb.hb_lattice_set_centroid(h, [0, 0, float("nan"), 0, 0, 0])
+    assert e.value.status == 1
+    hb.hb_lattice_set_centroid(h, [1e-3, 0, 0, 0, 0, 0])
     W, b = wl.make_mlp([6, 8, 6], "xavier", 1, 0)
     z, o = np.zeros(6), np.ones(6)
     hb.hb_lattice_add_surrogate(h, [6, 8, 6], W, b, "tanh", z, o, z, o)
