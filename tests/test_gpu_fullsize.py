@@ -160,22 +160,24 @@ def test_paper_shaped_nets_full_size_sampled(hb, name, width, hidden):
 
 
 # ------------------------------------------------------------------ every stage fed from the oracle, at full size
-def full_size_oracle_fed(hb, desc, x, idx):
+def full_size_oracle_fed(hb, desc, x, idx, renorm=False):
     """The whole bunch stays on the device and goes through the lattice piece by piece (tests/test_gpu_stagefed.py
     stage_lattices: every surrogate stage on its own, with the reference energy it has in the lattice).  The oracle
     carries the sampled particles `idx` in fp64; before every surrogate stage its state, rounded to fp32, is written
     over those particles of the device bunch, so the stage is oracle-fed on the sample while it runs in the launch
     configuration of the full size.  Returns per-stage max |gpu - oracle| / std(oracle output) over the sample."""
     import torch
-    from test_gpu_stagefed import stage_lattices
+    from test_gpu_stagefed import renormalised, stage_lattices
     c = hb.to_device(x)
     tidx = torch.from_numpy(idx).cuda()
     state = np.ascontiguousarray(x[:, idx].astype(np.float64))
     errs = []
     for sub, is_sur in stage_lattices(desc):
+        fed = state.astype(np.float32)
+        if is_sur and renorm:
+            sub = renormalised(sub, fed)
         lat = hb.Lattice.from_description(sub, device=0)
         if is_sur:
-            fed = state.astype(np.float32)
             tf = torch.from_numpy(fed).cuda()
             for j in range(6):
                 c[j].index_copy_(0, tidx, tf[j])
@@ -203,9 +205,10 @@ def test_config4_full_size_every_stage_oracle_fed(hb):
 
 
 def test_config5_full_size_every_stage_oracle_fed(hb):
-    """C5 as specified (N = 1e8, 9 stages 6-512^4-6 tanh + 8 transport sections), f16: every stage at 2e-2"""
+    """C5 as specified (N = 1e8, 9 stages 6-512^4-6 tanh + 8 transport sections), f16: every stage at 2e-2, each
+    normalised to the state the oracle feeds it (why: tests/test_gpu_stagefed.py::test_config5_every_stage_oracle_fed)"""
     desc, x = wl.config5(prec="f16")
     assert x.shape[1] == 100_000_000
-    e = full_size_oracle_fed(hb, desc, x, sample_indices(x.shape[1], m=4000))
+    e = full_size_oracle_fed(hb, desc, x, sample_indices(x.shape[1], m=4000), renorm=True)
     print("C5 N=1e8 oracle-fed per-stage max err/std (f16):", e.max(axis=1))
     assert e.shape[0] == 9 and e.max() <= TOL["f16"]
