@@ -306,7 +306,7 @@ const char* hb_surrogate_kernel(hb_prec prec, int n_linear, const int* widths) {
     char why[256];
     if (!hb_tc_supported((int)prec, n_linear, widths, why, sizeof why)) { fail(HB_ERR_UNSUPPORTED, "tensor-core surrogate: %s", why); return nullptr; }
     const int kind = hb_tc_kernel_kind((int)prec, n_linear, widths);
-    return kind == 3 ? "tcgen05-layered" : (kind == 2 ? "tcgen05-streamed" : "tcgen05-resident");
+    return kind == 3 ? "tcgen05-layered" : (kind == 2 ? "tcgen05-streamed" : "tcgen05-resident");   // kinds 1 and 4 keep their weights in shared memory
 }
 
 hb_status hb_lattice_create(double kin, double rest, hb_lattice** out) {
@@ -544,6 +544,7 @@ static hb_status build_surrogate(hb_lattice* lat, const SurHost& s, double bg_in
         if (st != HB_OK) return st;
         sd.w32 = (const float*)dw;
         sd.b32 = (const float*)db;
+        sd.fp32_tp = hb_fp32_env_tp();
         seg.tc = false;
     } else {
         char why[256];
@@ -553,10 +554,13 @@ static hb_status build_surrogate(hb_lattice* lat, const SurHost& s, double bg_in
         for (int l = 0; l < s.n_linear; ++l) Wp.push_back(s.W[l].data());
         std::vector<const float*> Bp;
         for (int l = 0; l < s.n_linear; ++l) Bp.push_back(s.b[l].data());
-        const size_t bytes = hb_tc_pack_weights(s.prec, s.n_linear, s.widths.data(), Wp.data(), nullptr, nullptr,
+        // kernel and launch shape are chosen here, once (test hooks of the environment included), and kept in the segment
+        const HbTcChoice ch = hb_tc_choose(s.prec, s.n_linear, s.widths.data());
+        sd.tc_kind = ch.kind; sd.tc_cg = ch.cg; sd.tc_g = ch.g; sd.tc_occ = ch.occ;
+        const size_t bytes = hb_tc_pack_weights(ch, s.prec, s.n_linear, s.widths.data(), Wp.data(), nullptr, nullptr,
                                                 sd.wtc_off, sd.kpad, sd.npadtc);
         std::vector<unsigned char> img(bytes);
-        hb_tc_pack_weights(s.prec, s.n_linear, s.widths.data(), Wp.data(), Bp.data(), img.data(), sd.wtc_off, sd.kpad,
+        hb_tc_pack_weights(ch, s.prec, s.n_linear, s.widths.data(), Wp.data(), Bp.data(), img.data(), sd.wtc_off, sd.kpad,
                            sd.npadtc);
         std::vector<float> b;
         for (int l = 0; l < s.n_linear; ++l) {
@@ -571,7 +575,6 @@ static hb_status build_surrogate(hb_lattice* lat, const SurHost& s, double bg_in
         if (st != HB_OK) return st;
         sd.wtc = dw;
         sd.btc = (const float*)db;
-        sd.tc_kind = hb_tc_kernel_kind(s.prec, s.n_linear, s.widths.data());   // the image above is this kernel's
         if (sd.tc_kind == 3) {      // wide net: activations of a chunk round-trip through global scratch
             void* da = nullptr;
             st = upload(lat, nullptr, hb_tcw_scratch_bytes(s.n_linear, s.widths.data()), &da);
@@ -579,6 +582,18 @@ static hb_status build_surrogate(hb_lattice* lat, const SurHost& s, double bg_in
             sd.act_scratch = (unsigned char*)da;
         }
         seg.tc = true;
+    }
+    // launch attributes of the kernel instantiations this stage uses (with and without fused moments): set once here
+    {
+        HbParticles none{};
+        for (int mom = 0; mom < 2; ++mom) {
+            double* fake = mom ? reinterpret_cast<double*>(sizeof(double)) : nullptr;    // only tested against nullptr
+            cudaError_t e;
+            if (seg.tc && sd.tc_kind == 3) e = hb_launch_sur_tcw(none, 1, sd, fake, false, nullptr, lat->sm_count, true, nullptr);
+            else if (seg.tc) e = hb_launch_sur_tc(none, 1, sd, fake, nullptr, lat->sm_count, true, nullptr);
+            else e = hb_launch_sur_fp32(none, 1, sd, fake, nullptr, lat->sm_count, true, nullptr);
+            if (e != cudaSuccess) return fail(HB_ERR_CUDA, "surrogate kernel attributes: %s", cudaGetErrorString(e));
+        }
     }
     return HB_OK;
 }
@@ -745,9 +760,9 @@ static hb_status enqueue_segments(hb_lattice* lat, const HbParticles& p, size_t 
             else e = hb_launch_run_sequential(p, n, lat->d_seq + g.seq_off, g.seq_cnt,
                                               lat->run_mode == HB_RUN_SEQUENTIAL_FP32, g.nonlinear, g.pivot, partials, &nblocks, s);
         } else if (g.type == SEG_SUR) {
-            if (g.tc && g.sd.tc_kind == 3) e = hb_launch_sur_tcw(p, n, g.sd, partials, host_partials != nullptr, &nblocks, lat->sm_count, s);
-            else e = g.tc ? hb_launch_sur_tc(p, n, g.sd, partials, &nblocks, lat->sm_count, s)
-                          : hb_launch_sur_fp32(p, n, g.sd, partials, &nblocks, lat->sm_count, s);
+            if (g.tc && g.sd.tc_kind == 3) e = hb_launch_sur_tcw(p, n, g.sd, partials, host_partials != nullptr, &nblocks, lat->sm_count, false, s);
+            else e = g.tc ? hb_launch_sur_tc(p, n, g.sd, partials, &nblocks, lat->sm_count, false, s)
+                          : hb_launch_sur_fp32(p, n, g.sd, partials, &nblocks, lat->sm_count, false, s);
         } else if (mom) {
             e = hb_launch_moments_partials(p, n, g.pivot, partials, &nblocks, s);
         }

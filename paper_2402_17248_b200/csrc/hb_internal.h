@@ -64,7 +64,9 @@ struct HbSurDev {             // passed by value to the surrogate kernels
     int btc_off[HB_MAX_LINEAR];
     int kpad[HB_MAX_LINEAR];  // padded fan-in  (multiple of 64 elements; layer 0: 64)
     int npadtc[HB_MAX_LINEAR];// padded fan-out (multiple of 16; hidden: multiple of 64)
-    int tc_kind;              // which tensor-core kernel the image was packed for (hb_tc_kernel_kind, fixed at finalize)
+    int tc_kind;              // which tensor-core kernel the image was packed for (hb_tc_choose, fixed at finalize)
+    int tc_cg, tc_g, tc_occ;  // resident kernels: cluster size, epilogue warp groups, CTAs per SM (fixed at finalize)
+    int fp32_tp;              // fp32 kernel: forced particles-per-block of the 4x4 shape, 0 = automatic (fixed at finalize)
     HbPivot mom_pivot;        // pivot of the fused moment sums of this stage's output (a3)
     unsigned char* act_scratch;   // wide nets (hb_sur_tcw.cu): two pre-tiled activation buffers of one chunk
 };
@@ -86,30 +88,37 @@ cudaError_t hb_launch_moments_partials(const HbParticles& p, size_t n, const dou
 // fixed-order sum of `nblocks` partials -> 27-double record (pivot added back to the means)
 cudaError_t hb_launch_moments_finalize(const double* partials, int nblocks, size_t n,
                                        const double* pivot6_host, double* d_out27, cudaStream_t s);
+// Surrogate launchers.  prepare = true (hb_lattice_finalize, once per stage): only set the launch attributes of the
+// kernel instantiation the stage will use (dynamic shared memory), launch nothing.
 cudaError_t hb_launch_sur_fp32(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials,
-                               int* nblocks_out, int sm_count, cudaStream_t s);
+                               int* nblocks_out, int sm_count, bool prepare, cudaStream_t s);
 cudaError_t hb_launch_sur_tc(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials,
-                             int* nblocks_out, int sm_count, cudaStream_t s);
+                             int* nblocks_out, int sm_count, bool prepare, cudaStream_t s);
+int hb_fp32_env_tp(void);     // HB_FP32_TP test hook (read at finalize)
+// kernel and launch shape of a tensor-core stage (hb_sur_tc.cu; reads the test hooks of the environment): kind 0 = no
+// schedule, 1 resident / one tile per CTA, 2 streamed, 3 layered, 4 resident / two tiles in flight
+struct HbTcChoice { int kind, cg, g, occ; };
+HbTcChoice hb_tc_choose(int prec, int n_linear, const int* widths);
 // host-side packing for the tensor-core path (hb_sur_tc.cu owns the layout)
 //  returns bytes needed; if dst != nullptr writes the image.  W row-major [out][in] fp32.
 //  B: biases [out] fp32 per layer (the resident kernel's image carries those of the hidden layers; may be nullptr
 //  when dst is).
-size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float* const* W, const float* const* B,
-                          void* dst, long long* off_bytes, int* kpad, int* npad);
+size_t hb_tc_pack_weights(const HbTcChoice& ch, int prec, int n_linear, const int* widths, const float* const* W,
+                          const float* const* B, void* dst, long long* off_bytes, int* kpad, int* npad);
 bool hb_tc_supported(int prec, int n_linear, const int* widths, char* why, size_t why_len);
 // streamed-weights variant (hb_sur_tcs.cu): hidden width <= 512, equal hidden widths, weights through an smem ring
 bool hb_tcs_supported(int prec, int n_linear, const int* widths);   // prec: hb_prec (1 bf16, 2 f16, 3 tf32)
 size_t hb_tcs_pack_weights(int prec, int n_linear, const int* widths, const float* const* W,
                            void* dst, long long* off_bytes, int* kpad, int* npad);
 cudaError_t hb_launch_sur_tcs(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials,
-                              int* nblocks_out, int sm_count, cudaStream_t s);
-// two-tiles-in-flight variant of the resident kernel (hb_sur_tc2.cu): same weight image as hb_tc_pack_weights
-bool hb_tc2_supported(int n_linear, const int* widths);
+                              int* nblocks_out, int sm_count, bool prepare, cudaStream_t s);
+// resident weights, two tiles in flight per CTA, hidden layers as N-halves (hb_sur_tc2.cu): hidden width 129..256
+int hb_tc2_plan_cg(int n_linear, const int* widths, int force_cg);     // 0: no plan, else the cluster size
+size_t hb_tc2_pack_weights(int prec, int cg, int n_linear, const int* widths, const float* const* W, const float* const* B,
+                           void* dst, long long* off_bytes, int* kpad, int* npad);
 cudaError_t hb_launch_sur_tc2(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials,
-                              int* nblocks_out, int sm_count, cudaStream_t s);
-// 0: no tensor-core schedule for this shape, 1: weights resident (hb_sur_tc.cu), 2: weights streamed (hb_sur_tcs.cu),
-// 3: wide nets, one launch per layer, activations through global scratch (hb_sur_tcw.cu)
-int hb_tc_kernel_kind(int prec, int n_linear, const int* widths);
+                              int* nblocks_out, int sm_count, bool prepare, cudaStream_t s);
+int hb_tc_kernel_kind(int prec, int n_linear, const int* widths);     // hb_tc_choose(...).kind
 // wide nets (hidden width 513..1024, equal widths; bf16 / f16): hb_sur_tcw.cu
 #define HB_TCW_CHUNK (1 << 20)        // particles per chunk (scratch: 2 buffers x chunk x padded width x 2 B)
 bool hb_tcw_supported(int prec, int n_linear, const int* widths);
@@ -117,4 +126,4 @@ size_t hb_tcw_scratch_bytes(int n_linear, const int* widths);
 size_t hb_tcw_pack_weights(int prec, int n_linear, const int* widths, const float* const* W,
                            void* dst, long long* off_bytes, int* kpad, int* npad);
 cudaError_t hb_launch_sur_tcw(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials, bool partials_zeroed,
-                              int* nblocks_out, int sm_count, cudaStream_t s);
+                              int* nblocks_out, int sm_count, bool prepare, cudaStream_t s);

@@ -232,14 +232,14 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
 
 template <int TP, bool MOM, int R, int OCB, int KCH>
 static cudaError_t launch_tp(const HbParticles& p, size_t n, const HbSurDev& sd, int hmax, double* partials,
-                             int grid, cudaStream_t s) {
+                             int grid, bool prepare, cudaStream_t s) {
     constexpr int NT = (TP / (4 * R)) * (OCB / (4 * R));
     const size_t smem = ((size_t)2 * hmax * TP + 2 * KCH * OCB) * sizeof(float) + (NT / 32) * HB_NMOM * sizeof(double);
 #define HB_LAUNCH_ACT(A)                                                                                         \
     {                                                                                                            \
-        cudaError_t e = cudaFuncSetAttribute(hb_sur_fp32_kernel<TP, A, MOM, R, OCB, KCH>,                        \
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);            \
-        if (e != cudaSuccess) return e;                                                                          \
+        if (prepare)                                                                                             \
+            return cudaFuncSetAttribute(hb_sur_fp32_kernel<TP, A, MOM, R, OCB, KCH>,                             \
+                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                 \
         hb_sur_fp32_kernel<TP, A, MOM, R, OCB, KCH><<<grid, NT, smem, s>>>(p, n, sd, hmax, partials);            \
     }
     switch (sd.act) {
@@ -252,15 +252,22 @@ static cudaError_t launch_tp(const HbParticles& p, size_t n, const HbSurDev& sd,
     return cudaGetLastError();
 }
 
+// HB_FP32_TP=16|32|64 : test / tuning hook, read by hb_lattice_finalize only (stored in the stage as fp32_tp): forces the
+// 4 x 4 register-tile shape with that many particles per block
+int hb_fp32_env_tp(void) {
+    const char* force = getenv("HB_FP32_TP");
+    return force ? atoi(force) : 0;
+}
+
 cudaError_t hb_launch_sur_fp32(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials,
-                               int* nblocks_out, int sm_count, cudaStream_t s) {
+                               int* nblocks_out, int sm_count, bool prepare, cudaStream_t s) {
     int hmax = 64;
     for (int l = 0; l < sd.n_linear; ++l) hmax = hmax > sd.npad32[l] ? hmax : sd.npad32[l];
     // 8 x 8 register tiles (R = 2), 64 particles per block.  128 < hmax <= 256: 256-wide output blocks, 256 threads,
     // 32-row weight slabs, one block per SM (192 KB).  hmax = 128: 128-wide output blocks, 128 threads, two blocks per
     // SM (80 KB each).  Every layer that runs through the blocked loop must be padded to a multiple of the block width.
-    const char* force = getenv("HB_FP32_TP");
-    const bool classic = force && atoi(force) != 0 && atoi(force) != 128;   // testing: force the 4 x 4 shapes
+    const int force = sd.fp32_tp;
+    const bool classic = force != 0 && force != 128;   // testing: force the 4 x 4 shapes
     auto blocked_multiple_of = [&](int m) {
         for (int l = 0; l < sd.n_linear; ++l) {
             const bool narrow_last = (l == sd.n_linear - 1) && sd.widths[l + 1] <= 8;
@@ -278,15 +285,15 @@ cudaError_t hb_launch_sur_fp32(const HbParticles& p, size_t n, const HbSurDev& s
         if (g < 1) g = 1;
         if (nblocks_out) *nblocks_out = (int)g;
         if (wide256)
-            return mom ? launch_tp<64, true, 2, 256, 32>(p, n, sd, hmax, partials, (int)g, s)
-                       : launch_tp<64, false, 2, 256, 32>(p, n, sd, hmax, partials, (int)g, s);
-        return mom ? launch_tp<64, true, 2, 128, 16>(p, n, sd, hmax, partials, (int)g, s)
-                   : launch_tp<64, false, 2, 128, 16>(p, n, sd, hmax, partials, (int)g, s);
+            return mom ? launch_tp<64, true, 2, 256, 32>(p, n, sd, hmax, partials, (int)g, prepare, s)
+                       : launch_tp<64, false, 2, 256, 32>(p, n, sd, hmax, partials, (int)g, prepare, s);
+        return mom ? launch_tp<64, true, 2, 128, 16>(p, n, sd, hmax, partials, (int)g, prepare, s)
+                   : launch_tp<64, false, 2, 128, 16>(p, n, sd, hmax, partials, (int)g, prepare, s);
     }
     // 4 x 4 tiles: two activation buffers of hmax x TP floats beside the weight slabs; several blocks per SM when they
     // fit (independent blocks hide each other's barriers and slab loads): hmax 256 -> TP 32, 72 KB, 3 blocks/SM
     int tp = hmax <= 128 ? 64 : (hmax <= 768 ? 32 : 16);
-    if (force) tp = atoi(force) == 64 && hmax <= 384 ? 64 : (atoi(force) == 16 ? 16 : (hmax <= 768 ? 32 : 16));
+    if (force) tp = force == 64 && hmax <= 384 ? 64 : (force == 16 ? 16 : (hmax <= 768 ? 32 : 16));
     const size_t smem_blk = ((size_t)2 * hmax * tp + 2 * KC * OC) * sizeof(float) + 1024;
     int per_sm = (int)((227 * 1024) / smem_blk);
     if (per_sm < 1) per_sm = 1;
@@ -297,7 +304,7 @@ cudaError_t hb_launch_sur_fp32(const HbParticles& p, size_t n, const HbSurDev& s
     if (g < 1) g = 1;
     const int grid = (int)g;
     if (nblocks_out) *nblocks_out = grid;
-    if (tp == 64) return mom ? launch_tp<64, true, 1, OC, KC>(p, n, sd, hmax, partials, grid, s) : launch_tp<64, false, 1, OC, KC>(p, n, sd, hmax, partials, grid, s);
-    if (tp == 32) return mom ? launch_tp<32, true, 1, OC, KC>(p, n, sd, hmax, partials, grid, s) : launch_tp<32, false, 1, OC, KC>(p, n, sd, hmax, partials, grid, s);
-    return mom ? launch_tp<16, true, 1, OC, KC>(p, n, sd, hmax, partials, grid, s) : launch_tp<16, false, 1, OC, KC>(p, n, sd, hmax, partials, grid, s);
+    if (tp == 64) return mom ? launch_tp<64, true, 1, OC, KC>(p, n, sd, hmax, partials, grid, prepare, s) : launch_tp<64, false, 1, OC, KC>(p, n, sd, hmax, partials, grid, prepare, s);
+    if (tp == 32) return mom ? launch_tp<32, true, 1, OC, KC>(p, n, sd, hmax, partials, grid, prepare, s) : launch_tp<32, false, 1, OC, KC>(p, n, sd, hmax, partials, grid, prepare, s);
+    return mom ? launch_tp<16, true, 1, OC, KC>(p, n, sd, hmax, partials, grid, prepare, s) : launch_tp<16, false, 1, OC, KC>(p, n, sd, hmax, partials, grid, prepare, s);
 }

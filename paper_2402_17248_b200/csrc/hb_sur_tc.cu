@@ -18,10 +18,15 @@
 // before the layer's first K slab is awaited.
 // Operand.  Layer l >= 1 reads A from tensor memory (tcgen05.mma [d], [a], b-desc): K step kappa of slab j is the
 // 8 columns at 64 j + 32 (kappa / 2) + 8 (kappa mod 2) of D[(l-1) & 1]; shared memory only feeds B.
-// Pipeline.  The accumulator is double-buffered in TMEM (layer l writes D[l & 1]) and the next operand is handed
-// to the MMA issuer per 64-column K slab: the MMAs of layer l+1 start as soon as the epilogue of layer l has
-// converted slab 0 and then run back to back while the epilogue finishes the other slabs; layer 0 of the next
-// tile is issued directly behind the last layer of the current one.
+// Pipeline.  The accumulator is double-buffered in TMEM.  The hidden-layer accumulators of a CTA form one sequence of
+// EVENTS e = 0, 1, 2, ... (tile t, layer l < L-1: e = t (L-1) + l); event e lives in D[e & 1], signals D_HID[e & 1] and
+// its operand slabs SLAB_FULL[e & 1][j].  The next operand is handed to the MMA issuer per 64-column K slab: the MMAs
+// of layer l+1 start as soon as the epilogue of layer l has converted slab 0 and then run back to back while the
+// epilogue finishes the other slabs.  The last layer (N = 16) does not take a buffer of its own: it writes its 16
+// output columns into the gap [16,32) that the in-place packing leaves in chunk 0 of its operand's buffer.  The
+// other buffer is dead by then (it held the operand of layer L-2), so layer 0 of the NEXT tile is issued into it
+// right behind layer L-2 of the current one: its epilogue runs under the current tile's last layer and output, and
+// the tensor pipe does not wait for it (one of the four hand-overs per tile of a 6-256^3-6 net is gone).
 #include "hb_tc_common.cuh"
 
 namespace {
@@ -48,11 +53,11 @@ enum : int {
     B_IN_FULL = 1,        // [2] coordinate rows staged (local)
     B_IN_EMPTY = 3,       // [2] stage consumed by the 4 IO warps (local)
     B_A0_FULL = 5,        // [2] layer-0 operand written (leader; 4 IO warps x CG)
-    B_SLAB_FULL = 7,      // [MAX_SLABS] K slab of the next A operand written (leader; 4G warps x CG)
-    B_D_HID = 11,         // [2] accumulator D[b] of a hidden layer complete (both CTAs, MMA commit)
-    B_D_LAST = 13,        // accumulator of the last layer complete (both CTAs, MMA commit)
-    B_OUT_READ = 14,      // last layer's accumulator read by the IO warps (leader; 4 IO warps x CG)
-    B_COUNT = 15
+    B_SLAB_FULL = 7,      // [2][MAX_SLABS] K slab of the operand packed from event e, set e & 1 (leader; 4G warps x CG)
+    B_D_HID = 15,         // [2] accumulator D[e & 1] of hidden event e complete (both CTAs, MMA commit)
+    B_D_LAST = 17,        // accumulator of the last layer complete (both CTAs, MMA commit)
+    B_OUT_READ = 18,      // last layer's accumulator read by the IO warps (leader; 4 IO warps x CG)
+    B_COUNT = 19
 };
 
 template <int CG, int ACT, bool F16, int G>
@@ -75,7 +80,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
     const size_t ngroups = (ntiles + CG - 1) / CG;
     const size_t cluster_id = blockIdx.x / CG, nclusters = gridDim.x / CG;
     const int L = pl.n_linear;
-    const int last_buf = (L - 1) & 1;
+    constexpr uint32_t OUT_GAP = 16;          // L >= 2: the 16 output columns sit in the gap of chunk 0 of the operand's buffer
 
     const uint32_t bar0 = sbase + pl.bar_off;
     auto bar = [&](int i) -> uint32_t { return bar0 + 8u * (uint32_t)i; };
@@ -90,7 +95,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
             mbar_init(bar(B_A0_FULL + s), 4 * CG);
             mbar_init(bar(B_D_HID + s), 1);
         }
-        for (int j = 0; j < MAX_SLABS; ++j) mbar_init(bar(B_SLAB_FULL + j), 4 * G * CG);
+        for (int j = 0; j < 2 * MAX_SLABS; ++j) mbar_init(bar(B_SLAB_FULL + j), 4 * G * CG);
         mbar_init(bar(B_D_LAST), 1);
         mbar_init(bar(B_OUT_READ), 4 * CG);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -150,11 +155,9 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
             const uint32_t idesc_base = (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)((TILE_M * CG) >> 4) << 24);
             const bool issuer = elect_one();
             const uint64_t w0_desc = make_desc_l0(sbase + pl.w_off[0]);
-            TR_DECL;
-            uint32_t ph_slab = 0;                    // bit j: parity of the next completion of SLAB_FULL[j]
-            uint32_t it = 0;
+            uint32_t ph_slab = 0;                    // bit 4 set + j: parity of the next completion of SLAB_FULL[set][j]
             // per-layer constants are fetched one layer ahead: anything issued behind a batch of MMAs waits for
-            // the tensor pipe's queue, so the loads for layer l+1 go out before the MMAs of layer l
+            // the tensor pipe, so the loads for layer l+1 go out before the MMAs of layer l
             struct LayerC { uint32_t idesc; int nsl; uint64_t bd, bd_step, wbd; };
             auto layer_consts = [&](int l) {
                 LayerC c;
@@ -167,55 +170,76 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
             };
             const LayerC c0 = layer_consts(0);
             const bool more_than_one = L > 1;
-            // layer 0 of tile `t`: one K = 16 MMA from the compact operand buffers.  It is issued directly behind
-            // the last layer of tile t-1, so that its epilogue runs while the IO warps finish tile t-1.
+            const uint32_t nmine = cluster_id < ngroups ? (uint32_t)((ngroups - cluster_id + nclusters - 1) / nclusters) : 0u;
+            // out_in[x]: 1 + the tile whose 16 output columns sit in D[x] and may not have been read yet (0: none).
+            // Whatever overwrites D[x] as a whole (layer 0, a hidden layer's bias MMA) waits for the IO warps first.
+            uint32_t out_in0 = 0u, out_in1 = 0u;
+            auto claim = [&](uint32_t x) {
+                const uint32_t v = x ? out_in1 : out_in0;
+                if (v) {
+                    mbar_wait<true>(bar(B_OUT_READ), (v - 1) & 1);
+                    if (x) out_in1 = 0u; else out_in0 = 0u;
+                }
+            };
+            // layer 0 of tile `t` = hidden event e0 = t (L-1) (or the tile's output when L = 1): one K = 16 MMA from the
+            // compact operand buffers into D[e0 & 1]
             auto issue_l0 = [&](uint32_t t) {
-                // L odd: D[0] is also the output buffer, the IO warps must have read tile t-1 out of it
-                if (last_buf == 0 && t > 0) mbar_wait<true>(bar(B_OUT_READ), (t - 1) & 1);
-                TR(0, 1);
+                const uint32_t x = more_than_one ? ((t * (uint32_t)(L - 1)) & 1u) : 0u;
+                claim(x);
                 mbar_wait<true>(bar(B_A0_FULL + (t & 1)), (t >> 1) & 1);
                 tc_fence_after();
-                TR(0, 2);
                 if (issuer) {
-                    umma<CG, false>(tmem_base, make_desc_l0(sbase + pl.a0_off + (t & 1) * A0_BYTES), w0_desc, c0.idesc);
-                    umma_commit<CG>(more_than_one ? bar(B_D_HID) : bar(B_D_LAST));
+                    umma<CG, false>(tmem_base + x * (uint32_t)pl.d_cols, make_desc_l0(sbase + pl.a0_off + (t & 1) * A0_BYTES),
+                                    w0_desc, c0.idesc);
+                    umma_commit<CG>(more_than_one ? bar(B_D_HID + (int)x) : bar(B_D_LAST));
                 }
                 __syncwarp();
-                TR(0, 32);
+                if (!more_than_one) out_in0 = t + 1;
             };
-            if (cluster_id < ngroups) issue_l0(0);
+            if (nmine > 0) issue_l0(0);
+            if (L == 2 && nmine > 1) issue_l0(1);        // layer L-2 IS layer 0: the next tile's goes out right behind it
             LayerC nxt = layer_consts(more_than_one ? 1 : 0);
-            for (size_t g = cluster_id; g < ngroups; g += nclusters, ++it) {
+            for (uint32_t it = 0; it < nmine; ++it) {
                 for (int l = 1; l < L; ++l) {
                     const LayerC cur = nxt;
                     nxt = layer_consts(l + 1 < L ? l + 1 : 1);
-                    const uint32_t d_tmem = tmem_base + (uint32_t)((l & 1) * pl.d_cols);
-                    // the operand of layer l sits in the accumulator buffer of layer l-1 (written there in place by
-                    // the epilogue): slab j = columns [64 j, 64 j + 16) and [64 j + 32, 64 j + 48), 8 per K = 16 step
-                    const uint32_t a_tmem = tmem_base + (uint32_t)(((l - 1) & 1) * pl.d_cols);
+                    const bool hid = l + 1 < L;
+                    // layer l consumes hidden event e_in (operand packed in place in D[e_in & 1]: slab j = columns
+                    // [64 j, 64 j + 16) and [64 j + 32, 64 j + 48), 8 per K = 16 step); a hidden layer produces event
+                    // e_in + 1 in the other buffer, the last layer writes the gap of its operand's buffer
+                    const uint32_t e_in = it * (uint32_t)(L - 1) + (uint32_t)(l - 1);
+                    const uint32_t xin = e_in & 1u, xout = hid ? xin ^ 1u : xin;
+                    const uint32_t a_tmem = tmem_base + xin * (uint32_t)pl.d_cols;
+                    const uint32_t d_tmem = tmem_base + xout * (uint32_t)pl.d_cols + (hid ? 0u : OUT_GAP);
                     const uint32_t idesc = cur.idesc;
                     const int nsl = cur.nsl;
                     const uint64_t bd = cur.bd, bd_step = cur.bd_step;
-                    // D[last_buf] still holds the previous tile's outputs until the IO warps have read them
-                    if (it > 0 && l == last_buf) mbar_wait<true>(bar(B_OUT_READ), (it - 1) & 1);
+                    if (hid) claim(xout);
                     // hidden layer: the bias goes in first, as one K = 16 MMA of this tile's layer-0 operand (ones
                     // in columns 12, 13) with the layer's bias block (b_hi, b_lo in columns 12, 13, zeros elsewhere).
                     // It depends on nothing the epilogue produces, so it runs in the bubble before slab 0 arrives.
-                    const bool hid = l + 1 < L;
                     if (hid && issuer)
                         umma<CG, false>(d_tmem, make_desc_l0(sbase + pl.a0_off + (it & 1) * A0_BYTES), cur.wbd, idesc);
-                    // fully unrolled over the (at most MAX_SLABS) K slabs
-                    uint32_t ready = 0;               // slab j's barrier already seen complete (peeked)
+                    // The K slabs of the operand arrive one by one from the epilogue warps.  One probe first: lane j
+                    // tests slab j's barrier (test_wait does not suspend) and a ballot tells the warp how many leading
+                    // slabs are already there -- for the last layer, whose operand is usually complete, that is one
+                    // ~150-cycle probe instead of four (polled one by one, the probes cost more than its 16 small MMAs
+                    // take).  The slabs that are not there yet are awaited one by one (try_wait sleeps in hardware and
+                    // wakes ~60 cycles after the last arrive).
+                    const int sset = (int)xin * MAX_SLABS;
+                    const int my_slab = lane < MAX_SLABS ? lane : 0;
+                    const uint32_t ok = lane < nsl ? mbar_test(bar(B_SLAB_FULL + sset + my_slab), (ph_slab >> (sset + my_slab)) & 1u) : 0u;
+                    const uint32_t have = __ballot_sync(0xffffffffu, ok != 0u);
+                    int there = 0;
+                    while (there < nsl && ((have >> there) & 1u)) ++there;
+                    if (there > 0) tc_fence_after();
 #pragma unroll
                     for (int j = 0; j < MAX_SLABS; ++j) {
                         if (j < nsl) {
-                            if (!ready) mbar_wait<true>(bar(B_SLAB_FULL + j), (ph_slab >> j) & 1);
-                            ph_slab ^= 1u << j;
-                            tc_fence_after();
-                            // peek at the next slab before this slab's MMAs go out: whatever the warp issues
-                            // behind a batch of MMAs waits while the tensor pipe's queue is full
-                            ready = (j + 1 < nsl) ? mbar_test(bar(B_SLAB_FULL + j + 1), (ph_slab >> (j + 1)) & 1) : 0u;
-                            if (j == 0) TR(0, 17);
+                            if (j >= there) {
+                                mbar_wait<true>(bar(B_SLAB_FULL + sset + j), (ph_slab >> (sset + j)) & 1);
+                                tc_fence_after();
+                            }
                             if (issuer) {
                                 // four K = 16 steps inside the 64-wide slab: B advances by 32 B, A by 8 columns
                                 // (second 32-column chunk of the slab: + 32)
@@ -229,11 +253,16 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                             }
                         }
                     }
-                    if (issuer) umma_commit<CG>(l == L - 1 ? bar(B_D_LAST) : bar(B_D_HID + (l & 1)));
+                    ph_slab ^= ((1u << nsl) - 1u) << sset;
+                    if (issuer) umma_commit<CG>(hid ? bar(B_D_HID + (int)xout) : bar(B_D_LAST));
                     __syncwarp();
-                    TR(0, 32 + l);
+                    if (!hid) { if (xout) out_in1 = it + 1; else out_in0 = it + 1; }
+                    // behind layer L-2 the buffer that held its operand is dead: layer 0 of the next tile goes there
+                    // (for L = 2 that was done one tile ahead; keep one tile ahead)
+                    if (L > 2 && l == L - 2 && it + 1 < nmine) issue_l0(it + 1);
                 }
-                if (g + nclusters < ngroups) issue_l0(it + 1);
+                if (L == 2 && it + 2 < nmine) issue_l0(it + 2);
+                if (L == 1 && it + 1 < nmine) issue_l0(it + 1);
             }
         }
         __syncwarp();
@@ -242,13 +271,12 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
         const int wq = warp & 3;                 // TMEM lane quarter this warp may access
         const int row = 32 * wq + lane;          // tile row = TMEM lane = particle within the tile
         const uint32_t a0_row = sbase + pl.a0_off + (uint32_t)(row >> 3) * 256 + (uint32_t)(row & 7) * 16;
-        const uint32_t tlane = tmem_base + ((uint32_t)(32 * wq) << 16) + (uint32_t)(last_buf * pl.d_cols);
+        const uint32_t tlane = tmem_base + ((uint32_t)(32 * wq) << 16);
         const float* bl = bias_s;
         HbMomAcc acc;
         acc.clear();
         int stage = 0;
         uint32_t pin = 0;
-        TR_DECL;
         // a4: load, convert, normalise, split, write the layer-0 operand of the tile of group g
         auto prologue = [&](size_t g, uint32_t buf) {
             const size_t tile = g * CG + rank;
@@ -285,7 +313,6 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
             fence_proxy_async();
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(bar(B_A0_FULL + buf), 0);
-            if (warp == IO_WARP0) TR(2, 1);
         };
         mbar_wait<false>(bar(B_W), 0);           // this CTA's weights are resident before the first MMA may start
         uint32_t it = 0;
@@ -295,12 +322,12 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
             const size_t tile = g * CG + rank;
             const size_t i = tile * TILE_M + row;
             const bool valid = tile < ntiles && i < n;
-            if (warp == IO_WARP0) TR(2, 2);
             mbar_wait<false>(bar(B_D_LAST), it & 1);
             tc_fence_after();
-            if (warp == IO_WARP0) TR(2, 3);
             uint32_t r[8];
-            tmem_ld8(tlane, r);
+            // the outputs sit in the gap of the buffer of the tile's last hidden event (L = 1: at column 0 of D[0])
+            const uint32_t e_last = it * (uint32_t)(L - 1) + (uint32_t)(L - 2);
+            tmem_ld8(L > 1 ? tlane + (e_last & 1u) * (uint32_t)pl.d_cols + OUT_GAP : tlane, r);
             tmem_ld_wait();
             tc_fence_before();
             __syncwarp();
@@ -314,7 +341,6 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                 p.v[0][i] = x; p.v[1][i] = px; p.v[2][i] = y; p.v[3][i] = py; p.v[4][i] = t; p.v[5][i] = pt;
                 if (partials) acc.add(sd.mom_pivot, x, px, y, py, t, pt);
             }
-            if (warp == IO_WARP0) TR(2, 4);
         }
         if (partials) {
             double* red = reinterpret_cast<double*>(smem + pl.red_off);
@@ -325,49 +351,46 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
         const int wq = warp & 3;
         const int grp = (warp - EPI_WARP0) >> 2;  // column group inside every 64-column slab
         const uint32_t tlane = tmem_base + ((uint32_t)(32 * wq) << 16);
-        TR_DECL;
-        [[maybe_unused]] const int trole = 4 + (warp - EPI_WARP0);
-        TR(trole, 0);
         uint32_t ph_d = 0;                        // bit b: parity of the next completion of D_HID[b]
-        for (size_t g = cluster_id; g < ngroups; g += nclusters) {
-            for (int l = 0; l < L - 1; ++l) {
-                const int b = l & 1;
-                const int nsl = pl.npad[l] >> 6;
-                const float slope = sd.prelu[l];
-                // this warp's 32-column chunks of the layer: columns 32 * (c * G + grp), c = 0 .. nch-1
-                // (G = 2: one chunk per 64-column slab; G = 1: both chunks of every slab)
-                const int nch = nsl * (2 / G);
-                const uint32_t tl = tlane + (uint32_t)(b * pl.d_cols);
-                mbar_wait<true>(bar(B_D_HID + b), (ph_d >> b) & 1);
-                ph_d ^= 1u << b;
-                tc_fence_after();
-                TR(trole, 2);
-                uint32_t ra[CW], rb[CW];
-                tmem_ld<CW>(tl + (uint32_t)(grp * CW), ra);
-                for (int c = 0; c < nch; c += 2) {
-                    const int col_a = CW * (c * G + grp), col_b = CW * ((c + 1) * G + grp);
+        const uint32_t nmine = cluster_id < ngroups ? (uint32_t)((ngroups - cluster_id + nclusters - 1) / nclusters) : 0u;
+        const uint32_t nev = nmine * (uint32_t)(L - 1);        // hidden events of this CTA, in the order they are issued
+        int l = 0;
+        for (uint32_t e = 0; e < nev; ++e) {
+            const int b = (int)(e & 1u);
+            const int nsl = pl.npad[l] >> 6;
+            const float slope = sd.prelu[l];
+            // this warp's 32-column chunks of the layer: columns 32 * (c * G + grp), c = 0 .. nch-1
+            // (G = 2: one chunk per 64-column slab; G = 1: both chunks of every slab)
+            const int nch = nsl * (2 / G);
+            const uint32_t tl = tlane + (uint32_t)(b * pl.d_cols);
+            const int sset = B_SLAB_FULL + b * MAX_SLABS;
+            mbar_wait<true>(bar(B_D_HID + b), (ph_d >> b) & 1);
+            ph_d ^= 1u << b;
+            tc_fence_after();
+            uint32_t ra[CW], rb[CW];
+            tmem_ld<CW>(tl + (uint32_t)(grp * CW), ra);
+            for (int c = 0; c < nch; c += 2) {
+                const int col_a = CW * (c * G + grp), col_b = CW * ((c + 1) * G + grp);
+                tmem_ld_wait();
+                if (c + 1 < nch) tmem_ld<CW>(tl + (uint32_t)col_b, rb);
+                epi_store_tmem<ACT, F16>(ra, tl + (uint32_t)col_a, slope);
+                if (G == 2 || c + 1 >= nch) {           // chunk a closes its slab
+                    tmem_st_wait();
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive_cluster(bar(sset + (col_a >> 6)), 0);
+                }
+                if (c + 1 < nch) {
                     tmem_ld_wait();
-                    if (c + 1 < nch) tmem_ld<CW>(tl + (uint32_t)col_b, rb);
-                    epi_store_tmem<ACT, F16>(ra, tl + (uint32_t)col_a, slope);
-                    if (G == 2 || c + 1 >= nch) {           // chunk a closes its slab
-                        tmem_st_wait();
-                        tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive_cluster(bar(B_SLAB_FULL + (col_a >> 6)), 0);
-                        if (c == 0) TR(trole, 16);
-                    }
-                    if (c + 1 < nch) {
-                        tmem_ld_wait();
-                        if (c + 2 < nch) tmem_ld<CW>(tl + (uint32_t)(CW * ((c + 2) * G + grp)), ra);
-                        epi_store_tmem<ACT, F16>(rb, tl + (uint32_t)col_b, slope);
-                        tmem_st_wait();
-                        tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive_cluster(bar(B_SLAB_FULL + (col_b >> 6)), 0);
-                        if (c + 2 >= nch) TR(trole, 19);
-                    }
+                    if (c + 2 < nch) tmem_ld<CW>(tl + (uint32_t)(CW * ((c + 2) * G + grp)), ra);
+                    epi_store_tmem<ACT, F16>(rb, tl + (uint32_t)col_b, slope);
+                    tmem_st_wait();
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive_cluster(bar(sset + (col_b >> 6)), 0);
                 }
             }
+            if (++l == L - 1) l = 0;
         }
     }
     // ---- teardown: everyone done with TMEM (both CTAs of a pair), then free it
@@ -437,10 +460,10 @@ bool make_plan(int cg, int n_linear, const int* widths, TcPlan& pl) {
 
 template <int CG, int ACT, bool F16, int G>
 cudaError_t launch_one(const HbParticles& p, size_t n, const HbSurDev& sd, const TcPlan& pl, double* partials, int grid,
-                       cudaStream_t s) {
+                       bool prepare, cudaStream_t s) {
     const size_t smem = (size_t)pl.total + 1024;   // slack so the 1024-byte alignment of the swizzle atoms always holds
-    cudaError_t e = cudaFuncSetAttribute(hb_sur_tc_kernel<CG, ACT, F16, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
+    if (prepare)       // hb_lattice_finalize: the attribute is set once per lattice, not per push
+        return cudaFuncSetAttribute(hb_sur_tc_kernel<CG, ACT, F16, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(tc_threads(G));
@@ -458,103 +481,100 @@ cudaError_t launch_one(const HbParticles& p, size_t n, const HbSurDev& sd, const
 
 template <int CG, bool F16, int G>
 cudaError_t launch_act(const HbParticles& p, size_t n, const HbSurDev& sd, const TcPlan& pl, double* partials, int grid,
-                       cudaStream_t s) {
+                       bool prepare, cudaStream_t s) {
     switch (sd.act) {
-    case 0: return launch_one<CG, 0, F16, G>(p, n, sd, pl, partials, grid, s);
-    case 1: return launch_one<CG, 1, F16, G>(p, n, sd, pl, partials, grid, s);
-    case 2: return launch_one<CG, 2, F16, G>(p, n, sd, pl, partials, grid, s);
-    default: return launch_one<CG, 3, F16, G>(p, n, sd, pl, partials, grid, s);
+    case 0: return launch_one<CG, 0, F16, G>(p, n, sd, pl, partials, grid, prepare, s);
+    case 1: return launch_one<CG, 1, F16, G>(p, n, sd, pl, partials, grid, prepare, s);
+    case 2: return launch_one<CG, 2, F16, G>(p, n, sd, pl, partials, grid, prepare, s);
+    default: return launch_one<CG, 3, F16, G>(p, n, sd, pl, partials, grid, prepare, s);
     }
 }
 
 template <int CG, bool F16>
 cudaError_t launch_g(int g, const HbParticles& p, size_t n, const HbSurDev& sd, const TcPlan& pl, double* partials, int grid,
-                     cudaStream_t s) {
-    if (g == 1) return launch_act<CG, F16, 1>(p, n, sd, pl, partials, grid, s);
-    return launch_act<CG, F16, 2>(p, n, sd, pl, partials, grid, s);
+                     bool prepare, cudaStream_t s) {
+    if (g == 1) return launch_act<CG, F16, 1>(p, n, sd, pl, partials, grid, prepare, s);
+    return launch_act<CG, F16, 2>(p, n, sd, pl, partials, grid, prepare, s);
 }
 
-int choose_cg(int n_linear, const int* widths, TcPlan& pl) {
-    // HB_TC_FORCE_CG=2 : test hook, runs shapes that fit one CTA on a CTA pair as well
-    const char* force = getenv("HB_TC_FORCE_CG");
-    if (force && force[0] == '2') return make_plan(2, n_linear, widths, pl) ? 2 : 0;
-    if (make_plan(1, n_linear, widths, pl)) return 1;
-    if (make_plan(2, n_linear, widths, pl)) return 2;
-    return 0;
-}
-
-// resident kernel if the weights fit in shared memory, else the streamed kernel (hb_sur_tcs.cu).
-// HB_TC_FORCE_STREAM=1 : test hook, runs shapes the resident kernel could take through the streamed one.
-bool use_stream(int prec, int n_linear, const int* widths) {
-    if (prec == 3) return hb_tcs_supported(prec, n_linear, widths);       // tf32 operands: streamed kernel only
-    const char* force = getenv("HB_TC_FORCE_STREAM");
-    if (force && force[0] == '1' && hb_tcs_supported(prec, n_linear, widths)) return true;
-    TcPlan pl;
-    return !choose_cg(n_linear, widths, pl) && hb_tcs_supported(prec, n_linear, widths);
-}
-
-// Launch shape.  Small networks (CTA-pair plan <= 113 KB of shared memory, two accumulators <= 256 TMEM
-// columns) run TWO CTAs per SM with 4 epilogue warps each (G = 1): the second tile's MMAs fill the tensor pipe
-// while the first tile is in its (MUFU- or latency-bound) epilogue.  Everything else: one CTA per SM, G = 2.
-// HB_TC_OCC2=0 : tuning/test hook, disables the two-CTAs-per-SM shape.
-struct TcShape { int cg, g, occ; };
-TcShape choose_shape(int n_linear, const int* widths, TcPlan& pl) {
-    const char* force = getenv("HB_TC_FORCE_CG");
-    const char* occ2 = getenv("HB_TC_OCC2");
-    const bool allow_occ2 = !(occ2 && occ2[0] == '0') && !force;
-    // single CTAs where the whole net fits one (local hand-over barriers: C4 1.45 -> 1.40 ms), else CTA pairs
-    for (int cg = 1; cg <= 2 && allow_occ2; ++cg)
-        if (make_plan(cg, n_linear, widths, pl) && (size_t)pl.total + 2048 <= SMEM_LIMIT / 2 && pl.tmem_cols <= 256)
-            return {cg, 1, 2};
-    const int cg = choose_cg(n_linear, widths, pl);
-    return {cg, 2, 1};
+bool env_is(const char* name, char v) {
+    const char* e = getenv(name);
+    return e && e[0] == v;
 }
 
 }  // namespace
 
-#ifdef HB_TC_TRACE
-extern "C" int hb_debug_tc_trace(long long* host, int count) {
-    return (int)cudaMemcpyFromSymbol(host, hb_tc_trace_buf, sizeof(long long) * (size_t)count);
-}
-#endif
-
-int hb_tc_kernel_kind(int prec, int n_linear, const int* widths) {
-    if (prec < 1 || prec > 3) return 0;
-    if (use_stream(prec, n_linear, widths)) return 2;
-    if (prec == 3) return 0;
+// Which kernel and launch shape a 16-bit / tf32 stage runs on.  Called ONCE per stage by hb_lattice_finalize (and by the
+// host query hb_surrogate_kernel); the choice is stored in the segment, so nothing is decided per push.
+//   kind 1  resident weights, one tile per CTA (this file): nets up to 128 wide run two CTAs per SM (G = 1: four
+//           epilogue warps each; as single CTAs when the whole net fits one, else as pairs), the rest one CTA per SM
+//   kind 4  resident weights, two tiles in flight per CTA (hb_sur_tc2.cu): hidden width above 128
+//   kind 2  weights streamed from L2 (hb_sur_tcs.cu): nets that do not fit resident, and every HB_PREC_TF32 stage
+//   kind 3  one launch per layer (hb_sur_tcw.cu): hidden widths 513..1024
+// Test / tuning hooks read from the environment here and nowhere else: HB_TC_FORCE_CG=2 (CTA-pair shapes for nets that
+// fit one CTA), HB_TC_FORCE_STREAM=1 (streamed kernel for nets that would stay resident), HB_TC_OCC2=0 (no
+// two-CTAs-per-SM shape), HB_TC_ONE_TILE=1 (kind 1 where kind 4 would run).
+HbTcChoice hb_tc_choose(int prec, int n_linear, const int* widths) {
+    HbTcChoice ch{0, 0, 0, 0};
+    if (prec < 1 || prec > 3) return ch;
+    const bool force_cg2 = env_is("HB_TC_FORCE_CG", '2');
     TcPlan pl;
-    if (choose_cg(n_linear, widths, pl)) return 1;
-    return hb_tcw_supported(prec, n_linear, widths) ? 3 : 0;
+    int cg1 = 0;                                         // cluster size of the one-tile plan, 0 = does not fit
+    if (prec != 3) {
+        if (!force_cg2 && make_plan(1, n_linear, widths, pl)) cg1 = 1;
+        else if (make_plan(2, n_linear, widths, pl)) cg1 = 2;
+    }
+    const int cg2 = prec == 3 ? 0 : hb_tc2_plan_cg(n_linear, widths, force_cg2 ? 2 : 0);
+    const bool resident = cg1 != 0 || cg2 != 0;
+    if (prec == 3 || (env_is("HB_TC_FORCE_STREAM", '1') && hb_tcs_supported(prec, n_linear, widths)) || !resident) {
+        if (hb_tcs_supported(prec, n_linear, widths)) ch.kind = 2;
+        else if (prec != 3 && hb_tcw_supported(prec, n_linear, widths)) ch.kind = 3;
+        return ch;
+    }
+    if (cg2 != 0 && !(env_is("HB_TC_ONE_TILE", '1') && cg1 != 0)) {
+        ch.kind = 4;
+        ch.cg = cg2;
+        ch.g = 2;
+        ch.occ = 1;
+        return ch;
+    }
+    ch.kind = 1;
+    // two CTAs per SM for small plans: the second tile's MMAs fill the tensor pipe while the first is in its epilogue
+    const bool allow_occ2 = !env_is("HB_TC_OCC2", '0') && !force_cg2;
+    for (int cg = 1; cg <= 2 && allow_occ2; ++cg)
+        if (make_plan(cg, n_linear, widths, pl) && (size_t)pl.total + 2048 <= SMEM_LIMIT / 2 && pl.tmem_cols <= 256) {
+            ch.cg = cg; ch.g = 1; ch.occ = 2;
+            return ch;
+        }
+    ch.cg = cg1; ch.g = 2; ch.occ = 1;
+    return ch;
 }
+
+int hb_tc_kernel_kind(int prec, int n_linear, const int* widths) { return hb_tc_choose(prec, n_linear, widths).kind; }
 
 bool hb_tc_supported(int prec, int n_linear, const int* widths, char* why, size_t why_len) {
-    if (prec == 3) {
-        if (hb_tcs_supported(prec, n_linear, widths)) return true;
-        snprintf(why, why_len, "HB_PREC_TF32 runs on the streamed kernel only: at least one hidden layer, equal hidden widths <= 256");
-        return false;
-    }
-    if (prec != 1 && prec != 2) {
+    if (prec < 1 || prec > 3) {
         snprintf(why, why_len, "unknown precision %d", prec);
         return false;
     }
-    TcPlan pl;
-    if (!choose_cg(n_linear, widths, pl) && !hb_tcs_supported(prec, n_linear, widths) && !hb_tcw_supported(prec, n_linear, widths)) {
+    if (hb_tc_choose(prec, n_linear, widths).kind != 0) return true;
+    if (prec == 3)
+        snprintf(why, why_len, "HB_PREC_TF32 runs on the streamed kernel only: at least one hidden layer, equal hidden widths <= 256");
+    else
         snprintf(why, why_len, "no tensor-core schedule for this shape: the weights do not fit resident in shared memory "
                                "and the streamed / layered kernels need equal hidden widths <= 512 / <= 1024");
-        return false;
-    }
-    return true;
+    return false;
 }
 
 // Packed operand image.  Layer 0 (K = 16, no swizzle): per 8-row group 256 bytes = K chunk 0 of the 8 rows
 // (8 x 16 B) followed by K chunk 1; W_0 is carried twice (columns 0..5 multiply the hi parts of the inputs,
 // 6..11 the lo parts).  Layers >= 1: per 64-wide K slab, npad rows of 128 bytes (K-major, 128-byte swizzle:
 // the 16-byte chunk c of row r sits at chunk position c ^ (r mod 8)).
-size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float* const* W, const float* const* B,
-                          void* dst, long long* off_bytes, int* kpad, int* npad) {
-    (void)B;
-    if (use_stream(prec, n_linear, widths)) return hb_tcs_pack_weights(prec, n_linear, widths, W, dst, off_bytes, kpad, npad);
-    if (hb_tc_kernel_kind(prec, n_linear, widths) == 3) return hb_tcw_pack_weights(prec, n_linear, widths, W, dst, off_bytes, kpad, npad);
+size_t hb_tc_pack_weights(const HbTcChoice& ch, int prec, int n_linear, const int* widths, const float* const* W,
+                          const float* const* B, void* dst, long long* off_bytes, int* kpad, int* npad) {
+    if (ch.kind == 2) return hb_tcs_pack_weights(prec, n_linear, widths, W, dst, off_bytes, kpad, npad);
+    if (ch.kind == 3) return hb_tcw_pack_weights(prec, n_linear, widths, W, dst, off_bytes, kpad, npad);
+    if (ch.kind == 4) return hb_tc2_pack_weights(prec, ch.cg, n_linear, widths, W, B, dst, off_bytes, kpad, npad);
     int ksteps[HB_MAX_LINEAR];
     layer_geometry(n_linear, widths, kpad, npad, ksteps);
     size_t total = 0;
@@ -610,30 +630,22 @@ size_t hb_tc_pack_weights(int prec, int n_linear, const int* widths, const float
     return total;
 }
 
+// prepare: only set the chosen kernel's shared-memory attribute (hb_lattice_finalize), launch nothing
 cudaError_t hb_launch_sur_tc(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials, int* nblocks_out,
-                             int sm_count, cudaStream_t s) {
-    if (sd.tc_kind == 2) return hb_launch_sur_tcs(p, n, sd, partials, nblocks_out, sm_count, s);
+                             int sm_count, bool prepare, cudaStream_t s) {
+    if (sd.tc_kind == 2) return hb_launch_sur_tcs(p, n, sd, partials, nblocks_out, sm_count, prepare, s);
+    if (sd.tc_kind == 4) return hb_launch_sur_tc2(p, n, sd, partials, nblocks_out, sm_count, prepare, s);
     TcPlan pl;
-    const TcShape sh = choose_shape(sd.n_linear, sd.widths, pl);
-    // HB_TC_TWO_TILES=1 : opt-in to the two-tiles-in-flight kernel (hb_sur_tc2.cu) where its operand ring fits.
-    // Measured slower than this file's pipeline on C3 (3.12 vs 2.63 ms): with an epilogue running under EVERY MMA
-    // phase the MMAs themselves slow from 512 to ~800 cycles per K slab (shared-memory traffic of the operand
-    // stores + proxy fences), which costs more than the exposed first-slab latency it removes.
-    {
-        const char* two = getenv("HB_TC_TWO_TILES");
-        if (sh.cg == 2 && sh.occ == 1 && two && two[0] == '1' && hb_tc2_supported(sd.n_linear, sd.widths))
-            return hb_launch_sur_tc2(p, n, sd, partials, nblocks_out, sm_count, s);
-    }
-    const int cg = sh.cg, g = sh.g;
-    if (cg == 0) return cudaErrorNotSupported;
+    const int cg = sd.tc_cg, g = sd.tc_g;
+    if ((cg != 1 && cg != 2) || !make_plan(cg, sd.n_linear, sd.widths, pl)) return cudaErrorNotSupported;
     const size_t ntiles = (n + TILE_M - 1) / TILE_M;
     const size_t ngroups = (ntiles + cg - 1) / cg;
-    size_t clusters = (size_t)(sm_count / cg) * sh.occ;
+    size_t clusters = (size_t)(sm_count / cg) * sd.tc_occ;
     if (clusters > ngroups) clusters = ngroups;
     if (clusters < 1) clusters = 1;
     const int grid = (int)clusters * cg;
     if (nblocks_out) *nblocks_out = grid;
     const bool f16 = sd.prec == 2;
-    if (cg == 1) return f16 ? launch_g<1, true>(g, p, n, sd, pl, partials, grid, s) : launch_g<1, false>(g, p, n, sd, pl, partials, grid, s);
-    return f16 ? launch_g<2, true>(g, p, n, sd, pl, partials, grid, s) : launch_g<2, false>(g, p, n, sd, pl, partials, grid, s);
+    if (cg == 1) return f16 ? launch_g<1, true>(g, p, n, sd, pl, partials, grid, prepare, s) : launch_g<1, false>(g, p, n, sd, pl, partials, grid, prepare, s);
+    return f16 ? launch_g<2, true>(g, p, n, sd, pl, partials, grid, prepare, s) : launch_g<2, false>(g, p, n, sd, pl, partials, grid, prepare, s);
 }

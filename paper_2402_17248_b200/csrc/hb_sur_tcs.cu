@@ -469,10 +469,9 @@ bool make_splan(int prec, int n_linear, const int* widths, TcsPlan& pl) {
 
 template <int ACT, int EL>
 cudaError_t s_launch_one(const HbParticles& p, size_t n, const HbSurDev& sd, const TcsPlan& pl, double* partials, int grid,
-                         cudaStream_t s) {
+                         bool prepare, cudaStream_t s) {
     const size_t smem = (size_t)pl.total + 1024;
-    cudaError_t e = cudaFuncSetAttribute(hb_sur_tcs_kernel<ACT, EL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
+    if (prepare) return cudaFuncSetAttribute(hb_sur_tcs_kernel<ACT, EL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(S_THREADS);
@@ -490,12 +489,12 @@ cudaError_t s_launch_one(const HbParticles& p, size_t n, const HbSurDev& sd, con
 
 template <int EL>
 cudaError_t s_launch_act(const HbParticles& p, size_t n, const HbSurDev& sd, const TcsPlan& pl, double* partials, int grid,
-                         cudaStream_t s) {
+                         bool prepare, cudaStream_t s) {
     switch (sd.act) {
-    case 0: return s_launch_one<0, EL>(p, n, sd, pl, partials, grid, s);
-    case 1: return s_launch_one<1, EL>(p, n, sd, pl, partials, grid, s);
-    case 2: return s_launch_one<2, EL>(p, n, sd, pl, partials, grid, s);
-    default: return s_launch_one<3, EL>(p, n, sd, pl, partials, grid, s);
+    case 0: return s_launch_one<0, EL>(p, n, sd, pl, partials, grid, prepare, s);
+    case 1: return s_launch_one<1, EL>(p, n, sd, pl, partials, grid, prepare, s);
+    case 2: return s_launch_one<2, EL>(p, n, sd, pl, partials, grid, prepare, s);
+    default: return s_launch_one<3, EL>(p, n, sd, pl, partials, grid, prepare, s);
     }
 }
 
@@ -592,7 +591,7 @@ size_t hb_tcs_pack_weights(int prec, int n_linear, const int* widths, const floa
 }
 
 cudaError_t hb_launch_sur_tcs(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials, int* nblocks_out,
-                              int sm_count, cudaStream_t s) {
+                              int sm_count, bool prepare, cudaStream_t s) {
     TcsPlan pl;
     if (!make_splan(sd.prec, sd.n_linear, sd.widths, pl)) return cudaErrorNotSupported;
     const size_t ntiles = (n + TILE_M - 1) / TILE_M;
@@ -602,6 +601,6 @@ cudaError_t hb_launch_sur_tcs(const HbParticles& p, size_t n, const HbSurDev& sd
     if (clusters < 1) clusters = 1;
     const int grid = (int)clusters * 2;
     if (nblocks_out) *nblocks_out = grid;
-    if (sd.prec == 3) return s_launch_act<2>(p, n, sd, pl, partials, grid, s);
-    return sd.prec == 2 ? s_launch_act<1>(p, n, sd, pl, partials, grid, s) : s_launch_act<0>(p, n, sd, pl, partials, grid, s);
+    if (sd.prec == 3) return s_launch_act<2>(p, n, sd, pl, partials, grid, prepare, s);
+    return sd.prec == 2 ? s_launch_act<1>(p, n, sd, pl, partials, grid, prepare, s) : s_launch_act<0>(p, n, sd, pl, partials, grid, prepare, s);
 }

@@ -368,10 +368,9 @@ long long w_layer_rank_bytes(const TcwPlan& pl, int n_linear, int l) {
 
 template <int ACT, bool F16>
 cudaError_t w_launch_one(const HbParticles& p, size_t n_chunk, const HbSurDev& sd, const TcwPlan& pl, const TcwLayer& ly,
-                         double* partials, int grid, cudaStream_t s) {
+                         double* partials, int grid, bool prepare, cudaStream_t s) {
     const size_t smem = (size_t)pl.total + 1024;
-    cudaError_t e = cudaFuncSetAttribute(hb_sur_tcw_kernel<ACT, F16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
+    if (prepare) return cudaFuncSetAttribute(hb_sur_tcw_kernel<ACT, F16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(W_THREADS);
@@ -389,12 +388,12 @@ cudaError_t w_launch_one(const HbParticles& p, size_t n_chunk, const HbSurDev& s
 
 template <bool F16>
 cudaError_t w_launch_act(int act, const HbParticles& p, size_t n_chunk, const HbSurDev& sd, const TcwPlan& pl,
-                         const TcwLayer& ly, double* partials, int grid, cudaStream_t s) {
+                         const TcwLayer& ly, double* partials, int grid, bool prepare, cudaStream_t s) {
     switch (act) {
-    case 0: return w_launch_one<0, F16>(p, n_chunk, sd, pl, ly, partials, grid, s);
-    case 1: return w_launch_one<1, F16>(p, n_chunk, sd, pl, ly, partials, grid, s);
-    case 2: return w_launch_one<2, F16>(p, n_chunk, sd, pl, ly, partials, grid, s);
-    default: return w_launch_one<3, F16>(p, n_chunk, sd, pl, ly, partials, grid, s);
+    case 0: return w_launch_one<0, F16>(p, n_chunk, sd, pl, ly, partials, grid, prepare, s);
+    case 1: return w_launch_one<1, F16>(p, n_chunk, sd, pl, ly, partials, grid, prepare, s);
+    case 2: return w_launch_one<2, F16>(p, n_chunk, sd, pl, ly, partials, grid, prepare, s);
+    default: return w_launch_one<3, F16>(p, n_chunk, sd, pl, ly, partials, grid, prepare, s);
     }
 }
 
@@ -487,9 +486,14 @@ size_t hb_tcw_pack_weights(int prec, int n_linear, const int* widths, const floa
 // One surrogate stage = chunks x n_linear launches.  partials: this stage's partial buffer (moment-major rows);
 // every chunk's last-layer launch writes its own row range; *nblocks_out = rows the finalize has to sum.
 cudaError_t hb_launch_sur_tcw(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials, bool partials_zeroed,
-                              int* nblocks_out, int sm_count, cudaStream_t s) {
+                              int* nblocks_out, int sm_count, bool prepare, cudaStream_t s) {
     TcwPlan pl;
     if (!make_wplan(sd.prec, sd.n_linear, sd.widths, pl)) return cudaErrorNotSupported;
+    if (prepare) {
+        TcwLayer ly{};
+        return sd.prec == 2 ? w_launch_act<true>(sd.act, p, 0, sd, pl, ly, nullptr, 2, true, s)
+                            : w_launch_act<false>(sd.act, p, 0, sd, pl, ly, nullptr, 2, true, s);
+    }
     if (!sd.act_scratch) return cudaErrorInvalidValue;
     const int grid_max = (sm_count / 2) * 2;
     const size_t nchunks = (n + HB_TCW_CHUNK - 1) / HB_TCW_CHUNK;
@@ -520,8 +524,8 @@ cudaError_t hb_launch_sur_tcw(const HbParticles& p, size_t n, const HbSurDev& sd
             ly.act_out = act[l & 1];
             ly.row_off = off;
             double* part = (partials && ly.last) ? partials + c * (size_t)grid_max : nullptr;
-            e = sd.prec == 2 ? w_launch_act<true>(sd.act, p, nc, sd, pl, ly, part, grid, s)
-                             : w_launch_act<false>(sd.act, p, nc, sd, pl, ly, part, grid, s);
+            e = sd.prec == 2 ? w_launch_act<true>(sd.act, p, nc, sd, pl, ly, part, grid, false, s)
+                             : w_launch_act<false>(sd.act, p, nc, sd, pl, ly, part, grid, false, s);
         }
     }
     if (nblocks_out) *nblocks_out = (int)(nchunks * (size_t)grid_max);

@@ -23,20 +23,6 @@ constexpr int STAGE_BYTES = 6 * TILE_M * 4;
 constexpr int MAX_SLABS = 4;                     // hidden width <= 256
 constexpr size_t SMEM_LIMIT = 227 * 1024;
 
-#ifdef HB_TC_TRACE   // debugging aid (never defined in the product build): per-role event timeline of block 0
-constexpr int TR_ROLES = 40, TR_MAXEV = 1024;
-__device__ long long hb_tc_trace_buf[TR_ROLES * TR_MAXEV];
-#define TR_DECL int trc_ = 0
-#define TR(role, code)                                                                                      \
-    do {                                                                                                    \
-        if (blockIdx.x < 2 && (threadIdx.x & 31) == 0 && trc_ < TR_MAXEV)                                   \
-            hb_tc_trace_buf[((role) + 20 * blockIdx.x) * TR_MAXEV + trc_++] = (clock64() << 8) | (long long)(code);             \
-    } while (0)
-#else
-#define TR_DECL
-#define TR(role, code)
-#endif
-
 // ------------------------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 

@@ -104,7 +104,7 @@ def test_shard_ranges_cover_everything():
 def test_surrogate_kernel_dispatch_is_a_host_decision(hb, monkeypatch):
     """which kernel a shape runs on (the decision hb_lattice_finalize takes) -- BASELINE.json's five configs and the
     edges of each kernel's envelope; unsupported shapes are an error with a reason, never a fallback"""
-    for k in ("HB_TC_FORCE_STREAM", "HB_TC_FORCE_CG", "HB_TC_OCC2", "HB_TC_TWO_TILES"):
+    for k in ("HB_TC_FORCE_STREAM", "HB_TC_FORCE_CG", "HB_TC_OCC2", "HB_TC_ONE_TILE"):
         monkeypatch.delenv(k, raising=False)
     K = hb.hb_surrogate_kernel
     assert K("fp32", [6, 64, 64, 6]) == "fp32-ffma"                       # C1 as specified
