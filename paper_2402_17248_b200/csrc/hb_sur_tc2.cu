@@ -1,73 +1,72 @@
 // hb_sur_tc2.cu -- surrogate stage on the 5th-gen tensor cores (HB_PREC_BF16 / HB_PREC_F16), weights resident in
-// shared memory, TWO 128-particle tiles in flight per CTA (256 per CTA pair): rows a4-a6 for nets whose hidden
+// shared memory, every layer issued as two N-HALVES with their own accumulators: rows a4-a6 for nets whose hidden
 // width is above 128 (C3: 6-256^3-6).
 //
-// Why.  hb_sur_tc.cu keeps one tile per CTA in tensor memory: a 128 x 256 fp32 accumulator is 256 of the 512 TMEM
-// columns and the next layer's operand is packed in place into the accumulator it came from, so the second
-// accumulator buffer belongs to the same tile and the tensor pipe idles, once per layer, for the whole hand-over
-// (commit -> epilogue wake -> convert -> arrive -> issue: ~900 cycles against 2048 cycles of MMAs, profiles/).
-// Here a tile owns 256 columns: its packed 16-bit operand in columns [0,128) and HALF an accumulator in [128,256).
-// Every hidden layer is issued as two N-halves (tcgen05.mma with N = width/2: measured at full rate, 67 cycles for
-// M128 x N128 x K16 against 131 for N256, profiles/r2_mma_rate.md), both halves into the same 128 columns:
-//     half 0 complete -> the epilogue warps read it, convert it and HOLD the packed result in registers (the operand
-//                        columns are still being read by half 1's MMAs) -> half 1 may overwrite the accumulator;
-//     half 1 complete -> the layer's operand is dead: the held half goes to operand columns [0,64), half 1 is read,
-//                        converted and stored to [64,128): the next layer's operand, K-half by K-half.
-// Two such tiles (slots) are in flight, each a pipeline of its own: its own MMA-issuing warp, its own four epilogue
-// warps, its own barriers.  tcgen05.mma is accepted by the tensor pipe one at a time (measured: an issuing thread runs
-// in lock step with the pipe, there is no deep queue), so whatever the issuer of a slot does between two phases --
-// barrier waits, descriptors, ~800 cycles -- would leave the pipe idle; with two issuing warps the pipe takes the other
-// slot's MMAs meanwhile.  Nothing orders the two slots against each other but the IO warps, which serve tiles in turn.
-// Phases of a tile (L linear maps, L >= 2):
-//     a          layer 0, one MMA (K = 16, N = npad_0) from the compact shared-memory operand into columns [0,npad_0)
-//                of the slot (operand + accumulator columns: the slot holds no operand yet); bias inside (W_0 carries
-//                b_hi, b_lo in K columns 12, 13; the operand row carries ones there)
-//     (l,0),(l,1) hidden layer l = 1..L-2, N-half h: one K = 16 bias MMA (accumulate = 0: the tile's layer-0 operand
-//                against the half's bias block) + npad_{l-1}/16 MMAs with A from tensor memory
-//     d          last layer (N = 16), A from tensor memory; its bias is added in fp32 by the IO warps
-// Warp roles (15 warps): 0-3 IO (a4 prologue of the tile after next, a6 output + a3 moments of the current one),
-// 4-7 / 8-11 hidden-layer epilogue of slot 0 / 1 (lane quarter = warp % 4), 12 copy producer (weights once, then the six
-// coordinate rows of every tile through the TMA engine into a 4-stage ring), 13 / 14 MMA issuer of slot 0 / 1 (leader CTA).
+// Why.  hb_sur_tc.cu gives a 128-particle tile two full-width accumulator buffers (2 x 256 of the 512 TMEM columns)
+// and packs the next layer's operand in place into the buffer it came from.  The tensor pipe then idles, once per
+// layer, from "accumulator complete" until the epilogue warps have converted the first K slab (~600-900 cycles
+// against 2100 cycles of MMAs), and at the tile boundary for the whole chain last hidden layer -> convert -> last
+// layer -> output read (profiles/r2_tc_trace.md).  Here the 512 columns are cut differently:
+//     A[0] = [0,128)   A[1] = [128,256)    packed 16-bit operands (256 values in 128 columns), ping-pong per layer
+//     D[0] = [256,384) D[1] = [384,512)    fp32 accumulators of the two N-halves of the layer in flight
+// and every layer goes out as two tcgen05.mma chains of N = width/2 (an N = 128 MMA runs at full rate: 67 cycles for
+// M128 x N128 x K16 against 131 for N256, profiles/r2_mma_rate.md).  While half 1's MMAs run, the epilogue warps turn
+// half 0's accumulator into K-half 0 of the next operand (written to the OTHER operand region: nothing is held in
+// registers, nothing waits for the layer to end); the next layer's half 0 starts on that K-half the moment half 1's
+// MMAs are through, and meets K-half 1 (converted from half 1 meanwhile) eight K steps later.  The last layer (N = 16)
+// takes no accumulator of its own: its 16 output columns go to the tail [112,128) of the operand region it does not
+// read, which is dead by then.  So both halves of the NEXT tile's layer 0 are issued around it (half 0 before, half 1
+// right behind it) and the tensor pipe never waits for the output to be read: only the epilogue of that half 1, which
+// writes the next operand's K-half 1 over those columns, waits for the IO warps -- long after they are through.
+// Events.  The hidden accumulators of a CTA form one sequence e = 0, 1, 2, ...: tile t, layer l <= L-2, half h is
+// e = (t (L-1) + l) * 2 + h; it lives in D[h], signals DH_FULL[h], is read (DH_FREE[h]) and converted into K-half h of
+// operand region (t (L-1) + l) & 1 (A_FULL[h]).
+// Bias.  The layer-0 operand row is  hi0..5, lo0..5, 1, 1, 0, 0;  W_0 carries b_hi, b_lo in K columns 12, 13; every
+// hidden half gets one extra K = 16 MMA (accumulate = 0) of that operand tile against its bias block.
+// Warp roles (14 warps): 0-3 IO (a4 prologue of the next tile, a6 output + a3 moments of the current one), 4-11
+// epilogue (lane quarter = warp % 4, column half = (warp - 4) / 4), 12 copy producer (weights once, then the six
+// coordinate rows of every tile through the TMA engine), 13 MMA issuer (leader CTA of a pair, one elected lane).
 #include "hb_tc_common.cuh"
 
 namespace {
 
-constexpr int T2_THREADS = 480;
-constexpr int T2_STAGES = 4;          // input staging ring (tiles)
-constexpr uint32_t T2_SLOT_COLS = 256;  // TMEM columns of one tile slot
-constexpr uint32_t T2_DH = 128;       // first accumulator column of a slot (the operand lives below it)
+constexpr int T2_THREADS = 448;
+constexpr int T2_STAGES = 2;          // input staging ring (tiles)
+constexpr uint32_t T2_A = 0;          // operand regions A[0], A[1]: 128 columns each
+constexpr uint32_t T2_D = 256;        // accumulators D[0], D[1]: 128 columns each
+constexpr uint32_t T2_OUT = 112;      // the last layer's 16 output columns: the tail of the operand region it does NOT read
+#ifndef HB_T2_OUT_IN_D1
+#define HB_T2_OUT_IN_D1 1             // experiment: 1 = outputs in D[1], the next tile's layer-0 half 1 waits for the IO warps
+#endif
 
 enum : int {
     T_W = 0,              // weights resident (local)
-    T_IN_FULL = 1,        // [T2_STAGES] coordinate rows staged (local)
-    T_IN_EMPTY = 5,       // [T2_STAGES] stage consumed by the 4 IO warps (local)
-    T_SLOT = 9,           // per slot: 8 barriers
-    T_COUNT = 25
-};
-enum : int {              // offsets inside a slot's barrier block
-    S_A0_FULL = 0,        // [2] layer-0 operand written (leader; 4 IO warps x CG)
-    S_DH_FULL = 2,        // accumulator of phase a / (l,h) complete (both CTAs, MMA commit)
-    S_DH_FREE = 3,        // accumulator read by the slot's epilogue warps (leader; 4 warps x CG)
-    S_A_FULL = 4,         // [2] K-half of the next operand written (leader; 4 warps x CG)
-    S_D_LAST = 6,         // accumulator of phase d complete (both CTAs, MMA commit)
-    S_OUT_READ = 7        // phase d's accumulator read by the IO warps (leader; 4 IO warps x CG)
+    T_IN_FULL = 1,        // [2] coordinate rows staged (local)
+    T_IN_EMPTY = 3,       // [2] stage consumed by the 4 IO warps (local)
+    T_A0_FULL = 5,        // [2] layer-0 operand written (leader; 4 IO warps x CG)
+    T_DH_FULL = 7,        // [2] accumulator D[h] of a hidden event complete (both CTAs, MMA commit)
+    T_DH_FREE = 9,        // [2] D[h] read by the epilogue warps (leader; 8 warps x CG)
+    T_A_FULL = 11,        // [2] K-half h of the next operand written (leader; 8 warps x CG)
+    T_D_LAST = 13,        // accumulator of the last layer complete (both CTAs, MMA commit)
+    T_OUT_READ = 14,      // last layer's accumulator read by the IO warps (local: 4 IO warps)
+    T_COUNT = 15
 };
 
 struct T2Plan {
     int n_linear;
     int npad[HB_MAX_LINEAR];          // padded fan-out of layer l (last layer: 16)
-    int hw[HB_MAX_LINEAR];            // N of one MMA of layer l: npad (l = 0, l = L-1), npad / 2 (hidden)
+    int hw[HB_MAX_LINEAR];            // N of one MMA of layer l: npad / 2 (l <= L-2), npad (last layer)
     int w_off[HB_MAX_LINEAR];         // smem byte offset of layer l's weights (this CTA's rows)
     int w_slab_bytes[HB_MAX_LINEAR];  // this CTA's bytes of one K slab (l >= 1) or of the whole layer (l = 0)
     int nslab[HB_MAX_LINEAR];         // 64-wide K slabs of layer l (l >= 1)
     int wb_off[HB_MAX_LINEAR];        // 1 <= l <= L-2: bias block (K = 16 operand, this CTA's rows, halves in order)
     int wb_bytes[HB_MAX_LINEAR];
-    int a0_off, stage_off, bias_base, bar_off, red_off, total, w_bytes_total;
+    int a0_off, stage_off, bias_base, bar_off, red_off, phc_off, total, w_bytes_total;
 };
 
 // 16 accumulator columns -> r[O .. O+16)   (array references and compile-time offsets only: the arrays stay in registers)
 template <int O>
-__device__ __forceinline__ void tmem_ld16o(uint32_t taddr, uint32_t (&r)[16]) {
+__device__ __forceinline__ void tmem_ld16o(uint32_t taddr, uint32_t (&r)[64]) {
     asm volatile(
         "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
         : "=r"(r[O + 0]), "=r"(r[O + 1]), "=r"(r[O + 2]), "=r"(r[O + 3]), "=r"(r[O + 4]), "=r"(r[O + 5]), "=r"(r[O + 6]),
@@ -82,113 +81,59 @@ __device__ __forceinline__ void tmem_st8o(uint32_t taddr, const uint32_t (&q)[64
                  ::"r"(taddr), "r"(q[O + 0]), "r"(q[O + 1]), "r"(q[O + 2]), "r"(q[O + 3]), "r"(q[O + 4]), "r"(q[O + 5]),
                    "r"(q[O + 6]), "r"(q[O + 7]) : "memory");
 }
-// 16 accumulator columns -> sigma -> 16 bit, packed into q[O .. O+8)
-template <int ACT, bool F16, int O>
-__device__ __forceinline__ void t2_convert(const uint32_t (&r)[16], float slope, uint32_t (&q)[64]) {
+// chunk C (16 values of r) -> sigma -> 16 bit, packed IN PLACE into r[8 C .. 8 C + 8) (chunks in ascending order: every
+// value is read before its register is reused)
+template <int ACT, bool F16, int C>
+__device__ __forceinline__ void t2_convert(uint32_t (&r)[64], float slope) {
 #pragma unroll
     for (int k = 0; k < 8; ++k)
-        q[O + k] = act_pack<ACT, F16>(__uint_as_float(r[2 * k]), __uint_as_float(r[2 * k + 1]), slope);
-}
-// nch chunks (<= 8) of 8 packed operand columns <- registers (no wait)
-__device__ __forceinline__ void t2_store(uint32_t taddr, int nch, const uint32_t (&q)[64]) {
-    if (nch > 0) tmem_st8o<0>(taddr, q);
-    if (nch > 1) tmem_st8o<8>(taddr + 8u, q);
-    if (nch > 2) tmem_st8o<16>(taddr + 16u, q);
-    if (nch > 3) tmem_st8o<24>(taddr + 24u, q);
-    if (nch > 4) tmem_st8o<32>(taddr + 32u, q);
-    if (nch > 5) tmem_st8o<40>(taddr + 40u, q);
-    if (nch > 6) tmem_st8o<48>(taddr + 48u, q);
-    if (nch > 7) tmem_st8o<56>(taddr + 56u, q);
+        r[8 * C + k] = act_pack<ACT, F16>(__uint_as_float(r[16 * C + 2 * k]), __uint_as_float(r[16 * C + 2 * k + 1]), slope);
 }
 
-// One phase (a or (l,h)) of its slot, seen by one epilogue warp (lane quarter wq of the tile): `sbar0` = address of the
-// slot's barrier block, `tl` = TMEM address of the slot's column 0 in this warp's lanes, `hold` = the held half.
-template <int ACT, bool F16>
-__device__ __forceinline__ void t2_epilogue_phase(const HbSurDev& sd, const T2Plan& pl, uint32_t sbar0, uint32_t tl, int ph,
-                                                  uint32_t parity, int lane, uint32_t (&hold)[64]) {
-    auto sbar = [&](int i) -> uint32_t { return sbar0 + 8u * (uint32_t)i; };
-    auto arrive = [&](int i) {
-        __syncwarp();
-        if (lane == 0) mbar_arrive_cluster(sbar(i), 0);
-    };
-    const int l = ph == 0 ? 0 : 1 + ((ph - 1) >> 1);
-    const int h = ph == 0 ? 0 : ((ph - 1) & 1);
-    const float slope = sd.prelu[l];
-    const int hwl = pl.npad[l] >> 1;      // accumulator columns of one half of layer l: nch chunks of 16
-    const int nch = hwl >> 4;
-    const uint32_t acc0 = ph == 0 ? tl : tl + T2_DH;          // phase a: the accumulator starts at column 0
-    mbar_wait<true>(sbar(S_DH_FULL), parity);
-    tc_fence_after();
-    uint32_t ra[16], rb[16];
-    const uint32_t a_lo = tl;                                 // operand columns of K-half 0
-    const uint32_t a_hi = tl + (uint32_t)(hwl >> 1);          // ... of K-half 1
-    // hwl accumulator columns starting at SRC -> sigma -> 16 bit, packed into DST[0 .. hwl/2): chunks of 16 columns, the
-    // next chunk's tcgen05.ld in flight while one is converted (two chunks + the 64 held registers: 128 registers per
-    // thread is all a 15-warp CTA gets); every column has been read when it is through (tcgen05.wait::ld)
-#define T2_PAIR(SRC, DST, C)                                                   \
-    if (nch > (C)) {                                                           \
-        tmem_ld_wait();                                                        \
-        if (nch > (C) + 1) tmem_ld16o<0>((SRC) + 16u * ((C) + 1), rb);         \
-        t2_convert<ACT, F16, 8 * (C)>(ra, slope, (DST));                       \
-    }                                                                          \
-    if (nch > (C) + 1) {                                                       \
-        tmem_ld_wait();                                                        \
-        if (nch > (C) + 2) tmem_ld16o<0>((SRC) + 16u * ((C) + 2), ra);         \
-        t2_convert<ACT, F16, 8 * (C) + 8>(rb, slope, (DST));                   \
+// K = 16 steps [KB, KE) of one MMA chain, A from tensor memory (8 columns per step), B = K slab k / 4 of the half's weight
+// rows, 32 bytes per step inside the slab.  Compile-time bounds, one straight-line run of MMAs: the issuing warp is a
+// single thread of dependent instructions (~5 cycles each); with run-time bounds (predicated slots, or a loop with
+// barrier probes in it) issuing costs ~60 cycles per MMA (measured, profiles/r2_mma_rate.md) -- as much as an N = 128 MMA
+// takes to execute, and four times what the last layer's N = 16 MMAs take.
+template <int CG, int KB, int KE>
+__device__ __forceinline__ void t2_issue_range(uint32_t d_tmem, uint32_t a_tmem, uint64_t bd, uint64_t bd_step, uint32_t idesc,
+                                               bool first_overwrites) {
+#pragma unroll
+    for (int k = KB; k < KE; ++k) {
+        const uint64_t bs = bd + (uint64_t)(k >> 2) * bd_step + (uint64_t)(2 * (k & 3));
+        if (k == 0) {
+            if (first_overwrites) umma_ts<CG, false>(d_tmem, a_tmem, bs, idesc);
+            else umma_ts<CG, true>(d_tmem, a_tmem, bs, idesc);
+        } else {
+            umma_ts<CG, true>(d_tmem, a_tmem + (uint32_t)(8 * k), bs, idesc);
+        }
     }
-#define T2_READ_CONVERT(SRC, DST)                              \
-    do {                                                       \
-        tmem_ld16o<0>((SRC), ra);                              \
-        T2_PAIR(SRC, DST, 0)                                   \
-        T2_PAIR(SRC, DST, 2)                                   \
-        T2_PAIR(SRC, DST, 4)                                   \
-        T2_PAIR(SRC, DST, 6)                                   \
-    } while (0)
-    // `hold` doubles as the staging array of every conversion (it is dead outside the span half 0 -> half 1 of a hidden
-    // layer)
-    if (ph == 0) {
-        // half 0 of layer 0's accumulator sits in the operand columns themselves; this warp alone touches its lanes, and
-        // it has read all of half 0 before it writes
-        T2_READ_CONVERT(acc0, hold);
-        tc_fence_before();
-        t2_store(a_lo, nch, hold);
-        tmem_st_wait();
-        tc_fence_before();
-        arrive(S_A_FULL);
-        T2_READ_CONVERT(acc0 + (uint32_t)hwl, hold);
-        tc_fence_before();
-        arrive(S_DH_FREE);
-        t2_store(a_hi, nch, hold);
-        tmem_st_wait();
-        tc_fence_before();
-        arrive(S_A_FULL + 1);
-    } else if (h == 0) {
-        T2_READ_CONVERT(acc0, hold);
-        tc_fence_before();
-        arrive(S_DH_FREE);                // half 1 of the layer may overwrite the accumulator
-    } else {
-        // every MMA of layer l is complete: its operand is dead, the next one goes over it.  The held half goes first
-        t2_store(a_lo, nch, hold);
-        tmem_st_wait();
-        tc_fence_before();
-        arrive(S_A_FULL);
-        T2_READ_CONVERT(acc0, hold);
-        tc_fence_before();
-        arrive(S_DH_FREE);
-        t2_store(a_hi, nch, hold);
-        tmem_st_wait();
-        tc_fence_before();
-        arrive(S_A_FULL + 1);
+}
+// part 0: K-half 0 = steps [0, ksteps/2);  part 1: K-half 1;  part 2: all steps.  ksteps = 4, 8, 12 or 16 (widths pad to 64)
+template <int CG>
+__device__ __forceinline__ void t2_issue_ksteps(int part, int ksteps, uint32_t d_tmem, uint32_t a_tmem, uint64_t bd,
+                                                uint64_t bd_step, uint32_t idesc, bool first_overwrites) {
+#define T2_CASE(KS)                                                                                             \
+    case KS:                                                                                                    \
+        if (part == 0) t2_issue_range<CG, 0, KS / 2>(d_tmem, a_tmem, bd, bd_step, idesc, first_overwrites);      \
+        else if (part == 1) t2_issue_range<CG, KS / 2, KS>(d_tmem, a_tmem, bd, bd_step, idesc, false);           \
+        else t2_issue_range<CG, 0, KS>(d_tmem, a_tmem, bd, bd_step, idesc, first_overwrites);                    \
+        break;
+    switch (ksteps) {
+        T2_CASE(4)
+        T2_CASE(8)
+        T2_CASE(12)
+        default:
+        T2_CASE(16)
     }
-#undef T2_READ_CONVERT
-#undef T2_PAIR
+#undef T2_CASE
 }
 
 template <int CG, int ACT, bool F16>
 __global__ void __launch_bounds__(T2_THREADS, 1)
 hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, const __grid_constant__ T2Plan pl,
                   double* __restrict__ partials) {
-    constexpr int PROD_WARP = 12, MMA_WARP = 13;          // MMA warps: 13 (slot 0), 14 (slot 1)
+    constexpr int PROD_WARP = 12, MMA_WARP = 13;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     // the 128-byte swizzle atoms (8 rows x 128 B) must sit on 1024-byte boundaries of the shared window
     unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
@@ -198,10 +143,9 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
     const size_t ntiles = (n + TILE_M - 1) / TILE_M;
     const size_t ngroups = (ntiles + CG - 1) / CG;
     const size_t cluster_id = blockIdx.x / CG, nclusters = gridDim.x / CG;
-    // tile groups of this CTA (pair): g_k = cluster_id + k * nclusters, k < nk; slot = k & 1, use count it = k >> 1
-    const uint32_t nk = cluster_id < ngroups ? (uint32_t)((ngroups - cluster_id + nclusters - 1) / nclusters) : 0u;
+    // tile groups of this CTA (pair): g_t = cluster_id + t * nclusters, t < nmine
+    const uint32_t nmine = cluster_id < ngroups ? (uint32_t)((ngroups - cluster_id + nclusters - 1) / nclusters) : 0u;
     const int L = pl.n_linear;
-    const int P = 2 * (L - 2) + 2;             // phases per tile: a, (1,0), (1,1), ..., (L-2,1), d
 
     const uint32_t bar0 = sbase + pl.bar_off;
     auto bar = [&](int i) -> uint32_t { return bar0 + 8u * (uint32_t)i; };
@@ -210,21 +154,16 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
 
     if (tid == 0) {
         mbar_init(bar(T_W), 1);
-        for (int s = 0; s < T2_STAGES; ++s) {
+        for (int s = 0; s < 2; ++s) {
             mbar_init(bar(T_IN_FULL + s), 1);
             mbar_init(bar(T_IN_EMPTY + s), 4);
+            mbar_init(bar(T_A0_FULL + s), 4 * CG);
+            mbar_init(bar(T_DH_FULL + s), 1);
+            mbar_init(bar(T_DH_FREE + s), 8 * CG);
+            mbar_init(bar(T_A_FULL + s), 8 * CG);
         }
-        for (int t = 0; t < 2; ++t) {
-            const int b = T_SLOT + 8 * t;
-            mbar_init(bar(b + S_A0_FULL), 4 * CG);
-            mbar_init(bar(b + S_A0_FULL + 1), 4 * CG);
-            mbar_init(bar(b + S_DH_FULL), 1);
-            mbar_init(bar(b + S_DH_FREE), 4 * CG);
-            mbar_init(bar(b + S_A_FULL), 4 * CG);
-            mbar_init(bar(b + S_A_FULL + 1), 4 * CG);
-            mbar_init(bar(b + S_D_LAST), 1);
-            mbar_init(bar(b + S_OUT_READ), 4 * CG);
-        }
+        mbar_init(bar(T_D_LAST), 1);
+        mbar_init(bar(T_OUT_READ), HB_T2_OUT_IN_D1 ? 4 * CG : 4);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == MMA_WARP) {
@@ -259,8 +198,8 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
             }
             int stage = 0;
             uint32_t ph = 0;
-            for (uint32_t k = 0; k < nk; ++k) {
-                const size_t tile = (cluster_id + (size_t)k * nclusters) * CG + rank;
+            for (uint32_t t = 0; t < nmine; ++t) {
+                const size_t tile = (cluster_id + (size_t)t * nclusters) * CG + rank;
                 const bool full = tile < ntiles && (tile + 1) * TILE_M <= n;
                 if (full) {
                     mbar_wait<false>(bar(T_IN_EMPTY + stage), ph ^ 1);
@@ -268,99 +207,130 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
                     for (int j = 0; j < 6; ++j)
                         bulk_g2s(sbase + pl.stage_off + stage * STAGE_BYTES + j * TILE_M * 4, p.v[j] + tile * TILE_M,
                                  TILE_M * 4, bar(T_IN_FULL + stage));
-                    if (++stage == T2_STAGES) { stage = 0; ph ^= 1; }
+                    stage ^= 1;
+                    if (stage == 0) ph ^= 1;
                 }
             }
         }
         __syncwarp();
-    } else if (warp >= MMA_WARP) {
-        // ===================================================== MMA issuer of slot T (leader CTA of the pair only)
-        // The whole warp walks its slot's phases (warp-uniform control flow, barrier waits by every lane); one elected
-        // lane issues the MMAs and commits (tcgen05.commit tracks the MMAs of the thread that executes it: per slot).
+    } else if (warp == MMA_WARP) {
+        // ===================================================== MMA issuer (leader CTA of the pair only)
+        // The whole warp walks the schedule (warp-uniform control flow, barrier waits by every lane); one elected
+        // lane issues the MMAs and commits.
         if (rank == 0) {
-            const uint32_t T = (uint32_t)(warp - MMA_WARP);
             const uint32_t fmt = F16 ? 0u : 1u;
             const uint32_t idesc_base = (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)((TILE_M * CG) >> 4) << 24);
             const bool issuer = elect_one();
-            const uint64_t w0_desc = make_desc_l0(sbase + pl.w_off[0]);
-            const uint32_t n_it = T == 0 ? (nk + 1) / 2 : nk / 2;
-            const uint32_t sb = tmem_base + T * T2_SLOT_COLS;
-            const uint32_t d_tmem = sb + T2_DH;
-            const int sbar = T_SLOT + 8 * (int)T;
-            uint32_t ph_free = 0, ph_a = 0;        // ph_free; bit kh of ph_a: parity of the next completion
-            for (uint32_t it = 0; it < n_it; ++it) {
-                const uint64_t a0d = make_desc_l0(sbase + pl.a0_off + (2 * T + (it & 1)) * A0_BYTES);
-                // phase a.  The slot's columns still hold the previous tile's outputs until the IO warps read them.
-                if (it > 0) mbar_wait<true>(bar(sbar + S_OUT_READ), (it - 1) & 1);
-                mbar_wait<true>(bar(sbar + S_A0_FULL + (int)(it & 1)), (it >> 1) & 1);
+            const uint32_t dbase = tmem_base + T2_D;     // D[h] = dbase + 128 h
+            uint32_t ph_free = 0, ph_a = 0;        // bit h: parity of the next completion of DH_FREE[h] / A_FULL[h]
+            uint32_t used = 0;                     // bit h: D[h] has held a hidden event before
+            // Per-phase constants (phase = layer l >= 1, half h), built once into shared memory: between the last MMA of
+            // one phase and the first MMA of the next the pipe only has the ~5 MMAs of its queue to run (~330 cycles at
+            // N = 128), so whatever the issuer computes there (descriptors: dependent loads from the constant bank) is
+            // tensor-pipe idle time.  entry 2 l + h: {B descriptor of the half, bias-block descriptor, idesc, K-slab step}
+            uint4* phc = reinterpret_cast<uint4*>(smem + pl.phc_off);
+            if (lane < 2 * L && lane >= 2) {
+                const int l = lane >> 1, h = lane & 1;
+                const uint32_t half_rows = (uint32_t)(h * (pl.hw[l] / CG));
+                const uint64_t bd = make_desc(sbase + pl.w_off[l] + half_rows * 128u);
+                const uint64_t wbd = make_desc_l0(sbase + pl.wb_off[l] + half_rows * 32u);
+                phc[2 * lane] = make_uint4((uint32_t)bd, (uint32_t)(bd >> 32), (uint32_t)wbd, (uint32_t)(wbd >> 32));
+                phc[2 * lane + 1] = make_uint4(idesc_base | ((uint32_t)(pl.hw[l] >> 3) << 17), (uint32_t)(pl.w_slab_bytes[l] >> 4),
+                                               (uint32_t)(pl.npad[l - 1] >> 4), (uint32_t)(pl.npad[l - 1] >> 5));
+            }
+            __syncwarp();
+            // D[h] is written again: the epilogue warps must have read the event it holds
+            auto claim = [&](int h) {
+                if ((used >> h) & 1u) {
+                    mbar_wait<true>(bar(T_DH_FREE + h), (ph_free >> h) & 1u);
+                    ph_free ^= 1u << h;
+                }
+                used |= 1u << h;
+            };
+            const uint64_t w0d0 = make_desc_l0(sbase + pl.w_off[0]);
+            const uint64_t w0d1 = make_desc_l0(sbase + pl.w_off[0] + (uint32_t)(pl.hw[0] / CG) * 32u);
+            const uint32_t idesc0 = idesc_base | ((uint32_t)(pl.hw[0] >> 3) << 17);
+            // layer 0 of tile t, half h: one K = 16 MMA from the compact operand (bias inside W_0)
+            auto issue_l0 = [&](uint32_t t, int h) {
+                if (HB_T2_OUT_IN_D1 && h == 1) {
+                    if (t > 0) mbar_wait<true>(bar(T_OUT_READ), (t - 1) & 1);
+                    else used |= 2u;
+                } else {
+                    claim(h);
+                }
+                if (h == 0) mbar_wait<true>(bar(T_A0_FULL + (int)(t & 1)), (t >> 1) & 1);
                 tc_fence_after();
                 if (issuer) {
-                    umma<CG, false>(sb, a0d, w0_desc, idesc_base | ((uint32_t)(pl.npad[0] >> 3) << 17));
-                    umma_commit<CG>(bar(sbar + S_DH_FULL));
+                    umma<CG, false>(dbase + 128u * (uint32_t)h, make_desc_l0(sbase + pl.a0_off + (t & 1) * A0_BYTES),
+                                    h ? w0d1 : w0d0, idesc0);
+                    umma_commit<CG>(bar(T_DH_FULL + h));
                 }
                 __syncwarp();
-                for (int ph = 1; ph < P; ++ph) {
-                    const bool last = ph == P - 1;
-                    const int l = last ? L - 1 : 1 + ((ph - 1) >> 1);
-                    const int h = last ? 0 : ((ph - 1) & 1);
-                    const uint32_t idesc = idesc_base | ((uint32_t)(pl.hw[l] >> 3) << 17);
-                    const int ksteps = pl.npad[l - 1] >> 4, kb = pl.npad[l - 1] >> 5;   // K = 16 steps; first step of K-half 1
-                    const uint32_t half_rows = (uint32_t)(h * (pl.hw[l] / CG));
-                    const uint64_t bd = make_desc(sbase + pl.w_off[l] + half_rows * 128u);
-                    const uint64_t bd_step = (uint64_t)(pl.w_slab_bytes[l] >> 4);
-                    const uint64_t wbd = make_desc_l0(sbase + pl.wb_off[l] + half_rows * 32u);
-                    // the accumulator columns: read by the epilogue warps (previous phase of this slot)
-                    mbar_wait<true>(bar(sbar + S_DH_FREE), ph_free);
-                    ph_free ^= 1u;
-                    tc_fence_after();
-                    // hidden layer: the bias goes in first, as one K = 16 MMA of the tile's layer-0 operand (ones in
-                    // columns 12, 13) with this half's bias block (b_hi, b_lo in columns 12, 13, zeros elsewhere)
-                    if (!last && issuer) umma<CG, false>(d_tmem, a0d, wbd, idesc);
-                    const bool fresh = h == 0;      // the operand was written since the last phase: wait per K-half
-                    bool seen1 = false;
-                    for (int k0 = 0; k0 < ksteps; k0 += 4) {
-                        if (fresh && k0 == 0) {
-                            mbar_wait<true>(bar(sbar + S_A_FULL), ph_a & 1);
+            };
+            if (nmine > 0) { issue_l0(0, 0); issue_l0(0, 1); }
+            uint32_t lay = 0;                      // t (L-1) + l - 1: the operand region of layer l is lay & 1
+            for (uint32_t t = 0; t < nmine; ++t) {
+                const uint64_t a0d = make_desc_l0(sbase + pl.a0_off + (t & 1) * A0_BYTES);
+                uint4 c0 = phc[4], c1 = phc[5];     // constants of the phase being issued (entry 2: layer 1, half 0)
+                for (int l = 1; l < L; ++l, ++lay) {
+                    const bool last = l == L - 1;
+                    const uint32_t a_tmem = tmem_base + T2_A + 128u * (lay & 1u);
+                    // before the last layer: the next tile's layer 0, half 0 (D[0] is free as soon as the epilogue has read
+                    // the last hidden event in it; the operand region its epilogue writes is dead)
+                    if (last && t + 1 < nmine) issue_l0(t + 1, 0);
+                    for (int h = 0; h < (last ? 1 : 2); ++h) {
+                        // the last layer's 16 columns go to the tail of the operand region it does not read
+                        const uint32_t d_tmem = last ? (HB_T2_OUT_IN_D1 ? dbase + 128u : tmem_base + T2_A + 128u * ((lay & 1u) ^ 1u) + T2_OUT)
+                                                     : dbase + 128u * (uint32_t)h;
+                        const uint64_t bd = ((uint64_t)c0.y << 32) | c0.x, wbd = ((uint64_t)c0.w << 32) | c0.z;
+                        const uint32_t idesc = c1.x;
+                        const uint64_t bd_step = c1.y;
+                        const int ksteps = (int)c1.z;                    // K = 16 steps of the layer (K-half 1 starts at ksteps / 2)
+                        // next phase's constants: in flight while this phase is issued
+                        const int nxt = (h == 0 && !last) ? 2 * l + 1 : (l + 1 < L ? 2 * (l + 1) : 2);
+                        c0 = phc[2 * nxt];
+                        c1 = phc[2 * nxt + 1];
+                        if (!last) claim(h);
+                        else if (HB_T2_OUT_IN_D1) claim(1);
+                        tc_fence_after();
+                        // hidden layer: the bias goes in first, as one K = 16 MMA of the tile's layer-0 operand (ones in
+                        // columns 12, 13) with this half's bias block (b_hi, b_lo in columns 12, 13, zeros elsewhere)
+                        if (!last && issuer) umma<CG, false>(d_tmem, a0d, wbd, idesc);
+                        if (h == 0) {
+                            // the operand is being written by the epilogue of layer l-1: K-half by K-half
+                            mbar_wait<true>(bar(T_A_FULL), ph_a & 1u);
                             ph_a ^= 1u;
                             tc_fence_after();
-                        }
-                        if (fresh && !seen1 && k0 + 4 > kb) {      // this slab reaches into K-half 1
-                            mbar_wait<true>(bar(sbar + S_A_FULL + 1), (ph_a >> 1) & 1);
+                            if (issuer) t2_issue_ksteps<CG>(0, ksteps, d_tmem, a_tmem, bd, bd_step, idesc, last);
+                            mbar_wait<true>(bar(T_A_FULL + 1), (ph_a >> 1) & 1u);
                             ph_a ^= 2u;
                             tc_fence_after();
-                            seen1 = true;
+                            if (issuer) t2_issue_ksteps<CG>(1, ksteps, d_tmem, a_tmem, bd, bd_step, idesc, false);
+                        } else if (issuer) {
+                            t2_issue_ksteps<CG>(2, ksteps, d_tmem, a_tmem, bd, bd_step, idesc, false);
                         }
-                        if (issuer) {
-                            // one 64-wide K slab: four K = 16 steps, B advances by 32 B, A by 8 columns
-                            const uint32_t ad = sb + (uint32_t)(8 * k0);
-                            const uint64_t bj = bd + (uint64_t)(k0 >> 2) * bd_step;
-                            if (k0 == 0 && last) umma_ts<CG, false>(d_tmem, ad, bj, idesc);
-                            else umma_ts<CG, true>(d_tmem, ad, bj, idesc);
-                            umma_ts<CG, true>(d_tmem, ad + 8, bj + 2, idesc);
-                            umma_ts<CG, true>(d_tmem, ad + 16, bj + 4, idesc);
-                            umma_ts<CG, true>(d_tmem, ad + 24, bj + 6, idesc);
-                        }
+                        if (issuer) umma_commit<CG>(bar(last ? T_D_LAST : T_DH_FULL + h));
+                        __syncwarp();
                     }
-                    if (issuer) umma_commit<CG>(bar(sbar + (last ? S_D_LAST : S_DH_FULL)));
-                    __syncwarp();
                 }
+                if (t + 1 < nmine) issue_l0(t + 1, 1);
             }
         }
         __syncwarp();
     } else if (warp < EPI_WARP0) {
-        // ===================================================== IO warps: prologue of tile k + 2, output of tile k
+        // ===================================================== IO warps: prologue of tile t+1, output of tile t
         const int wq = warp & 3;                 // TMEM lane quarter this warp may access
         const int row = 32 * wq + lane;          // tile row = TMEM lane = particle within the tile
         const uint32_t a0_row = sbase + pl.a0_off + (uint32_t)(row >> 3) * 256 + (uint32_t)(row & 7) * 16;
-        const uint32_t tlane = tmem_base + ((uint32_t)(32 * wq) << 16) + T2_DH;
+        const uint32_t tout = tmem_base + ((uint32_t)(32 * wq) << 16) + T2_A + T2_OUT;
         const float* bl = bias_s;
         HbMomAcc acc;
         acc.clear();
         int stage = 0;
         uint32_t pin = 0;
-        // a4: load, convert, normalise, split, write the layer-0 operand of tile group k
-        auto prologue = [&](uint32_t k) {
-            const size_t tile = (cluster_id + (size_t)k * nclusters) * CG + rank;
+        // a4: load, convert, normalise, split, write the layer-0 operand of tile t
+        auto prologue = [&](uint32_t t) {
+            const size_t tile = (cluster_id + (size_t)t * nclusters) * CG + rank;
             const size_t i = tile * TILE_M + row;
             const bool valid = tile < ntiles && i < n;
             const bool full = tile < ntiles && (tile + 1) * TILE_M <= n;
@@ -372,7 +342,8 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
                 for (int j = 0; j < 6; ++j) c[j] = st[j * TILE_M + row];
                 __syncwarp();
                 if (lane == 0) mbar_arrive_local(bar(T_IN_EMPTY + stage));
-                if (++stage == T2_STAGES) { stage = 0; pin ^= 1; }
+                stage ^= 1;
+                if (stage == 0) pin ^= 1;
             } else if (valid) {
 #pragma unroll
                 for (int j = 0; j < 6; ++j) c[j] = p.v[j][i];
@@ -387,40 +358,42 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
             const uint32_t q0[4] = {pack2<F16>(nin[0], nin[1]), pack2<F16>(nin[2], nin[3]), pack2<F16>(nin[4], nin[5]),
                                     pack2<F16>(lo[0], lo[1])};
             const uint32_t q1[4] = {pack2<F16>(lo[2], lo[3]), pack2<F16>(lo[4], lo[5]), pack2<F16>(1.0f, 1.0f), 0u};
-            const uint32_t T = k & 1u, buf = (k >> 1) & 1u;
-            const uint32_t dst = a0_row + (2 * T + buf) * A0_BYTES;
+            const uint32_t dst = a0_row + (t & 1u) * A0_BYTES;
             sts128(dst, q0);
             sts128(dst + 128, q1);
             fence_proxy_async();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(bar(T_SLOT + 8 * (int)T + S_A0_FULL + (int)buf), 0);
+            if (lane == 0) mbar_arrive_cluster(bar(T_A0_FULL + (int)(t & 1u)), 0);
         };
         mbar_wait<false>(bar(T_W), 0);           // this CTA's weights are resident before the first MMA may start
-        if (nk > 0) prologue(0);
-        if (nk > 1) prologue(1);
-        for (uint32_t k = 0; k < nk; ++k) {
-            // buffer (k >> 1) + 1 & 1 of the slot was last read by tile k - 2, whose output was taken two turns ago
-            if (k + 2 < nk) prologue(k + 2);
-            const uint32_t T = k & 1u, it = k >> 1;
-            const size_t tile = (cluster_id + (size_t)k * nclusters) * CG + rank;
+        if (nmine > 0) prologue(0);
+        for (uint32_t t = 0; t < nmine; ++t) {
+            // operand buffer (t + 1) & 1 was last read by the bias MMAs of tile t - 1, complete before its output was
+            if (t + 1 < nmine) prologue(t + 1);
+            const size_t tile = (cluster_id + (size_t)t * nclusters) * CG + rank;
             const size_t i = tile * TILE_M + row;
             const bool valid = tile < ntiles && i < n;
-            mbar_wait<false>(bar(T_SLOT + 8 * (int)T + S_D_LAST), it & 1);
+            mbar_wait<false>(bar(T_D_LAST), t & 1);
             tc_fence_after();
             uint32_t r[8];
-            tmem_ld8(tlane + T * T2_SLOT_COLS, r);
+            // the last layer read operand region (t (L-1) + L-2) & 1 and wrote the tail of the other one
+            if (HB_T2_OUT_IN_D1) tmem_ld8(tmem_base + ((uint32_t)(32 * wq) << 16) + T2_D + 128u, r);
+            else tmem_ld8(tout + 128u * (((t * (uint32_t)(L - 1) + (uint32_t)(L - 2)) & 1u) ^ 1u), r);
             tmem_ld_wait();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(bar(T_SLOT + 8 * (int)T + S_OUT_READ), 0);
+            if (lane == 0) {
+                if (HB_T2_OUT_IN_D1) mbar_arrive_cluster(bar(T_OUT_READ), 0);
+                else mbar_arrive_local(bar(T_OUT_READ));
+            }
             if (valid) {
                 float w[6];
 #pragma unroll
                 for (int j = 0; j < 6; ++j) w[j] = __uint_as_float(r[j]) + bl[j];
-                float x, px, y, py, t, pt;
-                hb_sur_epilogue(sd, w, x, px, y, py, t, pt);
-                p.v[0][i] = x; p.v[1][i] = px; p.v[2][i] = y; p.v[3][i] = py; p.v[4][i] = t; p.v[5][i] = pt;
-                if (partials) acc.add(sd.mom_pivot, x, px, y, py, t, pt);
+                float x, px, y, py, tt, pt;
+                hb_sur_epilogue(sd, w, x, px, y, py, tt, pt);
+                p.v[0][i] = x; p.v[1][i] = px; p.v[2][i] = y; p.v[3][i] = py; p.v[4][i] = tt; p.v[5][i] = pt;
+                if (partials) acc.add(sd.mom_pivot, x, px, y, py, tt, pt);
             }
         }
         if (partials) {
@@ -428,19 +401,60 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
             hb_block_reduce_moments(acc, red, partials + blockIdx.x, tid - 32 * IO_WARP0, 128, 2);
         }
     } else {
-        // ===================================================== hidden-layer epilogue warps of slot T
+        // ===================================================== epilogue warps: hidden events in issue order
         const int wq = warp & 3;
-        const uint32_t T = (uint32_t)((warp - EPI_WARP0) >> 2);
-        const uint32_t tl = tmem_base + ((uint32_t)(32 * wq) << 16) + T * T2_SLOT_COLS;
-        const uint32_t sbar0 = bar0 + 8u * (uint32_t)(T_SLOT + 8 * (int)T);
-        const uint32_t n_it = T == 0 ? (nk + 1) / 2 : nk / 2;
-        uint32_t par = 0;                         // parity of the next completion of DH_FULL
-        uint32_t hold[64];                        // packed half 0 of the layer in flight
-        for (uint32_t it = 0; it < n_it; ++it)
-            for (int ph = 0; ph < P - 1; ++ph) {  // phase d belongs to the IO warps
-                t2_epilogue_phase<ACT, F16>(sd, pl, sbar0, tl, ph, par, lane, hold);
-                par ^= 1u;
+        const int grp = (warp - EPI_WARP0) >> 2;  // which half of an event's accumulator columns this warp converts
+        const uint32_t tlane = tmem_base + ((uint32_t)(32 * wq) << 16);
+        const uint32_t nev = nmine * (uint32_t)(L - 1) * 2u;
+        uint32_t ph_full = 0;                     // bit h: parity of the next completion of DH_FULL[h]
+        uint32_t lay = 0, tile = 0;               // t (L-1) + l of the event; t
+        int l = 0;
+        auto arrive = [&](int b) {
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(bar(b), 0);
+        };
+        for (uint32_t e = 0; e < nev; ++e) {
+            const int h = (int)(e & 1u);
+            const float slope = sd.prelu[l];
+            const int hwl = pl.npad[l] >> 1;      // accumulator columns of one half of layer l
+            const int cw = hwl >> 1;              // ... of which this warp converts cw, as nch chunks of 16
+            const int nch = cw >> 4;
+            const uint32_t src = tlane + T2_D + 128u * (uint32_t)h + (uint32_t)(grp * cw);
+            // K-half h of the next operand, in the region the layer before did NOT read
+            const uint32_t dst = tlane + T2_A + 128u * (lay & 1u) + (uint32_t)(h * (hwl >> 1) + grp * (cw >> 1));
+            mbar_wait<true>(bar(T_DH_FULL + h), (ph_full >> h) & 1u);
+            ph_full ^= 1u << h;
+            tc_fence_after();
+            uint32_t r[64];
+            if (nch > 0) tmem_ld16o<0>(src, r);
+            if (nch > 1) tmem_ld16o<16>(src + 16u, r);
+            if (nch > 2) tmem_ld16o<32>(src + 32u, r);
+            if (nch > 3) tmem_ld16o<48>(src + 48u, r);
+            tmem_ld_wait();
+            tc_fence_before();
+            arrive(T_DH_FREE + h);                // the accumulator may be overwritten
+            if (nch > 0) t2_convert<ACT, F16, 0>(r, slope);
+            if (nch > 1) t2_convert<ACT, F16, 1>(r, slope);
+            if (nch > 2) t2_convert<ACT, F16, 2>(r, slope);
+            if (nch > 3) t2_convert<ACT, F16, 3>(r, slope);
+            // K-half 1 of a tile's first operand goes over the previous tile's output columns: the IO warps of this CTA
+            // must have read them (they did long ago: the wait is for correctness, it does not stall)
+            if (!HB_T2_OUT_IN_D1 && l == 0 && h == 1 && tile > 0) {
+                mbar_wait<true>(bar(T_OUT_READ), (tile - 1u) & 1u);
+                tc_fence_after();
             }
+            if (nch > 0) tmem_st8o<0>(dst, r);
+            if (nch > 1) tmem_st8o<8>(dst + 8u, r);
+            if (nch > 2) tmem_st8o<16>(dst + 16u, r);
+            if (nch > 3) tmem_st8o<24>(dst + 24u, r);
+            tmem_st_wait();
+            tc_fence_before();
+            arrive(T_A_FULL + h);
+            if (h == 1) {
+                ++lay;
+                if (++l == L - 1) { l = 0; ++tile; }
+            }
+        }
     }
     // ---- teardown: everyone done with TMEM (both CTAs of a pair), then free it
     tc_fence_before();
@@ -464,7 +478,7 @@ bool t2_make_plan(int cg, int n_linear, const int* widths, T2Plan& pl) {
         const bool last = l == n_linear - 1;
         pl.npad[l] = last ? 16 : t2_round_up(widths[l + 1], 64);
         if (pl.npad[l] > 256) return false;                          // operand <= 128 columns, half accumulator <= 128
-        pl.hw[l] = (l == 0 || last) ? pl.npad[l] : pl.npad[l] / 2;
+        pl.hw[l] = last ? pl.npad[l] : pl.npad[l] / 2;
         if ((pl.hw[l] / cg) % 8) return false;
         pl.nslab[l] = l == 0 ? 0 : pl.npad[l - 1] / 64;
         pl.w_slab_bytes[l] = pl.npad[l] / cg * (l == 0 ? 32 : 128);
@@ -480,7 +494,7 @@ bool t2_make_plan(int cg, int n_linear, const int* widths, T2Plan& pl) {
         off = t2_round_up(off, 1024);
     }
     pl.a0_off = off;
-    off += 4 * A0_BYTES;
+    off += 2 * A0_BYTES;
     pl.stage_off = off;
     off += T2_STAGES * STAGE_BYTES;
     pl.bias_base = off;
@@ -489,6 +503,8 @@ bool t2_make_plan(int cg, int n_linear, const int* widths, T2Plan& pl) {
     off += t2_round_up(8 * T_COUNT + 8, 16);
     pl.red_off = off;
     off += 4 * HB_NMOM * 8;
+    pl.phc_off = off;
+    off += 2 * HB_MAX_LINEAR * 32;
     pl.total = off;
     return (size_t)pl.total + 1024 <= SMEM_LIMIT;
 }
@@ -539,13 +555,13 @@ int hb_tc2_plan_cg(int n_linear, const int* widths, int force_cg) {
 }
 
 // Packed operand image of this kernel.  Per layer [rank 0 | rank 1] blocks (one block for cg = 1):
+//   Row order of every layer but the last: local row h (hw/cg) + i of rank r is neuron h hw + r (hw/cg) + i, hw = npad/2:
+//     the rows of N-half 0 first, then those of N-half 1 (a cta_group::2 MMA of N = hw takes hw/2 rows from each CTA).
 //   layer 0 (K = 16, no swizzle): per 8-row group 256 bytes = K chunk 0 of the 8 rows (8 x 16 B), then K chunk 1; W_0 is
-//     carried twice (columns 0..5 meet the hi parts of the inputs, 6..11 the lo parts), b_hi, b_lo in columns 12, 13;
-//     rank r holds the rows of neurons [r npad/cg, (r+1) npad/cg).
+//     carried twice (columns 0..5 meet the hi parts of the inputs, 6..11 the lo parts), b_hi, b_lo in columns 12, 13.
 //   hidden layer l: per 64-wide K slab, per rank npad/cg rows of 128 bytes (K-major, 128-byte swizzle: the 16-byte chunk
-//     c of local row i sits at chunk position c ^ (i mod 8)); local row h (hw/cg) + i of rank r is neuron
-//     h hw + r (hw/cg) + i: the rows of N-half 0 first, then those of N-half 1 (a cta_group::2 MMA of N = hw takes hw/2
-//     rows from each CTA).  Behind the slabs the bias block (K = 16 operand as layer 0, same row order).
+//     c of local row i sits at chunk position c ^ (i mod 8)).  Behind the slabs the bias block (K = 16 operand as
+//     layer 0, same row order).
 //   last layer: per K slab, per rank 16/cg rows.
 size_t hb_tc2_pack_weights(int prec, int cg, int n_linear, const int* widths, const float* const* W, const float* const* B,
                            void* dst, long long* off_bytes, int* kpad, int* npad) {
