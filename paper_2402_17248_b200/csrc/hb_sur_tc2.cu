@@ -13,11 +13,11 @@
 // M128 x N128 x K16 against 131 for N256, profiles/r2_mma_rate.md).  While half 1's MMAs run, the epilogue warps turn
 // half 0's accumulator into K-half 0 of the next operand (written to the OTHER operand region: nothing is held in
 // registers, nothing waits for the layer to end); the next layer's half 0 starts on that K-half the moment half 1's
-// MMAs are through, and meets K-half 1 (converted from half 1 meanwhile) eight K steps later.  The last layer (N = 16)
-// takes no accumulator of its own: its 16 output columns go to the tail [112,128) of the operand region it does not
-// read, which is dead by then.  So both halves of the NEXT tile's layer 0 are issued around it (half 0 before, half 1
-// right behind it) and the tensor pipe never waits for the output to be read: only the epilogue of that half 1, which
-// writes the next operand's K-half 1 over those columns, waits for the IO warps -- long after they are through.
+// MMAs are through, and meets K-half 1 (converted from half 1 meanwhile) eight K steps later.  At the tile boundary the
+// next tile's layer 0 (half 0) is issued right behind the last hidden layer, before the last layer (N = 16, into D[1]);
+// only its half 1 waits for the output read.  (Measured and dropped: the 16 output columns in the dead operand region
+// instead of D[1], so that no MMA waits for the output read: 2.40 ms against 2.20; and the next tile's first operand
+// half converted under the last hidden layer with its K-half 0 issued before the last layer: 2.42 ms.)
 // Events.  The hidden accumulators of a CTA form one sequence e = 0, 1, 2, ...: tile t, layer l <= L-2, half h is
 // e = (t (L-1) + l) * 2 + h; it lives in D[h], signals DH_FULL[h], is read (DH_FREE[h]) and converted into K-half h of
 // operand region (t (L-1) + l) & 1 (A_FULL[h]).
@@ -34,10 +34,6 @@ constexpr int T2_THREADS = 448;
 constexpr int T2_STAGES = 2;          // input staging ring (tiles)
 constexpr uint32_t T2_A = 0;          // operand regions A[0], A[1]: 128 columns each
 constexpr uint32_t T2_D = 256;        // accumulators D[0], D[1]: 128 columns each
-constexpr uint32_t T2_OUT = 112;      // the last layer's 16 output columns: the tail of the operand region it does NOT read
-#ifndef HB_T2_OUT_IN_D1
-#define HB_T2_OUT_IN_D1 1             // experiment: 1 = outputs in D[1], the next tile's layer-0 half 1 waits for the IO warps
-#endif
 
 enum : int {
     T_W = 0,              // weights resident (local)
@@ -48,7 +44,7 @@ enum : int {
     T_DH_FREE = 9,        // [2] D[h] read by the epilogue warps (leader; 8 warps x CG)
     T_A_FULL = 11,        // [2] K-half h of the next operand written (leader; 8 warps x CG)
     T_D_LAST = 13,        // accumulator of the last layer complete (both CTAs, MMA commit)
-    T_OUT_READ = 14,      // last layer's accumulator read by the IO warps (local: 4 IO warps)
+    T_OUT_READ = 14,      // last layer's accumulator read by the IO warps (leader; 4 IO warps x CG)
     T_COUNT = 15
 };
 
@@ -163,7 +159,7 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
             mbar_init(bar(T_A_FULL + s), 8 * CG);
         }
         mbar_init(bar(T_D_LAST), 1);
-        mbar_init(bar(T_OUT_READ), HB_T2_OUT_IN_D1 ? 4 * CG : 4);
+        mbar_init(bar(T_OUT_READ), 4 * CG);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == MMA_WARP) {
@@ -252,13 +248,15 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
             const uint32_t idesc0 = idesc_base | ((uint32_t)(pl.hw[0] >> 3) << 17);
             // layer 0 of tile t, half h: one K = 16 MMA from the compact operand (bias inside W_0)
             auto issue_l0 = [&](uint32_t t, int h) {
-                if (HB_T2_OUT_IN_D1 && h == 1) {
+                if (h == 1) {
+                    // D[1] holds the previous tile's outputs until the IO warps have read them (the last layer, not the
+                    // epilogue, wrote it last: its DH_FREE phase was consumed by that layer)
                     if (t > 0) mbar_wait<true>(bar(T_OUT_READ), (t - 1) & 1);
                     else used |= 2u;
                 } else {
-                    claim(h);
+                    claim(0);
+                    mbar_wait<true>(bar(T_A0_FULL + (int)(t & 1)), (t >> 1) & 1);
                 }
-                if (h == 0) mbar_wait<true>(bar(T_A0_FULL + (int)(t & 1)), (t >> 1) & 1);
                 tc_fence_after();
                 if (issuer) {
                     umma<CG, false>(dbase + 128u * (uint32_t)h, make_desc_l0(sbase + pl.a0_off + (t & 1) * A0_BYTES),
@@ -279,9 +277,7 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
                     // the last hidden event in it; the operand region its epilogue writes is dead)
                     if (last && t + 1 < nmine) issue_l0(t + 1, 0);
                     for (int h = 0; h < (last ? 1 : 2); ++h) {
-                        // the last layer's 16 columns go to the tail of the operand region it does not read
-                        const uint32_t d_tmem = last ? (HB_T2_OUT_IN_D1 ? dbase + 128u : tmem_base + T2_A + 128u * ((lay & 1u) ^ 1u) + T2_OUT)
-                                                     : dbase + 128u * (uint32_t)h;
+                        const uint32_t d_tmem = dbase + 128u * (uint32_t)(last ? 1 : h);   // the last layer's 16 columns go to D[1]
                         const uint64_t bd = ((uint64_t)c0.y << 32) | c0.x, wbd = ((uint64_t)c0.w << 32) | c0.z;
                         const uint32_t idesc = c1.x;
                         const uint64_t bd_step = c1.y;
@@ -290,22 +286,42 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
                         const int nxt = (h == 0 && !last) ? 2 * l + 1 : (l + 1 < L ? 2 * (l + 1) : 2);
                         c0 = phc[2 * nxt];
                         c1 = phc[2 * nxt + 1];
-                        if (!last) claim(h);
-                        else if (HB_T2_OUT_IN_D1) claim(1);
+                        // What this phase waits for: its accumulator read by the epilogue (DH_FREE), and, for half 0 (and
+                        // the last layer), the two K-halves of the operand the epilogue of layer l-1 is writing (A_FULL).
+                        // Every wait on an mbarrier costs this warp ~165 cycles even when the phase completed long ago, so
+                        // all three are probed at once first (lane i tests barrier i; test_wait does not suspend) and only
+                        // what is really missing is awaited.
+                        const int dh = last ? 1 : h;
+                        const bool need_free = ((used >> dh) & 1u) != 0u, fresh = h == 0;
+                        used |= 1u << dh;
+                        uint32_t pbar = bar(T_DH_FREE + dh), ppar = (ph_free >> dh) & 1u;
+                        if (lane == 1) { pbar = bar(T_A_FULL); ppar = ph_a & 1u; }
+                        if (lane == 2) { pbar = bar(T_A_FULL + 1); ppar = (ph_a >> 1) & 1u; }
+                        const bool probe = lane == 0 ? need_free : (lane < 3 && fresh);
+                        const uint32_t have = __ballot_sync(0xffffffffu, probe && mbar_test(pbar, ppar) != 0u);
+                        if (need_free) {
+                            if (!(have & 1u)) mbar_wait<true>(bar(T_DH_FREE + dh), (ph_free >> dh) & 1u);
+                            ph_free ^= 1u << dh;
+                        }
                         tc_fence_after();
                         // hidden layer: the bias goes in first, as one K = 16 MMA of the tile's layer-0 operand (ones in
                         // columns 12, 13) with this half's bias block (b_hi, b_lo in columns 12, 13, zeros elsewhere)
                         if (!last && issuer) umma<CG, false>(d_tmem, a0d, wbd, idesc);
-                        if (h == 0) {
+                        if (fresh) {
                             // the operand is being written by the epilogue of layer l-1: K-half by K-half
-                            mbar_wait<true>(bar(T_A_FULL), ph_a & 1u);
-                            ph_a ^= 1u;
-                            tc_fence_after();
-                            if (issuer) t2_issue_ksteps<CG>(0, ksteps, d_tmem, a_tmem, bd, bd_step, idesc, last);
-                            mbar_wait<true>(bar(T_A_FULL + 1), (ph_a >> 1) & 1u);
-                            ph_a ^= 2u;
-                            tc_fence_after();
-                            if (issuer) t2_issue_ksteps<CG>(1, ksteps, d_tmem, a_tmem, bd, bd_step, idesc, false);
+                            if ((have & 6u) == 6u) {
+                                if (issuer) t2_issue_ksteps<CG>(2, ksteps, d_tmem, a_tmem, bd, bd_step, idesc, last);
+                            } else {
+                                if (!(have & 2u)) {
+                                    mbar_wait<true>(bar(T_A_FULL), ph_a & 1u);
+                                    tc_fence_after();
+                                }
+                                if (issuer) t2_issue_ksteps<CG>(0, ksteps, d_tmem, a_tmem, bd, bd_step, idesc, last);
+                                mbar_wait<true>(bar(T_A_FULL + 1), (ph_a >> 1) & 1u);
+                                tc_fence_after();
+                                if (issuer) t2_issue_ksteps<CG>(1, ksteps, d_tmem, a_tmem, bd, bd_step, idesc, false);
+                            }
+                            ph_a ^= 3u;
                         } else if (issuer) {
                             t2_issue_ksteps<CG>(2, ksteps, d_tmem, a_tmem, bd, bd_step, idesc, false);
                         }
@@ -322,7 +338,7 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
         const int wq = warp & 3;                 // TMEM lane quarter this warp may access
         const int row = 32 * wq + lane;          // tile row = TMEM lane = particle within the tile
         const uint32_t a0_row = sbase + pl.a0_off + (uint32_t)(row >> 3) * 256 + (uint32_t)(row & 7) * 16;
-        const uint32_t tout = tmem_base + ((uint32_t)(32 * wq) << 16) + T2_A + T2_OUT;
+        const uint32_t tout = tmem_base + ((uint32_t)(32 * wq) << 16) + T2_D + 128u;     // D[1], columns 0..7
         const float* bl = bias_s;
         HbMomAcc acc;
         acc.clear();
@@ -377,15 +393,11 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
             tc_fence_after();
             uint32_t r[8];
             // the last layer read operand region (t (L-1) + L-2) & 1 and wrote the tail of the other one
-            if (HB_T2_OUT_IN_D1) tmem_ld8(tmem_base + ((uint32_t)(32 * wq) << 16) + T2_D + 128u, r);
-            else tmem_ld8(tout + 128u * (((t * (uint32_t)(L - 1) + (uint32_t)(L - 2)) & 1u) ^ 1u), r);
+            tmem_ld8(tout, r);
             tmem_ld_wait();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) {
-                if (HB_T2_OUT_IN_D1) mbar_arrive_cluster(bar(T_OUT_READ), 0);
-                else mbar_arrive_local(bar(T_OUT_READ));
-            }
+            if (lane == 0) mbar_arrive_cluster(bar(T_OUT_READ), 0);
             if (valid) {
                 float w[6];
 #pragma unroll
@@ -407,7 +419,7 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
         const uint32_t tlane = tmem_base + ((uint32_t)(32 * wq) << 16);
         const uint32_t nev = nmine * (uint32_t)(L - 1) * 2u;
         uint32_t ph_full = 0;                     // bit h: parity of the next completion of DH_FULL[h]
-        uint32_t lay = 0, tile = 0;               // t (L-1) + l of the event; t
+        uint32_t lay = 0;                         // t (L-1) + l of the event
         int l = 0;
         auto arrive = [&](int b) {
             __syncwarp();
@@ -437,12 +449,6 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
             if (nch > 1) t2_convert<ACT, F16, 1>(r, slope);
             if (nch > 2) t2_convert<ACT, F16, 2>(r, slope);
             if (nch > 3) t2_convert<ACT, F16, 3>(r, slope);
-            // K-half 1 of a tile's first operand goes over the previous tile's output columns: the IO warps of this CTA
-            // must have read them (they did long ago: the wait is for correctness, it does not stall)
-            if (!HB_T2_OUT_IN_D1 && l == 0 && h == 1 && tile > 0) {
-                mbar_wait<true>(bar(T_OUT_READ), (tile - 1u) & 1u);
-                tc_fence_after();
-            }
             if (nch > 0) tmem_st8o<0>(dst, r);
             if (nch > 1) tmem_st8o<8>(dst + 8u, r);
             if (nch > 2) tmem_st8o<16>(dst + 16u, r);
@@ -452,7 +458,7 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
             arrive(T_A_FULL + h);
             if (h == 1) {
                 ++lay;
-                if (++l == L - 1) { l = 0; ++tile; }
+                if (++l == L - 1) l = 0;
             }
         }
     }
