@@ -36,13 +36,20 @@ import workloads as wl  # noqa: E402
 
 METRIC = "particle-element pushes/s & surrogate particles/s at 1e7; % of HBM/tensor peak"
 L2_FLUSH_BYTES = 256 << 20
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch, from the `ncu --set full` captures summarised in
-# profiles/r1_kernels_v2.md (same commands as there; N = 1e7).  Algorithmic bytes are 480e6 per launch in all three.
-NCU_TRAFFIC = {
-    ("hb_sur_tc_kernel", 10_000_000): 421.3e6,
-    ("hb_sur_tcs_kernel", 10_000_000): 429.0e6,
-    ("hb_run_composed_kernel", 10_000_000): 422.8e6,
-}
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+
+
+def ncu_traffic(kernel, n):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of `kernel` at n particles, from the `ncu --set full`
+    captures under profiles/ (profiles/ncu_traffic.json lists them: kernel, n, bytes, capture file, command); None if
+    there is no capture of that kernel at that size"""
+    try:
+        for e in json.load(open(TRAFFIC_FILE))["entries"]:
+            if e["kernel"] == kernel and int(e["n"]) == int(n):
+                return float(e["dram_bytes"])
+    except Exception:
+        pass
+    return None
 
 
 def peaks():
@@ -55,7 +62,7 @@ def peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks line of B200_PROFILING.md, sampled every 20 ms during the timed region."""
+    """nvidia-smi clocks line of B200_PROFILING.md, sampled every 5 ms during the timed region."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -65,7 +72,7 @@ class ClockSampler:
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                                       "--format=csv,noheader,nounits", "-lms", "20"], stdout=self.f,
+                                       "--format=csv,noheader,nounits", "-lms", "5"], stdout=self.f,
                                       stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
@@ -246,14 +253,29 @@ def kernel_extras(torch, hb, args, pk, flush, dev):
     n = args.n or 10_000_000
     reps = 10
 
-    def measure(desc, xh, label, with_moments, steps=reps, run_mode="composed", prec=None):
+    PARITY_N = 100_000
+
+    def measure(desc, xh, label, with_moments, steps=reps, run_mode="composed", prec=None, parity=False):
+        """mean ms per step, per-segment ms [, max |gpu - oracle| / std(oracle) per coordinate over the first PARITY_N
+        particles of the last timed step]"""
         lat = hb.Lattice.from_description(desc, run_mode=run_mode, device=dev.index, prec=prec)
         pristine = torch.from_numpy(xh).to(dev)
         work = torch.empty_like(pristine)
         tot, seg, _ = timed_steps(torch, hb, lat, pristine, work, steps, 3, flush, with_moments=with_moments, segtimes=True)
         lat.close()
+        par = None
+        if parity:
+            import oracle
+            m = min(PARITY_N, xh.shape[1])
+            d2 = dict(desc)
+            if prec is not None:      # the oracle ignores the precision; keep the description as it is
+                pass
+            ref, _ = oracle.push(d2, np.ascontiguousarray(xh[:, :m]))
+            got = work[:, :m].cpu().numpy().astype(np.float64)
+            err = np.max(np.abs(got - ref), axis=1) / ref.std(axis=1)
+            par = {"max_abs_err_over_std": float(err.max()), "particles": int(m)}
         del pristine, work
-        return tot / steps, seg
+        return (tot / steps, seg, par) if parity else (tot / steps, seg)
 
     # (a) conventional run kernel, C2 lattice (500 elements) at N = 1e7: composed (HBM-bound)
     desc2, x2 = wl.config2(n=n)
@@ -264,7 +286,8 @@ def kernel_extras(torch, hb, args, pk, flush, dev):
         out.append({"kernel": "hb_run_composed_kernel" + ("<moments>" if mom else ""), "workload": "C2 lattice (500 elements, one run), N=%d" % n,
                     "ms": k_ms, "particle_element_pushes_per_s": 500.0 * n / (k_ms * 1e-3),
                     "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                                 "frac": gbs / pk["hbm_gbs"], "traffic": None, "peak_source": pk["source"]}})
+                                 "frac": gbs / pk["hbm_gbs"], "traffic": ncu_traffic("hb_run_composed_kernel", n),
+                                 "peak_source": pk["source"]}})
     # same kernel at N = 1e8 (2.4 GB per bunch, 4.8 GB of traffic per launch): launch + event overhead (~6 us) no
     # longer visible beside 730 us of streaming
     if not args.n:
@@ -308,29 +331,32 @@ def kernel_extras(torch, hb, args, pk, flush, dev):
         other = "bf16" if args.prec == "f16" else "f16"
         desc3, x3 = wl.config3(prec=other, n=n)
         fl = wl.flops_per_particle(desc3["elements"][0]["widths"])
-        ms, seg = measure(desc3, x3, "sur", True)
+        ms, seg, par = measure(desc3, x3, "sur", True, parity=True)
         k_ms = float(seg[0])
         tf = fl * n / (k_ms * 1e-3) / 1e12
-        out.append({"kernel": "hb_sur_tc_kernel<%s>" % other, "workload": "C3, N=%d" % n, "ms": k_ms,
-                    "particle_inferences_per_s": n / (k_ms * 1e-3),
+        out.append({"kernel": "hb_sur_tc2_kernel<%s>" % other, "workload": "C3, N=%d" % n, "ms": k_ms,
+                    "particle_inferences_per_s": n / (k_ms * 1e-3), "parity": par,
+                    "parity_bound": "2e-2 (BASELINE.json); plain bf16 operands are outside it: reported, not conforming (DESIGN.md 6.5)",
                     "roofline": {"bound": "tensor", "achieved": tf, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
-                                 "frac": tf / pk["bf16_tflops"], "traffic": None, "peak_source": pk["source"]}})
-        ms, seg = measure(desc3, x3, "sur", True, steps=5, prec="tf32")
+                                 "frac": tf / pk["bf16_tflops"], "traffic": ncu_traffic("hb_sur_tc2_kernel", n),
+                                 "peak_source": pk["source"]}})
+        ms, seg, par = measure(desc3, x3, "sur", True, steps=5, prec="tf32", parity=True)
         k_ms = float(seg[0])
         tf = fl * n / (k_ms * 1e-3) / 1e12
         out.append({"kernel": "hb_sur_tcs_kernel<tf32>", "workload": "C3, N=%d" % n, "ms": k_ms,
-                    "particle_inferences_per_s": n / (k_ms * 1e-3),
+                    "particle_inferences_per_s": n / (k_ms * 1e-3), "parity": par, "parity_bound": "2e-2",
                     "roofline": {"bound": "tensor", "achieved": tf, "peak": 0.5 * pk["bf16_tflops"], "unit": "TFLOP/s",
                                  "frac": tf / (0.5 * pk["bf16_tflops"]), "traffic": None,
                                  "peak_source": pk["source"] + " bf16 x 0.5 (nominal tf32 : bf16 ratio)"}})
-        ms, seg = measure(desc3, x3, "sur", True, steps=2, prec="fp32")
+        ms, seg, par = measure(desc3, x3, "sur", True, steps=2, prec="fp32", parity=True)
         k_ms = float(seg[0])
         fma_peak = 148 * 128 * 1.965e9 / 1e12
         ach = 0.5 * fl * n / (k_ms * 1e-3) / 1e12
         out.append({"kernel": "hb_sur_fp32_kernel", "workload": "C3, N=%d" % n, "ms": k_ms,
-                    "particle_inferences_per_s": n / (k_ms * 1e-3),
+                    "particle_inferences_per_s": n / (k_ms * 1e-3), "parity": par, "parity_bound": "1e-5",
                     "roofline": {"bound": "alu", "achieved": ach, "peak": fma_peak, "unit": "TFMA/s (fp32)",
-                                 "frac": ach / fma_peak, "traffic": None}})
+                                 "frac": ach / fma_peak, "traffic": None,
+                                 "peak_source": "derived: 148 SMs x 128 fp32 lanes x 1.965 GHz (datasheet unit counts, not measured)"}})
         del x3
         # (b2) one C5 stage (6-512^4-6 tanh, weights streamed from L2) at N = 1e7
         desc5, _ = wl.config5(prec=p16, particles=False)
@@ -344,7 +370,7 @@ def kernel_extras(torch, hb, args, pk, flush, dev):
                     "particle_inferences_per_s": n / (k_ms * 1e-3),
                     "roofline": {"bound": "tensor", "achieved": tf, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
                                  "frac": tf / pk["bf16_tflops"], "frac_of_sustained": tf / pk["bf16_tflops_sustained"],
-                                 "traffic": None, "peak_source": pk["source"]}})
+                                 "traffic": ncu_traffic("hb_sur_tcs_kernel", n), "peak_source": pk["source"]}})
         del x5
         # (b3) the paper's own network shapes on the layered kernel, one stage at N = 1e7; the paper's timings
         # (P:199, 1 x A100, PyTorch) are context, not the target
@@ -377,6 +403,53 @@ def kernel_extras(torch, hb, args, pk, flush, dev):
                     "surrogate_tflops": fl4 * n / (sur_ms * 1e-3) / 1e12, "run_gbs": 48.0 * n / (run_ms * 1e-3) / 1e9,
                     "roofline": {"bound": "alu", "achieved": xu_ach, "peak": xu_peak, "unit": "Ttanh/s (MUFU, surrogate kernel)",
                                  "frac": xu_ach / xu_peak, "traffic": None}})
+        del x4
+        # (d) NEXT-4: K candidate settings of one transport gap over the same resident bunch (hb_push_candidates): one
+        # pass over the particles whatever K is
+        gap = wl.lattice([wl.drift(0.5), wl.plens(0.05, 10.0), wl.drift(0.45), wl.monitor()], kinetic_MeV=8000.0)
+        latg = hb.Lattice.from_description(gap, device=dev.index)
+        xg = torch.from_numpy(wl.gaussian_bunch(n, 6)).to(dev)
+        K = 256
+        rng = np.random.default_rng(1)
+        d0 = rng.uniform(0.05, 0.9, K)
+        length = np.stack([d0, np.full(K, 0.05), 0.95 - d0], axis=1)
+        param = np.stack([np.zeros(K), rng.uniform(0.0, 40.0, K), np.zeros(K)], axis=1)
+        recs = torch.empty((K, 27), dtype=torch.float64, device=dev)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+        for it in range(3 + reps):
+            flush.fill_(it & 0xff)
+            if it >= 3:
+                evs[it - 3][0].record()
+            latg.push_candidates(xg, [0, 1, 2], length, param, out=recs)
+            if it >= 3:
+                evs[it - 3][1].record()
+        torch.cuda.synchronize()
+        c_ms = sum(a.elapsed_time(b) for a, b in evs) / reps
+        latg.close()
+        del xg
+        gbs = 24.0 * n / (c_ms * 1e-3) / 1e9
+        out.append({"kernel": "hb_push_candidates (moment partials + finalize + hb_candidates_kernel)",
+                    "workload": "%d candidate settings of a drift / plasma lens / drift gap, N=%d, bunch read once" % (K, n),
+                    "ms": c_ms, "candidate_evaluations_per_s": K / (c_ms * 1e-3),
+                    "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s (read only: 24 B per particle)",
+                                 "frac": gbs / pk["hbm_gbs"], "traffic": None, "peak_source": pk["source"] + " (copy bandwidth)"}})
+        # (e) C5 as BASELINE.json specifies it: N = 1e8 (2.4 GB bunch), 9 streamed-weights stages + 8 runs + 17 monitors
+        if not args.n:
+            desc5f, x5f = wl.config5(prec=p16, n=100_000_000)
+            ms, seg = measure(desc5f, x5f, "c5", True, steps=2)
+            kinds5 = segment_kinds(desc5f)
+            sur5 = float(np.mean([t for t, k in zip(seg, kinds5) if k == "sur"]))
+            run5 = float(np.mean([t for t, k in zip(seg, kinds5) if k == "run"]))
+            nb = x5f.shape[1]
+            tf = fl5 * nb / (sur5 * 1e-3) / 1e12
+            out.append({"kernel": "C5 whole push (9 x hb_sur_tcs_kernel + 8 x hb_run_composed_kernel + 17 finalizes)",
+                        "workload": "C5 as specified: N=%d, 9 x 6-512^4-6 tanh %s + 8 x 10 FODO cells, 17 monitors" % (nb, p16),
+                        "ms": ms, "particles_per_s": nb / (ms * 1e-3), "surrogate_inferences_per_s": 9.0 * nb / (ms * 1e-3),
+                        "surrogate_ms": sur5, "run_ms": run5, "run_gbs": 48.0 * nb / (run5 * 1e-3) / 1e9,
+                        "roofline": {"bound": "tensor", "achieved": tf, "peak": pk["bf16_tflops"], "unit": "TFLOP/s (one stage)",
+                                     "frac": tf / pk["bf16_tflops"], "frac_of_sustained": tf / pk["bf16_tflops_sustained"],
+                                     "traffic": None, "peak_source": pk["source"]}})
+            del x5f
     return out
 
 
@@ -482,7 +555,8 @@ def main():
         per = flops / max(n_sur, 1)
         ach = per * n / (dom_ms * 1e-3) / 1e12
         widest = max(max(e["widths"][1:-1]) for e in desc["elements"] if e["kind"] == "surrogate")
-        kname = "hb_sur_tcw_kernel" if widest > 512 else ("hb_sur_tcs_kernel" if widest > 256 else "hb_sur_tc_kernel")
+        kname = "hb_sur_tcw_kernel" if widest > 512 else ("hb_sur_tcs_kernel" if widest > 256 else
+                                                          ("hb_sur_tc2_kernel" if widest > 128 else "hb_sur_tc_kernel"))
         if args.prec == "fp32":
             # FFMA path on the CUDA cores: peak derived in DESIGN.md 6.3 (148 SMs x 128 lanes x 1.965 GHz)
             fma_peak = 148 * 128 * 1.965e9 / 1e12
@@ -498,14 +572,14 @@ def main():
                     "algorithmic_flop_per_particle": per}
         else:
             roof = {"bound": "tensor", "achieved": ach, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
-                    "frac": ach / pk["bf16_tflops"], "traffic": NCU_TRAFFIC.get((kname, n)), "kernel": kname,
+                    "frac": ach / pk["bf16_tflops"], "traffic": ncu_traffic(kname, n), "kernel": kname,
                     "kernel_ms": dom_ms, "peak_source": pk["source"] + " (burst, cuBLAS bf16; f16 and bf16 share tcgen05.mma.kind::f16 and its peak)",
                     "frac_of_sustained": ach / pk["bf16_tflops_sustained"],
                     "algorithmic_flop_per_particle": per}
     else:
         ach = 48.0 * n / (dom_ms * 1e-3) / 1e9
         roof = {"bound": "hbm", "achieved": ach, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": ach / pk["hbm_gbs"],
-                "traffic": NCU_TRAFFIC.get(("hb_run_composed_kernel", n)), "kernel": "hb_run_composed_kernel",
+                "traffic": ncu_traffic("hb_run_composed_kernel", n), "kernel": "hb_run_composed_kernel",
                 "kernel_ms": dom_ms, "peak_source": pk["source"]}
 
     # BASELINE.md holds the paper's number only for its own network shapes at N = 1e7 (P:199, 1 x A100: context)

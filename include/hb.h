@@ -197,6 +197,27 @@ hb_status hb_push_moments(hb_lattice *lat, float *x, float *px, float *y, float 
 hb_status hb_push_host(hb_lattice *lat, float *x, float *px, float *y, float *py, float *t, float *pt,
                        size_t n, double *h_moments, int chunks);
 
+/* K candidate settings of one transport section over the SAME resident bunch, in one pass (the
+ * paper optimises position and strength of the lens in every gap between stages, 2 (N_stage - 1) = 28 parameters,
+ * stage by stage with Nelder-Mead, one tracking run per evaluation -- and every evaluation of one gap starts from the
+ * same bunch).  elem_index: n_set elements (positions in the order of the add calls) of ONE run of conventional
+ * elements; length_m, param: HOST, [n_candidates][n_set], the settings of those elements for candidate k (meaning and
+ * validation as hb_lattice_set_element).  x..pt: the bunch AS IT ENTERS THAT RUN (device, n floats each, 16-byte
+ * aligned); it is only read.  The lattice itself is not changed.
+ * d_moments: DEVICE, n_candidates x 27 doubles: record k = the moments (R10, layout of hb_push_moments) of the bunch
+ * behind the run with candidate k's settings.
+ * How: every candidate's run is concatenated on the host in fp64 into one 6x6 map M_k (R5), as hb_lattice_finalize
+ * does; for a linear map the sample moments transform exactly (mean' = M mean, C' = M C M^T), so the bunch is read ONCE
+ * (24 B per particle, the fused fp64 reduction of hb_moments) whatever n_candidates is, and one thread per candidate
+ * does the 6x6 products in fp64: three launches per call.  The records are those of the exact image of the fp32 input;
+ * a push of the same setting rounds every coordinate to fp32 once more, which moves second moments by <= 1e-7 relative.
+ * Asynchronous on cuda_stream like hb_push (the host arrays are consumed before the call returns).  n = 0: NaN records.
+ * Errors: not finalized -> STATE; elements not all in one run, a multipole, invalid values -> INVALID_ARG; a run that
+ * holds a non-linear element (no composed map) -> UNSUPPORTED. */
+hb_status hb_push_candidates(hb_lattice *lat, int n_candidates, int n_set, const int *elem_index, const double *length_m,
+                             const double *param, const float *x, const float *px, const float *y, const float *py,
+                             const float *t, const float *pt, size_t n, double *d_moments, void *cuda_stream);
+
 /* Standalone moments of a bunch (R10).  pivot: 6 HOST doubles subtracted before accumulation (any
  * value near the bunch centre; NULL = zeros); the result does not depend on it beyond rounding.
  * d_out27: DEVICE, 27 doubles.  d_scratch: DEVICE scratch of hb_moments_scratch_bytes() bytes. */

@@ -22,7 +22,7 @@ EXPORTED_SYMBOLS = [
     "hb_lattice_add_surrogate",
     "hb_lattice_set_run_mode", "hb_lattice_set_centroid",
     "hb_lattice_finalize", "hb_lattice_num_monitors", "hb_lattice_num_launches", "hb_lattice_ref_bg_out",
-    "hb_push", "hb_push_moments", "hb_push_host", "hb_moments", "hb_moments_scratch_bytes", "hb_moments_merge",
+    "hb_push", "hb_push_moments", "hb_push_host", "hb_push_candidates", "hb_moments", "hb_moments_scratch_bytes", "hb_moments_merge",
     "hb_lattice_destroy",
     "hb_lattice_enable_timing", "hb_lattice_get_timing",
     "hb_status_string", "hb_last_error", "hb_version", "hb_surrogate_kernel",
@@ -84,6 +84,8 @@ def lib():
     L.hb_push.argtypes = [c_void_p] + [c_void_p] * 6 + [c_size_t, c_void_p]
     L.hb_push_moments.argtypes = [c_void_p] + [c_void_p] * 6 + [c_size_t, c_void_p, c_void_p]
     L.hb_push_host.argtypes = [c_void_p] + [c_void_p] * 6 + [c_size_t, c_void_p, c_int]
+    L.hb_push_candidates.argtypes = [c_void_p, c_int, c_int, POINTER(c_int), POINTER(c_double), POINTER(c_double)] + \
+        [c_void_p] * 6 + [c_size_t, c_void_p, c_void_p]
     L.hb_moments.argtypes = [c_void_p] * 6 + [c_size_t, POINTER(c_double), c_void_p, c_void_p, c_void_p]
     L.hb_moments_scratch_bytes.restype = c_size_t
     L.hb_moments_scratch_bytes.argtypes = []
@@ -228,6 +230,19 @@ def hb_push_moments(lat, x, px, y, py, t, pt, n: int, d_moments: int, cuda_strea
 def hb_push_host(lat, x, px, y, py, t, pt, n: int, h_moments: int, chunks: int = 4):
     """x..pt, h_moments: HOST addresses (h_moments may be 0)"""
     _check(lib().hb_push_host(lat, x, px, y, py, t, pt, n, h_moments, int(chunks)), "hb_push_host")
+
+
+def hb_push_candidates(lat, elem_index, length_m, param, x, px, y, py, t, pt, n: int, d_moments: int, cuda_stream: int = 0):
+    """length_m, param: [K][n_set] (host); x..pt, d_moments: device addresses.  Enqueues on cuda_stream and returns."""
+    idx = np.ascontiguousarray(elem_index, dtype=np.int32).reshape(-1)
+    Lm = np.ascontiguousarray(length_m, dtype=np.float64).reshape(-1, idx.size)
+    pm = np.ascontiguousarray(param, dtype=np.float64).reshape(-1, idx.size)
+    if Lm.shape != pm.shape:
+        raise ValueError("length_m and param must both be [K][n_set]")
+    pd = POINTER(c_double)
+    _check(lib().hb_push_candidates(lat, Lm.shape[0], idx.size, idx.ctypes.data_as(POINTER(c_int)), Lm.ctypes.data_as(pd),
+                                    pm.ctypes.data_as(pd), x, px, y, py, t, pt, n, d_moments, cuda_stream),
+           "hb_push_candidates")
 
 
 def hb_moments_scratch_bytes() -> int:
@@ -382,6 +397,18 @@ class Lattice:
         if out is None:
             out = torch.empty((m, 27), dtype=torch.float64, device=rows[0].device)
         hb_push_moments(self._h, *[r.data_ptr() for r in rows], n, out.data_ptr(), _stream(rows[0].device))
+        return out
+
+    def push_candidates(self, coords, elem_index, length_m, param, out=None):
+        """records [K, 27] of the bunch `coords` (as it enters the run that holds `elem_index`) behind that run, for K
+        settings (length_m, param: [K][n_set]) of those elements; the bunch and the lattice are not changed"""
+        import torch
+        rows, n = _rows(coords)
+        k = int(np.asarray(length_m).reshape(-1, len(elem_index)).shape[0])
+        if out is None:
+            out = torch.empty((k, 27), dtype=torch.float64, device=rows[0].device)
+        hb_push_candidates(self._h, elem_index, length_m, param, *[r.data_ptr() for r in rows], n, out.data_ptr(),
+                           _stream(rows[0].device))
         return out
 
     def push_host(self, host_coords, chunks=4, moments=True):

@@ -238,6 +238,10 @@ struct hb_lattice {
     double* d_host_records = nullptr;  // n_monitors x 27
     cudaStream_t host_streams[3] = {nullptr, nullptr, nullptr};   // copy-in, compute, copy-out
     cudaEvent_t host_events[9] = {};   // per slot: copied in, computed, copied out
+    // hb_push_candidates: candidate maps and the input record (allocated at the first call, grown when K grows)
+    double* d_cand_maps = nullptr;
+    double* d_cand_rec = nullptr;
+    int cand_cap = 0;
 };
 
 // Nominal centroid of the bunch behind every segment (host, fp64): the incoming centroid (default 0) through the
@@ -929,6 +933,92 @@ hb_status hb_push_host(hb_lattice* lat, float* x, float* px, float* y, float* py
         const cudaError_t e1 = cudaStreamSynchronize(sin), e2 = cudaStreamSynchronize(scmp), e3 = cudaStreamSynchronize(sout);
         if (e == cudaSuccess) e = e1 != cudaSuccess ? e1 : (e2 != cudaSuccess ? e2 : e3);
         if (e != cudaSuccess && st == HB_OK) st = fail(HB_ERR_CUDA, "hb_push_host: %s", cudaGetErrorString(e));
+    }
+    if (prev != lat->device) cudaSetDevice(prev);
+    return st;
+}
+
+hb_status hb_push_candidates(hb_lattice* lat, int n_candidates, int n_set, const int* elem_index, const double* length_m,
+                             const double* param, const float* x, const float* px, const float* y, const float* py,
+                             const float* t, const float* pt, size_t n, double* d_moments, void* stream) {
+    if (!lat) return fail(HB_ERR_INVALID_ARG, "lattice is NULL");
+    if (!lat->finalized) return fail(HB_ERR_STATE, "lattice not finalized");
+    if (n_candidates < 0 || n_candidates > 65536) return fail(HB_ERR_INVALID_ARG, "n_candidates must be 0..65536");
+    if (n_set < 1 || n_set > 64 || !elem_index || !length_m || !param) return fail(HB_ERR_INVALID_ARG, "n_set must be 1..64 with elem_index / length_m / param given");
+    if (n_candidates > 0 && !d_moments) return fail(HB_ERR_INVALID_ARG, "d_moments is NULL");
+    if ((uintptr_t)d_moments & 7u) return fail(HB_ERR_INVALID_ARG, "d_moments is not 8-byte aligned");
+    // the run that holds the elements: all of them in the same one, which must be linear
+    const Segment* run = nullptr;
+    for (const Segment& sg : lat->segs)
+        if (sg.type == SEG_RUN && elem_index[0] >= sg.e_lo && elem_index[0] < sg.e_hi) run = &sg;
+    if (!run) return fail(HB_ERR_INVALID_ARG, "element %d belongs to no run of conventional elements", elem_index[0]);
+    if (run->nonlinear) return fail(HB_ERR_UNSUPPORTED, "the run holds a non-linear element: it has no composed map to vary");
+    for (int j = 0; j < n_set; ++j) {
+        const int e = elem_index[j];
+        if (e < run->e_lo || e >= run->e_hi) return fail(HB_ERR_INVALID_ARG, "element %d is not in the run of element %d", e, elem_index[0]);
+        if (lat->elems[(size_t)e].kind == HB_ELEM_MULTIPOLE) return fail(HB_ERR_INVALID_ARG, "element %d is a multipole", e);
+    }
+    cudaStream_t s = (cudaStream_t)stream;
+    int prev = 0;
+    HB_CUDA(cudaGetDevice(&prev));
+    if (prev != lat->device) HB_CUDA(cudaSetDevice(lat->device));
+    hb_status st = HB_OK;
+    if (n_candidates > 0 && n == 0) {
+        cudaError_t e = cudaMemsetAsync(d_moments, 0xff, (size_t)n_candidates * HB_NMOM * sizeof(double), s);   // NaN records
+        if (e != cudaSuccess) st = fail(HB_ERR_CUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e));
+    } else if (n_candidates > 0) {
+        const float* arr[6] = {x, px, y, py, t, pt};
+        st = check_arrays(arr, n);
+        // candidate maps: the run's elements with the listed ones re-set, concatenated in fp64 (R5), as in finalize
+        std::vector<double> maps((size_t)n_candidates * 36);
+        for (int k = 0; k < n_candidates && st == HB_OK; ++k) {
+            Mat6 M = mat_identity();
+            for (int q = run->e_lo; q < run->e_hi; ++q) {
+                Elem el = lat->elems[(size_t)q];
+                for (int j = 0; j < n_set; ++j)
+                    if (elem_index[j] == q) {
+                        const double Lk = length_m[(size_t)k * n_set + j], pk = param[(size_t)k * n_set + j];
+                        const bool is_drift = el.kind == HB_ELEM_DRIFT;
+                        if (!std::isfinite(Lk) || (!is_drift && (!std::isfinite(pk) || Lk < 0.0)) ||
+                            (el.kind == HB_ELEM_SBEND && Lk == 0.0 && pk != 0.0)) {
+                            st = fail(HB_ERR_INVALID_ARG, "candidate %d: invalid length / parameter for element %d", k, q);
+                            break;
+                        }
+                        el.L = Lk;
+                        el.param = is_drift ? 0.0 : pk;
+                    }
+                M = mat_mul(elem_matrix(el, run->bg), M);
+            }
+            for (int r = 0; r < 6; ++r)
+                for (int c = 0; c < 6; ++c) maps[(size_t)k * 36 + r * 6 + c] = M.m[r][c];
+        }
+        if (st == HB_OK && n_candidates > lat->cand_cap) {
+            // (grown buffers: the old ones stay until destroy -- a push enqueued earlier may still read them)
+            void* d = nullptr;
+            st = upload(lat, nullptr, (size_t)n_candidates * 36 * sizeof(double), &d);
+            lat->d_cand_maps = (double*)d;
+            if (st == HB_OK && !lat->d_cand_rec) {
+                st = upload(lat, nullptr, HB_NMOM * sizeof(double), &d);
+                lat->d_cand_rec = (double*)d;
+            }
+            if (st == HB_OK) lat->cand_cap = n_candidates;
+        }
+        if (st == HB_OK) {
+            HbParticles p;
+            for (int j = 0; j < 6; ++j) p.v[j] = const_cast<float*>(arr[j]);
+            // pivot: the nominal centroid of the state that enters the run (= behind the segment before it)
+            const double* pivot = lat->centroid_in;
+            for (const Segment& sg : lat->segs) {
+                if (&sg == run) break;
+                pivot = sg.pivot;
+            }
+            int nblocks = 0;
+            cudaError_t e = cudaMemcpyAsync(lat->d_cand_maps, maps.data(), maps.size() * sizeof(double), cudaMemcpyHostToDevice, s);
+            if (e == cudaSuccess) e = hb_launch_moments_partials(p, n, pivot, lat->d_partials, &nblocks, s);
+            if (e == cudaSuccess) e = hb_launch_moments_finalize(lat->d_partials, nblocks, n, pivot, lat->d_cand_rec, s);
+            if (e == cudaSuccess) e = hb_launch_candidates(lat->d_cand_rec, lat->d_cand_maps, n_candidates, d_moments, s);
+            if (e != cudaSuccess) st = fail(HB_ERR_CUDA, "hb_push_candidates: %s", cudaGetErrorString(e));
+        }
     }
     if (prev != lat->device) cudaSetDevice(prev);
     return st;

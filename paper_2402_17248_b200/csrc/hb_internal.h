@@ -90,6 +90,8 @@ cudaError_t hb_launch_moments_finalize(const double* partials, int nblocks, size
                                        const double* pivot6_host, double* d_out27, cudaStream_t s);
 // Surrogate launchers.  prepare = true (hb_lattice_finalize, once per stage): only set the launch attributes of the
 // kernel instantiation the stage will use (dynamic shared memory), launch nothing.
+// records of K linear images of a bunch from the bunch's record: d_rec_in 27 doubles, d_maps K x 36 (row-major), d_rec_out K x 27
+cudaError_t hb_launch_candidates(const double* d_rec_in, const double* d_maps, int k_count, double* d_rec_out, cudaStream_t s);
 cudaError_t hb_launch_sur_fp32(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials,
                                int* nblocks_out, int sm_count, bool prepare, cudaStream_t s);
 cudaError_t hb_launch_sur_tc(const HbParticles& p, size_t n, const HbSurDev& sd, double* partials,

@@ -363,3 +363,46 @@ cudaError_t hb_launch_moments_finalize(const double* partials, int nblocks, size
     cudaError_t e = cudaLaunchKernelEx(&cfg, hb_moments_finalize_kernel, partials, nblocks, n, pv, d_out27);
     return e != cudaSuccess ? e : cudaGetLastError();
 }
+
+// ---------------------------------------------------------------------------------- candidate maps (NEXT-4)
+// Records of the images  M_k v  of one bunch under K linear maps, from the bunch's own record: for a linear map the mean
+// and the centred second moments transform exactly,  m' = M m,  C' = M C M^T  (sample moments, not a statistical statement),
+// so K candidate settings of a transport section cost ONE pass over the particles (24 B each, hb_moments_partials_kernel)
+// whatever K is.  One thread per candidate: 6 x 6 products in fp64.
+__global__ void hb_candidates_kernel(const double* __restrict__ rec_in, const double* __restrict__ maps, int k_count,
+                                     double* __restrict__ rec_out) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= k_count) return;
+    const double* M = maps + (size_t)k * 36;
+    double m[6], C[6][6];
+    for (int i = 0; i < 6; ++i) m[i] = rec_in[i];
+    int idx = 6;
+    for (int i = 0; i < 6; ++i)
+        for (int j = i; j < 6; ++j) { C[i][j] = rec_in[idx]; C[j][i] = rec_in[idx]; ++idx; }
+    double* out = rec_out + (size_t)k * HB_NMOM;
+    for (int i = 0; i < 6; ++i) {
+        double a = 0.0;
+        for (int j = 0; j < 6; ++j) a = fma(M[i * 6 + j], m[j], a);
+        out[i] = a;
+    }
+    double T[6][6];                        // T = M C
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) {
+            double a = 0.0;
+            for (int q = 0; q < 6; ++q) a = fma(M[i * 6 + q], C[q][j], a);
+            T[i][j] = a;
+        }
+    idx = 6;
+    for (int i = 0; i < 6; ++i)
+        for (int j = i; j < 6; ++j) {
+            double a = 0.0;
+            for (int q = 0; q < 6; ++q) a = fma(T[i][q], M[j * 6 + q], a);
+            out[idx++] = a;
+        }
+}
+
+cudaError_t hb_launch_candidates(const double* d_rec_in, const double* d_maps, int k_count, double* d_rec_out, cudaStream_t s) {
+    if (k_count <= 0) return cudaSuccess;
+    hb_candidates_kernel<<<(k_count + 63) / 64, 64, 0, s>>>(d_rec_in, d_maps, k_count, d_rec_out);
+    return cudaGetLastError();
+}

@@ -644,3 +644,66 @@ def test_num_launches_counts_what_a_push_enqueues(hb):
     lat.push_moments(c)
     assert np.array_equal(hb.to_host(c), x)            # a zero-length, zero-angle bend is the identity
     lat.close()
+
+
+# --------------------------------------------------------------------------------- NEXT-4: candidate settings in one pass
+def test_push_candidates_against_the_oracle(hb):
+    """hb_push_candidates: K settings (lens position and strength) of one transport gap over the same resident
+    bunch; every record against the oracle, which pushes the bunch element by element through every candidate gap
+    and takes the two-pass moments; and against the library's own push of that setting (which rounds to fp32)"""
+    import torch
+    gap = [wl.drift(0.3), wl.plens(0.05, 40.0), wl.drift(0.7), wl.quad(0.1, 1.2), wl.sbend(0.5, 0.02), wl.monitor()]
+    desc = wl.lattice(gap, kinetic_MeV=8000.0)
+    x = wl.gaussian_bunch(200_001, 61) + (wl.NOMINAL_SIGMA * [0.3, -0.2, 0.1, 0.4, 0.0, -0.5])[:, None].astype(np.float32)
+    rng = np.random.default_rng(12)
+    K = 37
+    d0 = rng.uniform(0.05, 0.95, K)                       # lens position: drifts d0 and 1 - d0 around it
+    kl = rng.uniform(-60.0, 80.0, K)                      # lens strength (both signs; one candidate without a lens)
+    kl[5] = 0.0
+    length = np.stack([d0, np.full(K, 0.05), 1.0 - d0], axis=1)
+    param = np.stack([np.zeros(K), kl, np.zeros(K)], axis=1)
+    lat = hb.Lattice.from_description(desc, device=0)
+    c = hb.to_device(x)
+    rec = lat.push_candidates(c, [0, 1, 2], length, param).cpu().numpy()
+    assert np.array_equal(hb.to_host(c), x)               # the bunch is only read
+    assert rec.shape == (K, 27) and np.all(np.isfinite(rec))
+    worst = 0.0
+    for k in range(K):
+        dk = wl.lattice([wl.drift(d0[k]), wl.plens(0.05, kl[k]), wl.drift(1.0 - d0[k])] + gap[3:], kinetic_MeV=8000.0)
+        _, ref = oracle.push(dk, x)
+        R = sym(ref[0]); C = sym(rec[k]); sd = np.sqrt(np.diag(R))
+        worst = max(worst, np.max(np.abs(rec[k][:6] - ref[0][:6]) / sd), np.max(np.abs(C - R) / np.outer(sd, sd)))
+    print("candidates vs oracle: worst moment error / (sigma_j sigma_k):", worst)
+    assert worst <= 1e-9
+    # the same setting through set_element + push_moments (fp32 images): 1e-6
+    for k in (0, 5, 36):
+        for j in range(3):
+            lat.set_element(j, length[k, j], param[k, j])
+        c2 = hb.to_device(x)
+        r2 = lat.push_moments(c2).cpu().numpy()[0]
+        moments_close(rec[k], r2, 1e-6)
+    # the lattice was not changed by the candidates call, K = 0 and n = 0 are legal
+    assert lat.push_candidates(c, [1], np.zeros((0, 1)), np.zeros((0, 1))).shape == (0, 27)
+    e = torch.zeros((6, 0), dtype=torch.float32, device="cuda")
+    assert bool(torch.isnan(lat.push_candidates(e, [1], [[0.05]], [[1.0]])).all())
+    lat.close()
+
+
+def test_push_candidates_errors(hb):
+    W, b = wl.make_mlp([6, 8, 6], "xavier", 1, 0)
+    z, o = np.zeros(6), np.ones(6)
+    desc = wl.lattice([wl.drift(0.5), wl.quad(0.1, 1.0), wl.surrogate([6, 8, 6], W, b, "tanh", z, o, z, o),
+                       wl.drift(0.5), wl.drift_exact(0.2), wl.monitor()])
+    lat = hb.Lattice.from_description(desc, device=0)
+    c = hb.to_device(wl.gaussian_bunch(1000, 3))
+    for idx, L, p in (([0, 3], [[0.1, 0.1]], [[0, 0]]),          # two different runs
+                      ([2], [[0.1]], [[0.0]]),                   # a surrogate stage
+                      ([1], [[-0.1]], [[1.0]]),                  # negative quadrupole length
+                      ([1], [[0.1]], [[float("nan")]])):
+        with pytest.raises(hb.HbError) as e:
+            lat.push_candidates(c, idx, L, p)
+        assert e.value.status == 1
+    with pytest.raises(hb.HbError) as e:                       # the second run holds an exact drift: no composed map
+        lat.push_candidates(c, [3], [[0.1]], [[0.0]])
+    assert e.value.status == 5
+    lat.close()
