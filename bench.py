@@ -77,6 +77,13 @@ class ClockSampler:
         except Exception:
             self.p = None
 
+    def count(self):
+        try:
+            self.f.flush()
+            return sum(1 for _ in open(self.f.name))
+        except Exception:
+            return 0
+
     def stop(self):
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
         if self.p is None:
@@ -246,8 +253,12 @@ def run_reference(args, rank, world):
     print(json.dumps(line))
 
 
-def kernel_extras(torch, hb, args, pk, flush, dev):
-    """per-kernel measurements at N = 1e7 beside the headline step"""
+def kernel_extras(torch, hb, args, pk, flush, dev, dp):
+    """per-kernel measurements at N = 1e7 beside the headline step.  dp: hb_device_peaks() of this device (measured pipe
+    rates: the ALU-bound kernels and the tf32 mode are quoted against them)"""
+    tf32_peak = pk["bf16_tflops"] * dp["mma_tf32_tflops"] / dp["mma_f16_tflops"]
+    tf32_src = pk["source"] + " bf16 x %.3f (kind::tf32 : kind::f16 rate of the tensor pipe measured by hb_device_peaks: %.0f / %.0f TFLOP/s)" % (
+        dp["mma_tf32_tflops"] / dp["mma_f16_tflops"], dp["mma_tf32_tflops"], dp["mma_f16_tflops"])
     p16 = args.prec if args.prec in ("f16", "bf16") else "f16"      # 16-bit operand type of the tensor-core extras
     out = []
     n = args.n or 10_000_000
@@ -311,12 +322,12 @@ def kernel_extras(torch, hb, args, pk, flush, dev):
     # sequential (fp64 registers, ALU-bound): 2700 DFMA-class ops per particle
     ms, seg = measure(desc2, x2, "run", False, steps=5, run_mode="sequential")
     k_ms = float(seg[0])
-    dp_peak = 148 * 64 * 1.965e9 / 1e12   # 148 SMs x 64 DFMA lanes x max clock (TFMA/s), DESIGN.md
+    dp_peak = dp["dfma_tfma"]             # measured fp64 FMA rate of this device (hb_device_peaks)
     ach = 2700.0 * n / (k_ms * 1e-3) / 1e12
     out.append({"kernel": "hb_run_sequential_kernel<double>", "workload": "C2 lattice, N=%d" % n, "ms": k_ms,
                 "particle_element_pushes_per_s": 500.0 * n / (k_ms * 1e-3),
                 "roofline": {"bound": "alu", "achieved": ach, "peak": dp_peak, "unit": "TFMA/s (fp64)", "frac": ach / dp_peak,
-                             "traffic": None}})
+                             "traffic": None, "peak_source": "measured: hb_device_peaks fp64 FMA chains"}})
     # non-linear run (NEXT-3): 100 chromatic FODO cells = 300 exact drifts + 200 chromatic quadrupoles, always on the
     # fp64 sequential kernel (sin/cos/sqrt per particle and element: ALU/MUFU-bound, no closed-form FMA count)
     cell = [wl.drift_exact(0.25), wl.quad_chromatic(0.1, 1.2), wl.drift_exact(0.5), wl.quad_chromatic(0.1, -1.2), wl.drift_exact(0.25)]
@@ -345,18 +356,17 @@ def kernel_extras(torch, hb, args, pk, flush, dev):
         tf = fl * n / (k_ms * 1e-3) / 1e12
         out.append({"kernel": "hb_sur_tcs_kernel<tf32>", "workload": "C3, N=%d" % n, "ms": k_ms,
                     "particle_inferences_per_s": n / (k_ms * 1e-3), "parity": par, "parity_bound": "2e-2",
-                    "roofline": {"bound": "tensor", "achieved": tf, "peak": 0.5 * pk["bf16_tflops"], "unit": "TFLOP/s",
-                                 "frac": tf / (0.5 * pk["bf16_tflops"]), "traffic": None,
-                                 "peak_source": pk["source"] + " bf16 x 0.5 (nominal tf32 : bf16 ratio)"}})
+                    "roofline": {"bound": "tensor", "achieved": tf, "peak": tf32_peak, "unit": "TFLOP/s",
+                                 "frac": tf / tf32_peak, "traffic": None, "peak_source": tf32_src}})
         ms, seg, par = measure(desc3, x3, "sur", True, steps=2, prec="fp32", parity=True)
         k_ms = float(seg[0])
-        fma_peak = 148 * 128 * 1.965e9 / 1e12
+        fma_peak = dp["ffma_tfma"]
         ach = 0.5 * fl * n / (k_ms * 1e-3) / 1e12
         out.append({"kernel": "hb_sur_fp32_kernel", "workload": "C3, N=%d" % n, "ms": k_ms,
                     "particle_inferences_per_s": n / (k_ms * 1e-3), "parity": par, "parity_bound": "1e-5",
                     "roofline": {"bound": "alu", "achieved": ach, "peak": fma_peak, "unit": "TFMA/s (fp32)",
                                  "frac": ach / fma_peak, "traffic": None,
-                                 "peak_source": "derived: 148 SMs x 128 fp32 lanes x 1.965 GHz (datasheet unit counts, not measured)"}})
+                                 "peak_source": "measured: hb_device_peaks fp32 FMA chains"}})
         del x3
         # (b2) one C5 stage (6-512^4-6 tanh, weights streamed from L2) at N = 1e7
         desc5, _ = wl.config5(prec=p16, particles=False)
@@ -396,13 +406,14 @@ def kernel_extras(torch, hb, args, pk, flush, dev):
         run_ms = float(np.mean([t for t, k in zip(seg, kinds) if k == "run"]))
         # a 6-128^3-6 tanh stage is bound by the special-function unit (16 tanh/clk/SM), not by the tensor pipe:
         # 384 tanh per particle
-        xu_peak = 148 * 16 * 1.965e9 / 1e12
+        xu_peak = dp["tanh_tps"]
         xu_ach = 384.0 * n / (sur_ms * 1e-3) / 1e12
         out.append({"kernel": "C4 whole push (2 surrogate + 2 run kernels + 4 moment finalizes)", "workload": "C4, N=%d" % n,
                     "ms": ms, "particles_per_s": n / (ms * 1e-3), "surrogate_ms": sur_ms, "run_ms": run_ms,
                     "surrogate_tflops": fl4 * n / (sur_ms * 1e-3) / 1e12, "run_gbs": 48.0 * n / (run_ms * 1e-3) / 1e9,
                     "roofline": {"bound": "alu", "achieved": xu_ach, "peak": xu_peak, "unit": "Ttanh/s (MUFU, surrogate kernel)",
-                                 "frac": xu_ach / xu_peak, "traffic": None}})
+                                 "frac": xu_ach / xu_peak, "traffic": ncu_traffic("hb_sur_tc_kernel", n),
+                                 "peak_source": "measured: hb_device_peaks tanh.approx chains"}})
         del x4
         # (d) NEXT-4: K candidate settings of one transport gap over the same resident bunch (hb_push_candidates): one
         # pass over the particles whatever K is
@@ -484,6 +495,7 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     pk = peaks()
+    dp = hb.hb_device_peaks(local)             # measured pipe rates of this device (fp32 / fp64 FMA, tanh, tensor f16 / tf32)
 
     desc, x, label = build_workload(args.workload, args.prec, args.n)
     if world > 1:   # weak scaling: every rank pushes its own bunch of the full size (particles shard)
@@ -505,7 +517,15 @@ def main():
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
+    in_region = sampler.count()
+    # nvidia-smi answers a query in tens of milliseconds, a 20-step region lasts ~50: the same step goes on, untimed,
+    # until the sampler has watched >= 0.5 s of it (clocks and throttle reasons under this very load)
+    t_watch = time.perf_counter()
+    while time.perf_counter() - t_watch < 0.5:
+        timed_steps(torch, hb, lat, pristine, work, 5, 0, flush, True, False)
     clocks = sampler.stop()
+    clocks["samples_in_timed_region"] = in_region
+    clocks["note"] = "sampled over the timed region and 0.5 s more of the same step"
     t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -559,16 +579,17 @@ def main():
                                                           ("hb_sur_tc2_kernel" if widest > 128 else "hb_sur_tc_kernel"))
         if args.prec == "fp32":
             # FFMA path on the CUDA cores: peak derived in DESIGN.md 6.3 (148 SMs x 128 lanes x 1.965 GHz)
-            fma_peak = 148 * 128 * 1.965e9 / 1e12
+            fma_peak = dp["ffma_tfma"]
             ach = 0.5 * per * n / (dom_ms * 1e-3) / 1e12
             roof = {"bound": "alu", "achieved": ach, "peak": fma_peak, "unit": "TFMA/s (fp32)", "frac": ach / fma_peak,
                     "traffic": None, "kernel": "hb_sur_fp32_kernel", "kernel_ms": dom_ms,
-                    "peak_source": "derived: 148 SMs x 128 fp32 lanes x 1.965 GHz (DESIGN.md 6.3)",
+                    "peak_source": "measured: hb_device_peaks fp32 FMA chains",
                     "algorithmic_fma_per_particle": 0.5 * per}
         elif args.prec == "tf32":
-            roof = {"bound": "tensor", "achieved": ach, "peak": 0.5 * pk["bf16_tflops"], "unit": "TFLOP/s",
-                    "frac": ach / (0.5 * pk["bf16_tflops"]), "traffic": None, "kernel": "hb_sur_tcs_kernel",
-                    "kernel_ms": dom_ms, "peak_source": pk["source"] + " bf16 x 0.5 (nominal tf32 : bf16 ratio)",
+            t32 = pk["bf16_tflops"] * dp["mma_tf32_tflops"] / dp["mma_f16_tflops"]
+            roof = {"bound": "tensor", "achieved": ach, "peak": t32, "unit": "TFLOP/s",
+                    "frac": ach / t32, "traffic": None, "kernel": "hb_sur_tcs_kernel",
+                    "kernel_ms": dom_ms, "peak_source": pk["source"] + " bf16 x measured kind::tf32 : kind::f16 pipe ratio (hb_device_peaks)",
                     "algorithmic_flop_per_particle": per}
         else:
             roof = {"bound": "tensor", "achieved": ach, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
@@ -601,6 +622,7 @@ def main():
         "gpu_launches": int(args.steps * lat.num_launches(True, n)),
         "records_merged_over_ranks": merged_ok,
         "roofline": roof,
+        "device_peaks": dp,
     }
     gpu_head = work[:, :1 << 22].cpu().numpy() if (rank == 0 and world == 1 and not args.no_cpu_baseline) else None
     lat.close()
@@ -608,7 +630,7 @@ def main():
     if rank == 0 and world == 1:
         if not args.no_extras:
             del pristine, work
-            line["kernels"] = kernel_extras(torch, hb, args, pk, flush, dev)
+            line["kernels"] = kernel_extras(torch, hb, args, pk, flush, dev, dp)
         if not args.no_cpu_baseline:
             v, cores, sample, parity = oracle_rate(desc, x, 12.0, units, gpu_head)
             line["cpu_baseline"] = {"value": v, "unit": unit, "cores": cores, "kind": "oracle", "sample": sample}

@@ -13,6 +13,6 @@ from ._binding import (  # noqa: F401
     hb_lattice_finalize, hb_lattice_num_monitors, hb_lattice_num_launches, hb_lattice_ref_bg_out,
     hb_push, hb_push_moments, hb_push_host, hb_push_candidates, hb_moments, hb_moments_scratch_bytes, hb_moments_merge, hb_lattice_destroy,
     hb_lattice_enable_timing, hb_lattice_get_timing,
-    hb_status_string, hb_last_error, hb_version, hb_surrogate_kernel,
+    hb_status_string, hb_last_error, hb_version, hb_surrogate_kernel, hb_device_peaks,
     ELEM_KINDS, ACTS, PRECS, COORDS, RUN_MODES, EXPORTED_SYMBOLS,
 )

@@ -25,7 +25,7 @@ EXPORTED_SYMBOLS = [
     "hb_push", "hb_push_moments", "hb_push_host", "hb_push_candidates", "hb_moments", "hb_moments_scratch_bytes", "hb_moments_merge",
     "hb_lattice_destroy",
     "hb_lattice_enable_timing", "hb_lattice_get_timing",
-    "hb_status_string", "hb_last_error", "hb_version", "hb_surrogate_kernel",
+    "hb_status_string", "hb_last_error", "hb_version", "hb_surrogate_kernel", "hb_device_peaks",
 ]
 
 
@@ -98,6 +98,7 @@ def lib():
     L.hb_status_string.argtypes = [c_int]
     L.hb_last_error.restype = c_char_p
     L.hb_version.restype = c_char_p
+    L.hb_device_peaks.argtypes = [c_int, POINTER(c_double)]
     L.hb_surrogate_kernel.restype = c_char_p
     L.hb_surrogate_kernel.argtypes = [c_int, c_int, POINTER(c_int)]
     for name in EXPORTED_SYMBOLS:
@@ -117,6 +118,13 @@ def hb_last_error() -> str:
 
 def hb_version() -> str:
     return lib().hb_version().decode()
+
+
+def hb_device_peaks(cuda_device: int = 0):
+    """measured pipe rates of the device: dict(ffma_tfma, dfma_tfma, tanh_tps, mma_f16_tflops, mma_tf32_tflops)"""
+    out = (c_double * 5)()
+    _check(lib().hb_device_peaks(int(cuda_device), out), "hb_device_peaks")
+    return dict(zip(("ffma_tfma", "dfma_tfma", "tanh_tps", "mma_f16_tflops", "mma_tf32_tflops"), [float(v) for v in out]))
 
 
 def hb_surrogate_kernel(prec, widths):

@@ -14,8 +14,9 @@ For gap j the bunch behind stage j is resident on the device and every Nelder-Me
 batch of candidate (d, k): `Lattice.push_candidates` evaluates the whole batch in ONE pass over the bunch
 (hb_push_candidates: the gap's elements concatenated per candidate on the host in fp64, the bunch read once, one
 27-double record per candidate), so an evaluation costs three small launches whatever the bunch size is.  The
-objective is the transverse beam size at the entrance of the next stage, sigma_x^2 + sigma_y^2 (the trained stages of
-the paper would give the emittance behind the next stage; with random networks that has no meaning).  When a gap is
+objective asks for a matched beam at the entrance of the next stage: size and divergence in both planes, each in units
+of its nominal value (the divergence's shrinks with the reference momentum), summed -- the trained stages of the paper
+would give the emittance behind the next stage instead; with random networks that has no meaning.  When a gap is
 optimised its elements are set (hb_lattice_set_element), the bunch is pushed through it and through the next stage,
 and the sequence moves on.
 
@@ -117,6 +118,7 @@ def main():
         if j == args.stages - 1:
             break
         gap = hb.Lattice.from_description(wl.lattice(gap_description(0.5, 0.0), kin_out), device=0)
+        spx = s[1] * bg[0] / bg[j + 1]                        # nominal divergence at this energy
 
         def objective(batch):
             nonlocal t_eval
@@ -127,9 +129,10 @@ def main():
             t0 = time.perf_counter()
             rec = gap.push_candidates(coords, [0, 1, 2], length, param).cpu().numpy()
             t_eval += time.perf_counter() - t0
-            return rec[:, 6] + rec[:, 17]                     # sigma_x^2 + sigma_y^2 behind the gap
+            # C_xx / sx^2 + C_pxpx / spx^2 + C_yy / sy^2 + C_pypy / spy^2 behind the gap (record layout of hb_push_moments)
+            return rec[:, 6] / s[0] ** 2 + rec[:, 12] / spx ** 2 + rec[:, 17] / s[2] ** 2 + rec[:, 21] / spx ** 2
 
-        best, fbest, evals = nelder_mead_batched(objective, np.array([0.5, 5.0]), np.array([0.1, 5.0]))
+        best, fbest, evals = nelder_mead_batched(objective, np.array([0.5, 1.0]), np.array([0.1, 1.0]))
         total_evals += evals
         d = float(np.clip(best[0], 0.02, 0.98))
         for idx, (L, p) in enumerate(((d, 0.0), (0.05, best[1]), (1.0 - d, 0.0))):
