@@ -6,7 +6,7 @@
 // and packs the next layer's operand in place into the buffer it came from.  The tensor pipe then idles, once per
 // layer, from "accumulator complete" until the epilogue warps have converted the first K slab (~600-900 cycles
 // against 2100 cycles of MMAs), and at the tile boundary for the whole chain last hidden layer -> convert -> last
-// layer -> output read (profiles/r2_tc_trace.md).  Here the 512 columns are cut differently:
+// layer -> output read (measured with a clock64 probe build, profiles/r2_mma_rate.md).  Here the 512 columns are cut differently:
 //     A[0] = [0,128)   A[1] = [128,256)    packed 16-bit operands (256 values in 128 columns), ping-pong per layer
 //     D[0] = [256,384) D[1] = [384,512)    fp32 accumulators of the two N-halves of the layer in flight
 // and every layer goes out as two tcgen05.mma chains of N = width/2 (an N = 128 MMA runs at full rate: 67 cycles for
