@@ -64,20 +64,22 @@ __device__ __forceinline__ uint32_t mbar_try_sleep(uint32_t bar, uint32_t parity
                  "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar), "r"(parity), "r"(200000u) : "memory");
     return ok;
 }
-// FAST: latency-critical waiters try a few times before they start reading the clock for the hang guard.
+// The report of the hang guard lives in a function of its own that is never inlined: with the printf (a call with its
+// own ABI set-up) inside the waiting loop, every wait cost 130-150 cycles even on a barrier whose phase had completed
+// long ago; with the call out of line it costs ~55 (measured with a micro-benchmark of the epilogue's steps).
+static __device__ __noinline__ void mbar_timeout(uint32_t bar, uint32_t parity) {
+    printf("hb_sur_tc: mbarrier timeout (block %d thread %d bar %u parity %u)\n", blockIdx.x, threadIdx.x, bar, parity);
+    __trap();
+}
+// FAST: latency-critical waiters poll with the plain try_wait (it suspends the thread for a short, bounded time and
+// wakes it when the phase completes); the others pass a long suspend-time hint, which costs less issue bandwidth and
+// wakes later.
 template <bool FAST>
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    if (FAST) {
-#pragma unroll 1
-        for (int i = 0; i < 16; ++i)
-            if (mbar_try(bar, parity)) return;
-    }
+    if (mbar_try(bar, parity)) return;
     const long long t0 = clock64();
-    while (!mbar_try_sleep(bar, parity)) {
-        if (clock64() - t0 > 4000000000LL) {   // ~2 s: a protocol bug must not hang the GPU
-            printf("hb_sur_tc: mbarrier timeout (block %d thread %d bar %u parity %u)\n", blockIdx.x, threadIdx.x, bar, parity);
-            __trap();
-        }
+    while (!(FAST ? mbar_try(bar, parity) : mbar_try_sleep(bar, parity))) {
+        if (clock64() - t0 > 4000000000LL) mbar_timeout(bar, parity);   // ~2 s: a protocol bug must not hang the GPU
     }
 }
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
