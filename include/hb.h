@@ -242,6 +242,22 @@ hb_status hb_moments(const float *x, const float *px, const float *y, const floa
                      void *cuda_stream);
 size_t hb_moments_scratch_bytes(void);
 
+/* hb_moments() for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same two kernels, the same record (bit-identical), with the block-partials
+ * scratch in a file-scope array of the library's device image -- 27 x 4736 doubles = 999 KB that every GPU which loads
+ * libhb.so holds until the process exits.  The call allocates and frees NOTHING (no cudaMalloc / cudaFree, no allocating
+ * library routine); the first call on a device looks the array's address up (cudaGetSymbolAddress, with that device
+ * current -- make one call before starting a capture).  Runs on the CURRENT device, on cuda_stream, asynchronously.
+ * Arguments as hb_moments(); n <= HB_MOMENTS_STATIC_MAX_N, else HB_ERR_INVALID_ARG (hb_last_error() names the limit);
+ * NULL / misaligned arrays: HB_ERR_INVALID_ARG; a device other than compute capability 10.0: HB_ERR_UNSUPPORTED.
+ * SHARED STATE: every call on a device uses the same array.  Nothing in it has to start at zero and nothing of the
+ * previous call is read (each call overwrites the rows it reads), but two calls that overlap on the GPU (different
+ * streams, no ordering between them) RACE: order them on one stream or with events. */
+#define HB_MOMENTS_STATIC_MAX_N 268435456ull /* 2^28 particles: a 6.4 GB bunch */
+hb_status hb_moments_static(const float *x, const float *px, const float *y, const float *py, const float *t,
+                            const float *pt, size_t n, const double *pivot, double *d_out27, void *cuda_stream);
+size_t hb_moments_static_max_particles(void); /* HB_MOMENTS_STATIC_MAX_N, for bindings */
+
 /* Record of the union of two disjoint particle sets from their records (HOST arithmetic, no device needed):
  * the sharded-monitor step of a distributed bunch (every rank pushes its own particles; a monitor, P:138,
  * is over all of them).  rec_a / rec_b: HOST, 27 doubles each as hb_push_moments writes them (6 means, then the

@@ -23,6 +23,7 @@ EXPORTED_SYMBOLS = [
     "hb_lattice_set_run_mode", "hb_lattice_set_centroid",
     "hb_lattice_finalize", "hb_lattice_num_monitors", "hb_lattice_num_launches", "hb_lattice_ref_bg_out",
     "hb_push", "hb_push_moments", "hb_push_host", "hb_push_candidates", "hb_moments", "hb_moments_scratch_bytes", "hb_moments_merge",
+    "hb_moments_static", "hb_moments_static_max_particles",
     "hb_lattice_destroy",
     "hb_lattice_enable_timing", "hb_lattice_get_timing",
     "hb_status_string", "hb_last_error", "hb_version", "hb_surrogate_kernel", "hb_device_peaks",
@@ -89,6 +90,9 @@ def lib():
     L.hb_moments.argtypes = [c_void_p] * 6 + [c_size_t, POINTER(c_double), c_void_p, c_void_p, c_void_p]
     L.hb_moments_scratch_bytes.restype = c_size_t
     L.hb_moments_scratch_bytes.argtypes = []
+    L.hb_moments_static.argtypes = [c_void_p] * 6 + [c_size_t, POINTER(c_double), c_void_p, c_void_p]
+    L.hb_moments_static_max_particles.restype = c_size_t
+    L.hb_moments_static_max_particles.argtypes = []
     L.hb_moments_merge.argtypes = [POINTER(c_double), ctypes.c_ulonglong, POINTER(c_double), ctypes.c_ulonglong,
                                    POINTER(c_double)]
     L.hb_lattice_destroy.argtypes = [c_void_p]
@@ -262,6 +266,18 @@ def hb_moments(x, px, y, py, t, pt, n: int, pivot, d_out27: int, d_scratch: int,
     if pivot is not None:
         pv = (c_double * 6)(*[float(v) for v in pivot])
     _check(lib().hb_moments(x, px, y, py, t, pt, n, pv, d_out27, d_scratch, cuda_stream), "hb_moments")
+
+
+def hb_moments_static_max_particles() -> int:
+    return int(lib().hb_moments_static_max_particles())
+
+
+def hb_moments_static(x, px, y, py, t, pt, n: int, pivot, d_out27: int, cuda_stream: int = 0):
+    """hb_moments with the scratch in a static array of the library's device image: allocates nothing (include/hb.h)."""
+    pv = None
+    if pivot is not None:
+        pv = (c_double * 6)(*[float(v) for v in pivot])
+    _check(lib().hb_moments_static(x, px, y, py, t, pt, n, pv, d_out27, cuda_stream), "hb_moments_static")
 
 
 def hb_moments_merge(rec_a, n_a: int, rec_b, n_b: int):
@@ -462,6 +478,15 @@ def moments(coords, pivot=None, out=None):
     if key not in _scratch:
         _scratch[key] = torch.empty(hb_moments_scratch_bytes(), dtype=torch.uint8, device=dev)
     hb_moments(*[r.data_ptr() for r in rows], n, pivot, out.data_ptr(), _scratch[key].data_ptr(), _stream(dev))
+    return out
+
+
+def moments_static(coords, out, pivot=None):
+    """As moments(), through hb_moments_static: the caller owns `out` (27 float64 on the bunch's device), the scratch is
+    the library's static device array, nothing is allocated.  Calls that overlap on the GPU race on that array."""
+    rows, n = _rows(coords)
+    dev = rows[0].device
+    hb_moments_static(*[r.data_ptr() for r in rows], n, pivot, out.data_ptr(), _stream(dev))
     return out
 
 

@@ -11,7 +11,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libhb.so")
 SOURCES = ["hb_api.cu", "hb_run.cu", "hb_sur_fp32.cu", "hb_sur_tc.cu", "hb_sur_tc2.cu", "hb_sur_tcs.cu", "hb_sur_tcw.cu",
-           "hb_peaks.cu"]
+           "hb_peaks.cu", "hb_noalloc.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"] + os.environ.get("HB_NVCC_EXTRA", "").split()

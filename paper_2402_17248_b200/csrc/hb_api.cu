@@ -284,6 +284,8 @@ static void track_pivots(hb_lattice* lat) {
     }
 }
 
+void hb_internal_set_error(const char* msg) { g_err = msg ? msg : ""; }
+
 extern "C" {
 
 const char* hb_status_string(hb_status s) {
@@ -299,6 +301,7 @@ const char* hb_status_string(hb_status s) {
 }
 
 const char* hb_last_error(void) { return g_err.c_str(); }
+
 const char* hb_version(void) { return "hb 0.1 (sm_100a)"; }
 
 const char* hb_surrogate_kernel(hb_prec prec, int n_linear, const int* widths) {

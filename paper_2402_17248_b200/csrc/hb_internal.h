@@ -83,6 +83,9 @@ cudaError_t hb_launch_run_composed(const HbParticles& p, size_t n, const HbRunMa
 cudaError_t hb_launch_run_sequential(const HbParticles& p, size_t n, const HbSeqElem* d_elems, int count,
                                      bool fp32_regs, bool nonlinear, const double* pivot6_host, double* partials,
                                      int* nblocks_out, cudaStream_t s);
+// sets the calling thread's hb_last_error() text (for entry points that live outside hb_api.cu)
+void hb_internal_set_error(const char* msg);
+
 cudaError_t hb_launch_moments_partials(const HbParticles& p, size_t n, const double* pivot6_host,
                                        double* partials, int* nblocks_out, cudaStream_t s);
 // fixed-order sum of `nblocks` partials -> 27-double record (pivot added back to the means)
