@@ -177,7 +177,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
             auto claim = [&](uint32_t x) {
                 const uint32_t v = x ? out_in1 : out_in0;
                 if (v) {
-                    mbar_wait<true>(bar(B_OUT_READ), (v - 1) & 1);
+                    mbar_spin(bar(B_OUT_READ), (v - 1) & 1);
                     if (x) out_in1 = 0u; else out_in0 = 0u;
                 }
             };
@@ -186,7 +186,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
             auto issue_l0 = [&](uint32_t t) {
                 const uint32_t x = more_than_one ? ((t * (uint32_t)(L - 1)) & 1u) : 0u;
                 claim(x);
-                mbar_wait<true>(bar(B_A0_FULL + (t & 1)), (t >> 1) & 1);
+                mbar_spin(bar(B_A0_FULL + (t & 1)), (t >> 1) & 1);
                 tc_fence_after();
                 if (issuer) {
                     umma<CG, false>(tmem_base + x * (uint32_t)pl.d_cols, make_desc_l0(sbase + pl.a0_off + (t & 1) * A0_BYTES),
@@ -237,7 +237,7 @@ hb_sur_tc_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, c
                     for (int j = 0; j < MAX_SLABS; ++j) {
                         if (j < nsl) {
                             if (j >= there) {
-                                mbar_wait<true>(bar(B_SLAB_FULL + sset + j), (ph_slab >> (sset + j)) & 1);
+                                mbar_spin(bar(B_SLAB_FULL + sset + j), (ph_slab >> (sset + j)) & 1);
                                 tc_fence_after();
                             }
                             if (issuer) {

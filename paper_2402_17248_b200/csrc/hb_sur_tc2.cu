@@ -30,24 +30,6 @@
 
 namespace {
 
-// The wait of the MMA-issuing warp: mbar_wait<true> as it was before hb_tc_common.cuh moved the hang-guard report out
-// of line.  The cheap form helps every other waiter of every kernel (this kernel's epilogue and IO warps included); for
-// this kernel's issuer it measured slower on C3 whichever of its six wait sites used it (2.45-2.51 ms against 2.21 ms):
-// the issuer then probes a phase's barriers earlier, finds fewer of them complete and issues more phases as two
-// K-halves with a blocking wait in between.  Kept as measured.
-__device__ __forceinline__ void t2_issuer_wait(uint32_t bar, uint32_t parity) {
-#pragma unroll 1
-    for (int i = 0; i < 16; ++i)
-        if (mbar_try(bar, parity)) return;
-    const long long t0 = clock64();
-    while (!mbar_try_sleep(bar, parity)) {
-        if (clock64() - t0 > 4000000000LL) {   // ~2 s: a protocol bug must not hang the GPU
-            printf("hb_sur_tc2: mbarrier timeout (block %d thread %d bar %u parity %u)\n", blockIdx.x, threadIdx.x, bar, parity);
-            __trap();
-        }
-    }
-}
-
 constexpr int T2_THREADS = 448;
 constexpr int T2_STAGES = 2;          // input staging ring (tiles)
 constexpr uint32_t T2_A = 0;          // operand regions A[0], A[1]: 128 columns each
@@ -256,7 +238,7 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
             // D[h] is written again: the epilogue warps must have read the event it holds
             auto claim = [&](int h) {
                 if ((used >> h) & 1u) {
-                    t2_issuer_wait(bar(T_DH_FREE + h), (ph_free >> h) & 1u);
+                    mbar_spin(bar(T_DH_FREE + h), (ph_free >> h) & 1u);
                     ph_free ^= 1u << h;
                 }
                 used |= 1u << h;
@@ -269,11 +251,11 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
                 if (h == 1) {
                     // D[1] holds the previous tile's outputs until the IO warps have read them (the last layer, not the
                     // epilogue, wrote it last: its DH_FREE phase was consumed by that layer)
-                    if (t > 0) t2_issuer_wait(bar(T_OUT_READ), (t - 1) & 1);
+                    if (t > 0) mbar_spin(bar(T_OUT_READ), (t - 1) & 1);
                     else used |= 2u;
                 } else {
                     claim(0);
-                    t2_issuer_wait(bar(T_A0_FULL + (int)(t & 1)), (t >> 1) & 1);
+                    mbar_spin(bar(T_A0_FULL + (int)(t & 1)), (t >> 1) & 1);
                 }
                 tc_fence_after();
                 if (issuer) {
@@ -318,7 +300,7 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
                         const bool probe = lane == 0 ? need_free : (lane < 3 && fresh);
                         const uint32_t have = __ballot_sync(0xffffffffu, probe && mbar_test(pbar, ppar) != 0u);
                         if (need_free) {
-                            if (!(have & 1u)) t2_issuer_wait(bar(T_DH_FREE + dh), (ph_free >> dh) & 1u);
+                            if (!(have & 1u)) mbar_spin(bar(T_DH_FREE + dh), (ph_free >> dh) & 1u);
                             ph_free ^= 1u << dh;
                         }
                         tc_fence_after();
@@ -331,11 +313,11 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
                                 if (issuer) t2_issue_ksteps<CG>(2, ksteps, d_tmem, a_tmem, bd, bd_step, idesc, last);
                             } else {
                                 if (!(have & 2u)) {
-                                    t2_issuer_wait(bar(T_A_FULL), ph_a & 1u);
+                                    mbar_spin(bar(T_A_FULL), ph_a & 1u);
                                     tc_fence_after();
                                 }
                                 if (issuer) t2_issue_ksteps<CG>(0, ksteps, d_tmem, a_tmem, bd, bd_step, idesc, last);
-                                t2_issuer_wait(bar(T_A_FULL + 1), (ph_a >> 1) & 1u);
+                                mbar_spin(bar(T_A_FULL + 1), (ph_a >> 1) & 1u);
                                 tc_fence_after();
                                 if (issuer) t2_issue_ksteps<CG>(1, ksteps, d_tmem, a_tmem, bd, bd_step, idesc, false);
                             }

@@ -178,7 +178,7 @@ hb_sur_tcs_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
             uint32_t it = 0;
             auto wait_block = [&]() -> uint32_t {
                 const uint32_t slot = cnt % S_RING;
-                mbar_wait<true>(bar(S_W_READY + slot), (cnt / S_RING) & 1);
+                mbar_spin(bar(S_W_READY + slot), (cnt / S_RING) & 1);
                 tc_fence_after();
                 return slot;
             };
@@ -187,7 +187,7 @@ hb_sur_tcs_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
                 ++cnt;
             };
             auto wait_slab = [&](int j) {
-                mbar_wait<true>(bar(S_SLAB_FULL + j), (ph_slab >> j) & 1);
+                mbar_spin(bar(S_SLAB_FULL + j), (ph_slab >> j) & 1);
                 ph_slab ^= 1u << j;
             };
             // slabs a layer needs before its MMA on slab s may go out.  s = 0: all of half 0's slabs -- the first
@@ -199,8 +199,8 @@ hb_sur_tcs_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
             };
             for (size_t g = cluster_id; g < ngroups; g += nclusters, ++it) {
                 // ---- layer 0: two N = nh MMAs (K = 16) from the compact operand buffers
-                if (it > 0) mbar_wait<true>(bar(S_OUT_READ), (it - 1) & 1);     // D_0[0..16) = previous outputs
-                mbar_wait<true>(bar(S_A0_FULL + (it & 1)), (it >> 1) & 1);
+                if (it > 0) mbar_spin(bar(S_OUT_READ), (it - 1) & 1);     // D_0[0..16) = previous outputs
+                mbar_spin(bar(S_A0_FULL + (it & 1)), (it >> 1) & 1);
                 {
                     const uint32_t slot = wait_block();
                     if (issuer) {

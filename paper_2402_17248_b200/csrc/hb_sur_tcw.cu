@@ -163,18 +163,18 @@ hb_sur_tcw_kernel(HbParticles p, size_t n_chunk, const __grid_constant__ HbSurDe
             uint32_t use[2] = {0, 0};                // how often D[b] has been filled so far
             uint32_t it = 0;
             for (size_t g = cluster_id; g < ngroups; g += nclusters, ++it) {
-                if (ly.first) mbar_wait<true>(bar(Q_A0_FULL + (it & 1)), (it >> 1) & 1);
-                if (ly.last && it > 0) mbar_wait<true>(bar(Q_OUT_READ), (it - 1) & 1);   // D[0][0..16) = previous outputs
+                if (ly.first) mbar_spin(bar(Q_A0_FULL + (it & 1)), (it >> 1) & 1);
+                if (ly.last && it > 0) mbar_spin(bar(Q_OUT_READ), (it - 1) & 1);   // D[0][0..16) = previous outputs
                 for (int nb = 0; nb < NB; ++nb) {
                     const uint32_t b = (uint32_t)nb & 1u;
                     const uint32_t d_tmem = tmem_base + b * 256u;
                     const uint32_t idesc = idesc_base | ((uint32_t)(blk_w(nb) >> 3) << 17);
                     // the epilogue must have read the block that filled D[b] before
-                    if (!ly.last && use[b] > 0) mbar_wait<true>(bar(Q_D_FREE + b), (use[b] - 1) & 1);
+                    if (!ly.last && use[b] > 0) mbar_spin(bar(Q_D_FREE + b), (use[b] - 1) & 1);
                     ++use[b];
                     for (int s = 0; s < KS; ++s, ++cnt) {
                         const uint32_t slot = cnt % W_RING;
-                        mbar_wait<true>(bar(Q_W_READY + slot), (cnt / W_RING) & 1);
+                        mbar_spin(bar(Q_W_READY + slot), (cnt / W_RING) & 1);
                         tc_fence_after();
                         if (issuer) {
                             const uint32_t st = sbase + pl.ring_off + slot * W_STAGE_BYTES;

@@ -64,23 +64,30 @@ __device__ __forceinline__ uint32_t mbar_try_sleep(uint32_t bar, uint32_t parity
                  "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar), "r"(parity), "r"(200000u) : "memory");
     return ok;
 }
-// The report of the hang guard lives in a function of its own that is never inlined: with the printf (a call with its
-// own ABI set-up) inside the waiting loop, every wait cost 130-150 cycles even on a barrier whose phase had completed
-// long ago; with the call out of line it costs ~55 (measured with a micro-benchmark of the epilogue's steps).
-static __device__ __noinline__ void mbar_timeout(uint32_t bar, uint32_t parity) {
-    printf("hb_sur_tc: mbarrier timeout (block %d thread %d bar %u parity %u)\n", blockIdx.x, threadIdx.x, bar, parity);
-    __trap();
-}
-// FAST: latency-critical waiters poll with the plain try_wait (it suspends the thread for a short, bounded time and
-// wakes it when the phase completes); the others pass a long suspend-time hint, which costs less issue bandwidth and
-// wakes later.
+// Guarded wait of every warp role but the MMA issuer.  FAST: latency-critical waiters poll with the plain try_wait (it
+// suspends the thread for a short, bounded time and wakes it when the phase completes); the others pass a long
+// suspend-time hint, which costs less issue bandwidth and wakes later.  The hang guard (~2 s: a protocol bug must not
+// hang the GPU) is a bare trap: a printf in the waiting loop -- or a call to a function that holds it -- cost every wait
+// 100 cycles more even when the phase had completed long ago (152 against 55 cycles, csrc/microbench/hb_epi_cost.cu),
+// and, worse, made ptxas give up the uniform datapath in whatever code surrounds the wait (see mbar_spin).
 template <bool FAST>
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     if (mbar_try(bar, parity)) return;
     const long long t0 = clock64();
     while (!(FAST ? mbar_try(bar, parity) : mbar_try_sleep(bar, parity))) {
-        if (clock64() - t0 > 4000000000LL) mbar_timeout(bar, parity);   // ~2 s: a protocol bug must not hang the GPU
+        if (clock64() - t0 > 4000000000LL) __trap();
     }
+}
+// Wait of the MMA-issuing warp: a bare spin on test_wait, no guard.
+// Why bare.  The issuing warp walks its schedule in warp-uniform control flow and feeds tcgen05.mma from UNIFORM
+// registers (descriptors, tensor-memory addresses).  ptxas keeps that arithmetic on the uniform datapath only while it can
+// prove the warp converged; a trap, a printf or a call inside a wait loop of that region makes it fall back to
+// per-thread registers plus an R2UR (and R2UR.BROADCAST / WARPSYNC) in front of every MMA: 278 R2UR instead of 34 in the
+// issuing region of hb_sur_tc2_kernel, 2.21 ms instead of 2.05 ms on C3 (profiles/r2_issuer_codegen.md).
+// Why that is safe.  Every wait of an issuer precedes MMAs and a tcgen05.commit that guarded waiters (epilogue and IO
+// warps, mbar_wait above) depend on: an issuer stuck here surfaces as THEIR timeout, and the trap ends the whole grid.
+__device__ __forceinline__ void mbar_spin(uint32_t bar, uint32_t parity) {
+    while (!mbar_test(bar, parity)) {}
 }
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
