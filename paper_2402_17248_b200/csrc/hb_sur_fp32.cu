@@ -17,6 +17,30 @@
 #define KC 16
 #define OC 64
 
+// Two fp32 FMAs per instruction (sm_100: fma.rn.f32x2, SASS FFMA2): d.lo = a.lo * b.lo + c.lo, d.hi likewise, each rounded
+// exactly as a scalar fmaf.  The register tile's outer product issues (4R)^2 / 2 of these per k step instead of (4R)^2
+// FFMA; ptxas folds the duplicated activation of pk2(a, a) into the instruction's scalar-broadcast operand (no moves).
+// Why: the scalar kernel was bound by instruction issue and operand dispatch, not by the FMA pipe (ncu: issue slots
+// 72.9 % busy, 0.34 dispatch-stall cycles per issued instruction, FMA pipe 63 %).
+__device__ __forceinline__ unsigned long long pk2(float lo, float hi) {
+    unsigned long long d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi));
+    return d;
+}
+__device__ __forceinline__ void unpk2(unsigned long long v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigned long long b, unsigned long long c) {
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ unsigned long long add2(unsigned long long a, unsigned long long b) {
+    unsigned long long d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
 // R = 1: 4 x 4 register tile, OCB = 64-wide output blocks; R = 2: 8 x 8 register tile (two float4 per operand and
 // k step: half the shared-memory wavefronts per FFMA) with OCB = 256 (one 256-thread block of 64 particles per SM, two
 // warps per scheduler at ~240 registers) or OCB = 128 (two 128-thread blocks per SM).  KCH = rows per weight slab.
@@ -32,6 +56,15 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
     const uint32_t ws_addr = (uint32_t)__cvta_generic_to_shared(Ws);
 
     const int tid = threadIdx.x;
+    // Activation rows are XOR-swizzled: the 16-byte chunk (4 particles) q of feature row f sits at chunk q ^ SWZ(f),
+    // SWZ(f) = ((f >> 2) & 3) << 1.  A k step reads ONE row (every lane the same f: a permutation, still two wavefronts
+    // per LDS.128); the store of a finished output block writes FOUR rows per quarter warp (rows 4 apart, the same
+    // chunks): unswizzled that was 16 wavefronts per STS.128 (ncu: 13.2-way store conflicts, 11 % of all shared-memory
+    // wavefronts), swizzled it is 4, the minimum for 512 bytes.
+    constexpr int SWM = TP >= 32 ? 3 : 0;
+    auto act_idx = [&](int f, int e) -> size_t {
+        return (size_t)f * TP + (size_t)(((((e >> 2) ^ (((f >> 2) & SWM) << 1)) << 2) | (e & 3)));
+    };
     // a warp = 8 particle groups x 4 output groups.  Lane bits (4,3,0) pick the particle group and bits (2,1) the
     // output group: both LDS.128 of a k step then cost two shared-memory wavefronts (with output group = lane % 4
     // the weight load took four: ncu, L1 Wavefronts Shared per instruction)
@@ -41,6 +74,9 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
     const int pl = PW == 8 ? ((lane & 1) | ((lane >> 3) << 1)) : lane / OW;
     const int og = ((tid >> 5) / (P / PW)) * OW + ol;
     const int pg = ((tid >> 5) % (P / PW)) * PW + pl;
+    // float offset of this thread's particle chunk in a row of swizzle class c (compile-time c: a register per class)
+    auto pgx = [&](int c) -> int { return 4 * (pg ^ ((c & SWM) << 1)); };
+    const int pgx_out = pgx(og);                 // ... in the rows this thread stores (class og & 3)
     HbMomAcc acc;
     if (MOM) acc.clear();
     int c = 0;                                   // running K-chunk counter (selects the weight-slab buffer)
@@ -54,7 +90,7 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
             float nin[6] = {0, 0, 0, 0, 0, 0};
             if (i < n) hb_sur_prologue(sd, p.v[0][i], p.v[1][i], p.v[2][i], p.v[3][i], p.v[4][i], p.v[5][i], nin);
 #pragma unroll
-            for (int j = 0; j < 6; ++j) actA[j * TP + tid] = nin[j];
+            for (int j = 0; j < 6; ++j) actA[act_idx(j, tid)] = nin[j];
         }
         float* in = actA;
         float* out = actB;
@@ -75,8 +111,9 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
                 const int kb = kq * KQ, ke = min(K, kb + KQ);
                 float d[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
                 __syncthreads();                                 // layer input complete
+#pragma unroll 4
                 for (int k = kb; k < ke; ++k) {
-                    const float a = in[(size_t)k * TP + pl_];
+                    const float a = in[act_idx(k, pl_)];
                     const float4 w0 = __ldg(reinterpret_cast<const float4*>(Wt + (size_t)k * npad));
                     const float4 w1 = __ldg(reinterpret_cast<const float4*>(Wt + (size_t)k * npad) + 1);
                     d[0] = fmaf(a, w0.x, d[0]); d[1] = fmaf(a, w0.y, d[1]);
@@ -93,16 +130,17 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
                         float z = 0.0f;
 #pragma unroll
                         for (int q = 0; q < NQ; ++q) z += out[(size_t)(8 + j * NQ + q) * TP + tid];
-                        if (j < nout) out[(size_t)j * TP + tid] = z + __ldg(bias + j);
+                        if (j < nout) out[act_idx(j, tid)] = z + __ldg(bias + j);
                     }
                 }
             } else
             for (int o0 = 0; o0 < npad; o0 += OCB) {
-                float tot[4 * R][4 * R], part[4 * R][4 * R];
+                // accumulators as pairs of adjacent outputs: [particle][output pair]
+                unsigned long long tot[4 * R][2 * R], part[4 * R][2 * R];
 #pragma unroll
                 for (int a = 0; a < 4 * R; ++a)
 #pragma unroll
-                    for (int b = 0; b < 4 * R; ++b) { tot[a][b] = 0.0f; part[a][b] = 0.0f; }
+                    for (int b = 0; b < 2 * R; ++b) { tot[a][b] = 0ull; part[a][b] = 0ull; }
                 // weight slab of K chunk c: global -> shared by cp.async into buffer c & 1 while chunk c - 1 is being
                 // multiplied; every thread moves PER 16-byte pieces (rows past K are not fetched and not read)
                 constexpr int RP = OCB / 4;                              // 16-byte pieces per slab row
@@ -121,9 +159,11 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
                     asm volatile("cp.async.commit_group;" ::: "memory");
                 };
                 // one k step: R float4 of the activation row, R float4 of the weight row, (4R)^2 FFMA
+                // ap = first row of a span that starts at a multiple of 16: the swizzle class of row k is (k >> 2) & 3
                 auto lda = [&](const float* ap, int k, float4 (&av)[R]) {
 #pragma unroll
-                    for (int r = 0; r < R; ++r) av[r] = *reinterpret_cast<const float4*>(ap + k * TP + r * (TP / R));
+                    for (int r = 0; r < R; ++r)
+                        av[r] = *reinterpret_cast<const float4*>(ap + k * TP + pgx(k >> 2) + r * (TP / R));
                 };
                 auto ldw = [&](const float* wp, int k, float4 (&wv)[R]) {
 #pragma unroll
@@ -135,12 +175,13 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
                         const float a4[4] = {av[ra].x, av[ra].y, av[ra].z, av[ra].w};
 #pragma unroll
                         for (int rb = 0; rb < R; ++rb) {
-                            const float w4[4] = {wv[rb].x, wv[rb].y, wv[rb].z, wv[rb].w};
+                            const unsigned long long w01 = pk2(wv[rb].x, wv[rb].y), w23 = pk2(wv[rb].z, wv[rb].w);
 #pragma unroll
-                            for (int a = 0; a < 4; ++a)
-#pragma unroll
-                                for (int b = 0; b < 4; ++b)
-                                    part[4 * ra + a][4 * rb + b] = fmaf(a4[a], w4[b], part[4 * ra + a][4 * rb + b]);
+                            for (int a = 0; a < 4; ++a) {
+                                const unsigned long long aa = pk2(a4[a], a4[a]);
+                                part[4 * ra + a][2 * rb] = fma2(aa, w01, part[4 * ra + a][2 * rb]);
+                                part[4 * ra + a][2 * rb + 1] = fma2(aa, w23, part[4 * ra + a][2 * rb + 1]);
+                            }
                         }
                     }
                 };
@@ -151,7 +192,7 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
                     asm volatile("cp.async.wait_all;" ::: "memory");
                     __syncthreads();          // slab c visible; slab c - 1 consumed by every warp; layer input complete
                     if (k0 + KCH < K) fetch(k0 + KCH, (c + 1) & 1);
-                    const float* __restrict__ ap = in + (size_t)k0 * TP + 4 * pg;
+                    const float* __restrict__ ap = in + (size_t)k0 * TP;
                     const float* __restrict__ wp = Ws + (c & 1) * (KCH * OCB) + 4 * og;
                     if (kk == KCH) {
                         // operands of step k + 1 are loaded before the FFMAs of step k (the shared-memory latency
@@ -185,7 +226,7 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
 #pragma unroll
                         for (int a = 0; a < 4 * R; ++a)
 #pragma unroll
-                            for (int b = 0; b < 4 * R; ++b) { tot[a][b] += part[a][b]; part[a][b] = 0.0f; }
+                            for (int b = 0; b < 2 * R; ++b) { tot[a][b] = add2(tot[a][b], part[a][b]); part[a][b] = 0ull; }
                     }
                 }
 #pragma unroll
@@ -199,11 +240,14 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
                             float r[4];
 #pragma unroll
                             for (int a = 0; a < 4; ++a) {
-                                const float z = tot[4 * ra + a][4 * rb + b] + b4[b];
+                                float t0, t1;
+                                unpk2(tot[4 * ra + a][2 * rb + (b >> 1)], t0, t1);
+                                const float z = ((b & 1) ? t1 : t0) + b4[b];
                                 r[a] = last ? z : hb_activate<ACT, false>(z, slope);
                             }
+                            // rows o0 + rb OCB/R + 4 og + b: swizzle class og & 3 (o0 and OCB / R are multiples of 16)
                             *reinterpret_cast<float4*>(out + (size_t)(o0 + rb * (OCB / R) + 4 * og + b) * TP +
-                                                       ra * (TP / R) + 4 * pg) = make_float4(r[0], r[1], r[2], r[3]);
+                                                       ra * (TP / R) + pgx_out) = make_float4(r[0], r[1], r[2], r[3]);
                         }
                     }
                 }
@@ -216,7 +260,7 @@ hb_sur_fp32_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd,
             if (i < n) {
                 float w[6];
 #pragma unroll
-                for (int j = 0; j < 6; ++j) w[j] = in[j * TP + tid];
+                for (int j = 0; j < 6; ++j) w[j] = in[act_idx(j, tid)];
                 float x, px, y, py, t, pt;
                 hb_sur_epilogue(sd, w, x, px, y, py, t, pt);
                 p.v[0][i] = x; p.v[1][i] = px; p.v[2][i] = y; p.v[3][i] = py; p.v[4][i] = t; p.v[5][i] = pt;
