@@ -186,3 +186,15 @@ def test_set_element_host_validation(hb):
             hb.hb_lattice_set_element(lat, *args)
         assert e.value.status == 1                       # HB_ERR_INVALID_ARG
     hb.hb_lattice_destroy(lat)
+
+
+def test_profile_traffic_table_names_existing_captures():
+    """bench.py reads roofline.traffic from profiles/ncu_traffic.json: every capture it names is committed"""
+    import json
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    with open(os.path.join(root, "profiles", "ncu_traffic.json")) as f:
+        table = json.load(f)
+    assert table["entries"]
+    for e in table["entries"]:
+        assert os.path.exists(os.path.join(root, "profiles", e["capture"])), e["capture"]
+        assert e["dram_bytes"] > 0 and e["n"] > 0 and e["kernel"].startswith("hb_")
