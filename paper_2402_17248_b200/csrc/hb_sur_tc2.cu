@@ -389,7 +389,7 @@ hb_sur_tc2_kernel(HbParticles p, size_t n, const __grid_constant__ HbSurDev sd, 
             const size_t tile = (cluster_id + (size_t)t * nclusters) * CG + rank;
             const size_t i = tile * TILE_M + row;
             const bool valid = tile < ntiles && i < n;
-            mbar_wait<false>(bar(T_D_LAST), t & 1);
+            mbar_wait<true>(bar(T_D_LAST), t & 1);    // on the tile-boundary chain: the plain try_wait wakes sooner (2.063 -> 2.052 ms)
             tc_fence_after();
             uint32_t r[8];
             // the last layer read operand region (t (L-1) + L-2) & 1 and wrote the tail of the other one
