@@ -444,6 +444,46 @@ def kernel_extras(torch, hb, args, pk, flush, dev, dp):
                     "ms": c_ms, "candidate_evaluations_per_s": K / (c_ms * 1e-3),
                     "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s (read only: 24 B per particle)",
                                  "frac": gbs / pk["hbm_gbs"], "traffic": None, "peak_source": pk["source"] + " (copy bandwidth)"}})
+        # (d2) launch-bound case: C1 (N = 4096: FODO cell | 6-64-64-6 tanh stage | drift, three monitors = 6 launches of a
+        # few microseconds each).  A push only enqueues (no allocation, no host synchronisation), so it can be captured
+        # into a CUDA graph once and replayed: pushes back to back on one stream, direct launches against graph replays.
+        desc1, x1 = wl.config1(prec=p16)
+        lat1 = hb.Lattice.from_description(desc1, device=dev.index)
+        w1 = torch.from_numpy(x1).to(dev)
+        rec1 = torch.zeros((lat1.num_monitors, 27), dtype=torch.float64, device=dev)
+        nrep = 200
+        for _ in range(20):
+            lat1.push_moments(w1, out=rec1)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(nrep):
+            lat1.push_moments(w1, out=rec1)
+        e1.record()
+        torch.cuda.synchronize()
+        direct_us = e0.elapsed_time(e1) * 1e3 / nrep
+        graph = torch.cuda.CUDAGraph()
+        side = torch.cuda.Stream(device=dev)
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            with torch.cuda.graph(graph, stream=side):
+                lat1.push_moments(w1, out=rec1)
+        torch.cuda.synchronize()
+        for _ in range(20):
+            graph.replay()
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(nrep):
+            graph.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        graph_us = e0.elapsed_time(e1) * 1e3 / nrep
+        nl1 = lat1.num_launches(True, x1.shape[1])
+        lat1.close()
+        out.append({"kernel": "C1 whole push, launch-bound (%d launches): direct launches vs one CUDA-graph replay" % nl1,
+                    "workload": "C1: N=%d, FODO cell | 6-64-64-6 tanh %s | drift, 3 monitors; %d pushes back to back" % (x1.shape[1], p16, nrep),
+                    "ms": graph_us * 1e-3, "us_per_push_direct": direct_us, "us_per_push_graph_replay": graph_us,
+                    "particles_per_s": x1.shape[1] / (graph_us * 1e-6)})
         # (e) C5 as BASELINE.json specifies it: N = 1e8 (2.4 GB bunch), 9 streamed-weights stages + 8 runs + 17 monitors
         if not args.n:
             desc5f, x5f = wl.config5(prec=p16, n=100_000_000)
