@@ -17,7 +17,9 @@
 // next tile's layer 0 (half 0) is issued right behind the last hidden layer, before the last layer (N = 16, into D[1]);
 // only its half 1 waits for the output read.  (Measured and dropped: the 16 output columns in the dead operand region
 // instead of D[1], so that no MMA waits for the output read: 2.40 ms against 2.20; and the next tile's first operand
-// half converted under the last hidden layer with its K-half 0 issued before the last layer: 2.42 ms.)
+// half converted under the last hidden layer with its K-half 0 issued before the last layer: 2.42 ms.  After the issuing
+// warp's waits were changed -- hb_tc_common.cuh, mbar_spin: 2.20 -> 2.05 ms -- five more re-orderings of the tile boundary and
+// of the epilogue were built, verified and measured slower: profiles/r2_issuer_codegen.md lists them with their times.)
 // Events.  The hidden accumulators of a CTA form one sequence e = 0, 1, 2, ...: tile t, layer l <= L-2, half h is
 // e = (t (L-1) + l) * 2 + h; it lives in D[h], signals DH_FULL[h], is read (DH_FREE[h]) and converted into K-half h of
 // operand region (t (L-1) + l) & 1 (A_FULL[h]).
